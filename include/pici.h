@@ -1,0 +1,183 @@
+/*
+ * pici.h - C ABI of libpici_b200: the per-GPU data-parallel hot path of SpCCL's sparse collectives
+ * (arxiv/paper_2607_04676), hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations are "PAPER.md:<line>" of the paper text plus its section / algorithm, and
+ * "SURVEY.md S8(x)" for the scope table and the readings taken where the paper is silent.
+ *
+ * ------------------------------------------------------------------------------------------------
+ * The Pici format (SIII-B)
+ *   An n-element dense buffer is viewed as T = ceil(n/4096) row-major 64x64 "virtual" tiles.
+ *   B : uint64_t[64*T]  B[64*t + c] is COLUMN c of tile t; bit r (LSB = row 0) is set iff the element
+ *                       at dense index 4096*t + 64*r + c is nonzero.  Bits for indices >= n are 0.
+ *   I : uint32_t[T+1]   I[t] = number of nonzeros in tiles 0..t-1 (exclusive prefix sum);
+ *                       I[T] = nnz of the whole buffer.
+ *   A : packed nonzero values (bit-for-bit copies), ordered tile -> column -> row.
+ *   Nonzero predicate: nz(x) := (bits(x) & ~signbit) != 0, i.e. IEEE x != 0:
+ *   +0.0 and -0.0 are zeros (never stored; -0.0 decompresses to +0.0); NaN, +-Inf, subnormals are
+ *   nonzero.  No flush-to-zero anywhere.
+ *
+ * Conventions common to every call
+ *   - All data pointers are DEVICE pointers unless the name starts with h_ (host).  `stream` is a
+ *     cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Calls only enqueue work on `stream` and return; nothing synchronises the device.  Results,
+ *     including nnz and switch flags, live in device memory.
+ *   - The caller owns every buffer.  The library never allocates, frees or retains pointers and has
+ *     no global state; it is re-entrant.  `ws` is scratch that must not be shared by calls that may
+ *     run concurrently (one workspace per stream).
+ *   - Alignment: dense, B, A, ws pointers 16-byte aligned; I 4-byte aligned.  Violations return
+ *     PICI_ERR_ALIGN.
+ *   - Sizes: B holds 64*T words and I holds T+1 entries even when n % 4096 != 0; A (and Ao) must
+ *     have capacity >= n elements - the worst case, mirroring the paper's enlarged FIFOs
+ *      - so no device-side overflow can occur.
+ *   - Limits: 0 <= n < 2^32 (I is 32-bit).  n == 0 is valid: I[0] = 0 is written.
+ *   - dtype: PICI_F32 or PICI_BF16 for compress / decompress / nnz / maybe_densify;
+ *     reductions (reduce_sd, reduce_ss, dense_add) are PICI_F32 only (PICI_ERR_DTYPE otherwise).
+ *   - Return value: PICI_OK (0) or a negative PICI_ERR_* code; pici_strerror() names it.  No call
+ *     throws, aborts or prints.
+ *   - Gating: calls that take `d_gate` run only if d_gate == NULL or *d_gate == gate_value when the
+ *     kernel starts (read on the device, no host sync); otherwise they leave every output untouched.
+ *     This is how the ring driver takes format decisions without reading flags back
+ *     (SURVEY.md S7 hard part 6).
+ */
+#ifndef PICI_H_
+#define PICI_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PICI_VERSION 100
+
+enum { PICI_F32 = 0, PICI_BF16 = 1 };
+
+enum {
+    PICI_OK = 0,
+    PICI_ERR_INVALID_ARG = -1, /* NULL pointer where one is required, n >= 2^32, bad flag          */
+    PICI_ERR_DTYPE       = -2, /* unknown dtype, or dtype not supported by this call               */
+    PICI_ERR_ALIGN       = -3, /* a pointer violates the alignment rule above                      */
+    PICI_ERR_CAPACITY    = -4, /* A_capacity / Ao_capacity < n                                     */
+    PICI_ERR_WORKSPACE   = -5, /* ws_bytes < pici_sizes(..).workspace_bytes                        */
+    PICI_ERR_CUDA        = -6  /* a CUDA runtime call or the launch failed (cudaGetLastError)      */
+};
+
+/* Message formats used by the ring entry points (the paper's per-message header carries the same
+ * fact). */
+enum { PICI_FMT_PICI = 0, PICI_FMT_DENSE = 1 };
+
+int         pici_version(void);
+const char *pici_strerror(int code);
+
+/* Sizes for an n-element buffer: number of B words (64*T), I entries (T+1), the required A capacity
+ * in ELEMENTS (n) and the scratch bytes compress / reduce_ss / nnz_dense need.  Any output pointer
+ * may be NULL.  Host-only, no CUDA call. */
+int pici_sizes(uint64_t n, int dtype, uint64_t *bitvec_words, uint64_t *index_entries,
+               uint64_t *values_capacity, uint64_t *workspace_bytes);
+
+/* a1-a3. Compress (Algorithm 1): dense[n] -> (B, I, A) in ONE pass over `dense`:
+ * mask words + tile counts (Phase 1), device-wide exclusive scan of tile counts by decoupled
+ * look-back (Phase 2; the paper scans block-locally per segment, PAPER.md:124 - here I is one global
+ * prefix, reading C9 #3), compaction staged through shared memory (Phase 3).
+ * Reads dense; writes all 64*T words of B, all T+1 entries of I and A[0 .. nnz).  ws is scratch. */
+int pici_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,
+                  uint64_t A_capacity, void *ws, uint64_t ws_bytes, void *stream);
+
+/* a4. Decompress: (B, I, A) -> dense_out[n].  EVERY element of dense_out is written
+ * (absent elements become +0.0). */
+int pici_decompress(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
+                    void *dense_out, void *stream);
+
+/* a5. reduce_sd, the scatter-add "decompression" used by reduce-scatter / all-reduce
+ * (PAPER.md:193, 219): dense_inout[i] = dense_inout[i] + a_i for every set bit, one fp32 add each;
+ * all other elements are left untouched (bit-exact, a -0.0 there survives).  fp32 only. */
+int pici_reduce_sd(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
+                   void *dense_inout, void *stream);
+
+/* a6. reduce_ss, sparse + sparse merge: O = compress(decompress(X) + decompress(Y)) without
+ * materialising a dense buffer - the fused form of the paper's "scatter-add into dense, then
+ * recompress" ring step.  o_i = x_i + y_i (an absent operand reads as +0.0) for every
+ * position where X or Y has its bit set; the predicate is RE-APPLIED to the sum, so an exact
+ * cancellation is not stored.  Outputs must not alias inputs.  fp32 only. */
+int pici_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void *Ax,
+                   const uint64_t *By, const uint32_t *Iy, const void *Ay, uint64_t n, int dtype,
+                   uint64_t *Bo, uint32_t *Io, void *Ao, uint64_t Ao_capacity,
+                   void *ws, uint64_t ws_bytes, void *stream);
+
+/* a7. nnz of a Pici buffer = I[T], copied to *d_nnz on the device. */
+int pici_nnz(const uint32_t *I, uint64_t n, uint32_t *d_nnz, void *stream);
+
+/* a7'. nnz of a dense buffer: *d_nnz = #{ i : nz(dense[i]) } (the measurement the paper lacks after
+ * a scatter-add).  ws needs 0 bytes today; pass what pici_sizes() reports. */
+int pici_nnz_dense(const void *dense, uint64_t n, int dtype, uint32_t *d_nnz, void *ws,
+                   uint64_t ws_bytes, void *stream);
+
+/* a8. maybe_densify: the sparse -> dense switch "when sparsity sigma is <= tau",
+ * taken ON THE DEVICE on the measured nnz as an integer compare (readings C9 #9/#10):
+ *   switched = (I[T] >= nnz_switch);  *d_switched = switched (int32 0/1, always written);
+ *   if switched: dense_out[n] = decompress(B, I, A); else dense_out is untouched.
+ * dense_out may be NULL: then only the flag is written (the caller already holds the dense data). */
+int pici_maybe_densify(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
+                       uint64_t nnz_switch, void *dense_out, int32_t *d_switched, void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Device-gated forms used by the host ring driver (a9).  Same arithmetic as above.
+ * ---------------------------------------------------------------------------------------------- */
+
+/* compress that runs only if *d_gate == gate_value (see "Gating"). */
+int pici_compress_gated(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,
+                        uint64_t A_capacity, void *ws, uint64_t ws_bytes, const int32_t *d_gate,
+                        int32_t gate_value, void *stream);
+
+/* reduce_ss that runs only if *d_gate == gate_value (see "Gating"). */
+int pici_reduce_ss_gated(const uint64_t *Bx, const uint32_t *Ix, const void *Ax,
+                         const uint64_t *By, const uint32_t *Iy, const void *Ay, uint64_t n, int dtype,
+                         uint64_t *Bo, uint32_t *Io, void *Ao, uint64_t Ao_capacity,
+                         void *ws, uint64_t ws_bytes, const int32_t *d_gate, int32_t gate_value,
+                         void *stream);
+
+/* maybe_densify that runs only if *d_gate == gate_value; *d_fmt_out = PICI_FMT_DENSE if switched
+ * else PICI_FMT_PICI.  When the gate is closed *d_fmt_out is left untouched.  d_fmt_out must not be
+ * the gate word itself (PICI_ERR_INVALID_ARG). */
+int pici_maybe_densify_gated(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
+                             uint64_t nnz_switch, void *dense_out, int32_t *d_fmt_out,
+                             const int32_t *d_gate, int32_t gate_value, void *stream);
+
+/* out[i] = recv[i] + local[i] in fp32 (the dense ring step once a chunk has switched, the paper's
+ * reduceCopy).  Runs only if the gate is open; then also sets *d_fmt_out (if not
+ * NULL) to PICI_FMT_DENSE.  out may alias recv or local. */
+int pici_dense_add_gated(const void *recv, const void *local, uint64_t n, int dtype, void *out,
+                         int32_t *d_fmt_out, const int32_t *d_gate, int32_t gate_value, void *stream);
+
+/* out[i] = local[i] + (bit_i ? a_i : nothing): reduce_sd with a separate output (the last
+ * reduce-scatter step writes the rank's result buffer).  out may alias local (then == reduce_sd).
+ * Runs only if the gate is open. */
+int pici_reduce_sd_out_gated(const uint64_t *B, const uint32_t *I, const void *A, const void *local,
+                             uint64_t n, int dtype, void *out, const int32_t *d_gate,
+                             int32_t gate_value, void *stream);
+
+/* decompress that runs only if the gate is open. */
+int pici_decompress_gated(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
+                          void *dense_out, const int32_t *d_gate, int32_t gate_value, void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Host-buffer forms (end-to-end path): h_* are HOST pointers (pinned for full speed), d_* device
+ * scratch owned by the caller.  These DO synchronise `stream` before returning.
+ * ---------------------------------------------------------------------------------------------- */
+
+/* h_dense[n] -> host (h_B[64T], h_I[T+1], h_A[nnz]); returns nnz in *h_nnz.  Device scratch:
+ * d_dense (n elements), d_B, d_I, d_A (capacity n), ws. */
+int pici_compress_host(const void *h_dense, uint64_t n, int dtype, uint64_t *h_B, uint32_t *h_I,
+                       void *h_A, uint64_t *h_nnz, void *d_dense, uint64_t *d_B, uint32_t *d_I,
+                       void *d_A, void *ws, uint64_t ws_bytes, void *stream);
+
+/* host (h_B, h_I, h_A[nnz]) -> h_dense_out[n]. */
+int pici_decompress_host(const uint64_t *h_B, const uint32_t *h_I, const void *h_A, uint64_t nnz,
+                         uint64_t n, int dtype, void *h_dense_out, uint64_t *d_B, uint32_t *d_I,
+                         void *d_A, void *d_dense, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PICI_H_ */

@@ -1,0 +1,43 @@
+// launch.h - internal host-side launchers (one per kernel family).  The C ABI in api.cu validates
+// arguments and calls these; nothing here is exported.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pici {
+
+struct Gate {
+    const int32_t *ptr;
+    int32_t value;
+};
+
+int num_sms();  // cached cudaDevAttrMultiProcessorCount of the current device
+
+uint64_t scan_workspace_bytes(uint64_t n);
+
+cudaError_t launch_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,
+                            void *ws, Gate g, cudaStream_t s);
+
+// mode 0: decompress (overwrite), 1: out = local + sparse (reduce_sd, out may alias local).
+// d_switch / nnz_switch: if d_switch != nullptr the kernel first evaluates switched = I[T] >= nnz_switch,
+// writes *d_switch = switched ? on_value : off_value and does nothing else unless switched.
+struct DensifyCtl {
+    int32_t *d_flag;      // nullptr = unconditional
+    uint64_t nnz_switch;
+    int32_t on_value, off_value;
+};
+cudaError_t launch_expand(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
+                          const void *local, void *out, int mode, DensifyCtl ctl, Gate g, cudaStream_t s);
+
+cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void *Ax, const uint64_t *By,
+                             const uint32_t *Iy, const void *Ay, uint64_t n, uint64_t *Bo, uint32_t *Io,
+                             void *Ao, void *ws, Gate g, cudaStream_t s);
+
+cudaError_t launch_nnz_pici(const uint32_t *I, uint64_t n, uint32_t *d_nnz, cudaStream_t s);
+cudaError_t launch_nnz_dense(const void *dense, uint64_t n, int dtype, uint32_t *d_nnz, cudaStream_t s);
+cudaError_t launch_dense_add(const void *recv, const void *local, uint64_t n, void *out, int32_t *d_fmt_out,
+                             Gate g, cudaStream_t s);
+cudaError_t launch_set_u32(uint32_t *p, uint32_t v, Gate g, cudaStream_t s);
+
+}  // namespace pici

@@ -1,0 +1,120 @@
+// misc.cu - the small kernels of the path: pici_nnz, pici_nnz_dense (the on-device
+// measurement the paper lacks after a scatter-add), the dense+dense ring step (the
+// paper's reduceCopy) and a gated 32-bit store.
+#include "launch.h"
+#include "pici_common.cuh"
+#include "../../include/pici.h"
+
+namespace pici {
+
+__global__ void set_u32_kernel(uint32_t *p, uint32_t v, const int32_t *gate, int32_t gate_value) {
+    if (gate_closed(gate, gate_value)) return;
+    *p = v;
+}
+
+cudaError_t launch_set_u32(uint32_t *p, uint32_t v, Gate g, cudaStream_t s) {
+    set_u32_kernel<<<1, 1, 0, s>>>(p, v, g.ptr, g.value);
+    return cudaGetLastError();
+}
+
+__global__ void nnz_pici_kernel(const uint32_t *__restrict__ I, uint32_t T, uint32_t *d_nnz) { *d_nnz = I[T]; }
+
+cudaError_t launch_nnz_pici(const uint32_t *I, uint64_t n, uint32_t *d_nnz, cudaStream_t s) {
+    nnz_pici_kernel<<<1, 1, 0, s>>>(I, (uint32_t)((n + kTile - 1) / kTile), d_nnz);
+    return cudaGetLastError();
+}
+
+// Count of nz(x) over a dense buffer.  128-bit loads, 4 in flight per thread; integer atomics, so the
+// result does not depend on scheduling.
+template <int DT>
+__global__ void __launch_bounds__(256) nnz_dense_kernel(const void *__restrict__ dense, uint64_t n, uint32_t *d_nnz) {
+    constexpr int kPerVec = DT == PICI_F32 ? 4 : 8;
+    const uint64_t nvec = n / kPerVec;
+    const uint4 *p = reinterpret_cast<const uint4 *>(dense);
+    uint32_t cnt = 0;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    auto count4 = [&](uint4 v) {
+        if constexpr (DT == PICI_F32) {
+            cnt += nz32(v.x) + nz32(v.y) + nz32(v.z) + nz32(v.w);
+        } else {
+            cnt += nz16lo(v.x) + nz16hi(v.x) + nz16lo(v.y) + nz16hi(v.y) + nz16lo(v.z) + nz16hi(v.z) + nz16lo(v.w) + nz16hi(v.w);
+        }
+    };
+    for (; i + 3 * stride < nvec; i += 4 * stride) {
+        uint4 a = ldg_nc_u4(p + i), b = ldg_nc_u4(p + i + stride), c = ldg_nc_u4(p + i + 2 * stride), d = ldg_nc_u4(p + i + 3 * stride);
+        count4(a); count4(b); count4(c); count4(d);
+    }
+    for (; i < nvec; i += stride) count4(ldg_nc_u4(p + i));
+    if (blockIdx.x == 0 && threadIdx.x == 0) {  // ragged tail (< one vector)
+        for (uint64_t j = nvec * kPerVec; j < n; ++j) {
+            if constexpr (DT == PICI_F32) cnt += nz32(reinterpret_cast<const uint32_t *>(dense)[j]);
+            else cnt += nz16lo(reinterpret_cast<const uint16_t *>(dense)[j]);
+        }
+    }
+    cnt = warp_sum(cnt);
+    __shared__ uint32_t part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t s = 0;
+        for (int w = 0; w < 8; ++w) s += part[w];
+        if (s) atomicAdd(d_nnz, s);
+    }
+}
+
+cudaError_t launch_nnz_dense(const void *dense, uint64_t n, int dtype, uint32_t *d_nnz, cudaStream_t s) {
+    cudaError_t e = cudaMemsetAsync(d_nnz, 0, sizeof(uint32_t), s);
+    if (e != cudaSuccess || n == 0) return e;
+    const uint64_t nvec = n / (dtype == PICI_F32 ? 4 : 8);
+    uint64_t blocks = (nvec + 256 * 4 - 1) / (256 * 4);
+    const uint64_t cap = (uint64_t)num_sms() * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks == 0) blocks = 1;
+    if (dtype == PICI_F32) nnz_dense_kernel<PICI_F32><<<(unsigned)blocks, 256, 0, s>>>(dense, n, d_nnz);
+    else nnz_dense_kernel<PICI_BF16><<<(unsigned)blocks, 256, 0, s>>>(dense, n, d_nnz);
+    return cudaGetLastError();
+}
+
+// out[i] = recv[i] + local[i], one fp32 add each, order "received + local" (C9 #7).
+__global__ void __launch_bounds__(256) dense_add_kernel(const float *recv, const float *local, uint64_t n, float *out,
+                                                        int32_t *d_fmt_out, const int32_t *gate, int32_t gate_value) {
+    if (gate_closed(gate, gate_value)) return;
+    if (d_fmt_out != nullptr && blockIdx.x == 0 && threadIdx.x == 0) *d_fmt_out = PICI_FMT_DENSE;
+    const uint64_t nvec = n / 4;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint4 *a = reinterpret_cast<const uint4 *>(recv), *b = reinterpret_cast<const uint4 *>(local);
+    uint4 *o = reinterpret_cast<uint4 *>(out);
+    auto add4 = [](uint4 x, uint4 y) {
+        uint4 r;
+        r.x = __float_as_uint(__fadd_rn(__uint_as_float(x.x), __uint_as_float(y.x)));
+        r.y = __float_as_uint(__fadd_rn(__uint_as_float(x.y), __uint_as_float(y.y)));
+        r.z = __float_as_uint(__fadd_rn(__uint_as_float(x.z), __uint_as_float(y.z)));
+        r.w = __float_as_uint(__fadd_rn(__uint_as_float(x.w), __uint_as_float(y.w)));
+        return r;
+    };
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + stride < nvec; i += 2 * stride) {
+        uint4 x0 = ldg_stream_u4(a + i), y0 = ldg_stream_u4(b + i);
+        uint4 x1 = ldg_stream_u4(a + i + stride), y1 = ldg_stream_u4(b + i + stride);
+        stg_stream_u4(o + i, add4(x0, y0));
+        stg_stream_u4(o + i + stride, add4(x1, y1));
+    }
+    for (; i < nvec; i += stride) stg_stream_u4(o + i, add4(ldg_stream_u4(a + i), ldg_stream_u4(b + i)));
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        for (uint64_t j = nvec * 4; j < n; ++j) out[j] = __fadd_rn(recv[j], local[j]);
+}
+
+cudaError_t launch_dense_add(const void *recv, const void *local, uint64_t n, void *out, int32_t *d_fmt_out, Gate g,
+                             cudaStream_t s) {
+    const uint64_t nvec = n / 4;
+    uint64_t blocks = (nvec + 256 * 2 - 1) / (256 * 2);
+    const uint64_t cap = (uint64_t)num_sms() * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks == 0) blocks = 1;
+    dense_add_kernel<<<(unsigned)blocks, 256, 0, s>>>(reinterpret_cast<const float *>(recv), reinterpret_cast<const float *>(local),
+                                                      n, reinterpret_cast<float *>(out), d_fmt_out, g.ptr, g.value);
+    return cudaGetLastError();
+}
+
+}  // namespace pici

@@ -1,0 +1,221 @@
+"""GPU parity: every C-ABI entry point of libpici_b200 against the CPU oracle, element by element,
+on the same seeded inputs (workloads.py).  Integer / byte / index outputs (B, I, A, nnz, flags) are
+bit-exact; fp32 sums are taken in the oracle's operand order so they are bit-exact too (NaN results
+compare as "is NaN").  All calls go through the ctypes binding of the C ABI.
+"""
+import numpy as np
+import pytest
+import torch
+
+import workloads as wl
+from oracle import pici_oracle as po
+
+pytestmark = pytest.mark.gpu
+
+SIZES = (1, 63, 64, 65, 4095, 4096, 4097, 8192, 8193, 3 * 4096 + 17, (1 << 20), (1 << 22) + 123)
+DENSITIES = (0.0, 0.0001, 0.01, 0.1, 0.5, 1.0)
+
+
+@pytest.fixture(scope="module")
+def pk():
+    from paper_2607_04676_b200 import pici
+    pici.lib()
+    return pici
+
+
+def _bits(t: torch.Tensor) -> np.ndarray:
+    t = t.detach().cpu().contiguous()
+    if t.dtype == torch.float32:
+        return t.view(torch.int32).numpy().view(np.uint32)
+    return t.view(torch.int16).numpy().view(np.uint16)
+
+
+def _assert_pici_equal(pk, got, want: po.Pici):
+    B, I, A = got.to_host()
+    T = po.num_tiles(want.n)
+    assert np.array_equal(I[:T + 1], want.I), "index array differs"
+    assert np.array_equal(B[:64 * T], want.B), "bitvector differs"
+    assert got.nnz_host() == want.nnz
+    assert np.array_equal(A, want.A), "packed values differ"
+
+
+def _assert_bits_equal_nan_aware(got_bits, want_bits):
+    g, w = got_bits.view(np.float32), want_bits.view(np.float32)
+    nan = np.isnan(w)
+    assert np.array_equal(np.isnan(g), nan)
+    assert np.array_equal(got_bits[~nan], want_bits[~nan])
+
+
+def _upload(pk, o: po.Pici, device="cuda"):
+    """Oracle Pici -> device Pici (inputs for decompress / reductions come from the ORACLE's encoder)."""
+    d = pk.alloc_pici(o.n, pk.F32 if o.dtype == "f32" else pk.BF16, device)
+    d.B[:o.B.size] = torch.from_numpy(o.B.view(np.int64)).to(device)
+    d.I[:o.I.size] = torch.from_numpy(o.I.view(np.int32)).to(device)
+    if o.A.size:
+        a = torch.from_numpy(o.A.view(np.int32 if o.dtype == "f32" else np.int16))
+        d.A[:o.A.size] = a.view(torch.float32 if o.dtype == "f32" else torch.bfloat16).to(device)
+    return d
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("n", SIZES)
+def test_compress_and_decompress_match_oracle(pk, n, dtype):
+    for j, dens in enumerate(DENSITIES):
+        host = wl.sparse_buffer(n, dens, seed=17 * n + j, dtype=dtype)
+        want = po.compress(_bits(host), dtype)
+        dev = host.cuda()
+        out = pk.alloc_pici(n, pk.F32 if dtype == "f32" else pk.BF16)
+        out.B.fill_(-1); out.I.fill_(-1)
+        ws = pk.alloc_workspace(n)
+        pk.compress(dev, out, ws)
+        _assert_pici_equal(pk, out, want)
+        # decompress the ORACLE's encoding on the GPU
+        back = torch.full_like(dev, 7.0)
+        pk.decompress(_upload(pk, want), back)
+        assert np.array_equal(_bits(back), po.decompress(want))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_special_values_and_negative_zero(pk, dtype):
+    n = 4096 * 2 + 100
+    sp = wl.special_values_f32()
+    host = sp.repeat((n + sp.numel() - 1) // sp.numel())[:n].contiguous()
+    if dtype == "bf16":
+        host = (host.view(torch.int32) >> 16).to(torch.int16).view(torch.bfloat16).contiguous()
+    want = po.compress(_bits(host), dtype)
+    out = pk.alloc_pici(n, pk.F32 if dtype == "f32" else pk.BF16)
+    pk.compress(host.cuda(), out, pk.alloc_workspace(n))
+    _assert_pici_equal(pk, out, want)
+    back = torch.empty_like(host, device="cuda")
+    pk.decompress(out, back)
+    assert np.array_equal(_bits(back), po.decompress(want))   # -0.0 -> +0.0, NaN payloads kept
+
+
+@pytest.mark.parametrize("n", (1, 4097, 3 * 4096 + 17, 1 << 20))
+@pytest.mark.parametrize("dens", (0.0, 0.01, 0.05, 0.3, 1.0))
+def test_reduce_sd_matches_oracle(pk, n, dens):
+    x = wl.sparse_buffer(n, dens, seed=5 + n)
+    local = wl.sparse_buffer(n, 0.5, seed=6 + n)
+    local[::7] = -0.0                               # untouched elements must keep their bits
+    xo = po.compress(_bits(x), "f32")
+    want = local.numpy().copy()
+    po.reduce_sd(xo, want)
+    xd = _upload(pk, xo)
+    got = local.cuda()
+    pk.reduce_sd(xd, got)
+    assert np.array_equal(_bits(got), want.view(np.uint32))
+    out = torch.full((n,), 3.0, device="cuda")
+    pk.reduce_sd_out(xd, local.cuda(), out)
+    assert np.array_equal(_bits(out), want.view(np.uint32))
+
+
+@pytest.mark.parametrize("n", (1, 64, 4097, 3 * 4096 + 17, 1 << 20))
+@pytest.mark.parametrize("dx,dy", ((0.0, 0.0), (0.01, 0.01), (0.0, 0.2), (0.3, 0.02), (0.6, 0.6), (1.0, 1.0)))
+def test_reduce_ss_matches_oracle(pk, n, dx, dy):
+    x = wl.sparse_buffer(n, dx, seed=11 + n)
+    y = wl.sparse_buffer(n, dy, seed=12 + n)
+    # exact cancellations: wherever both are present on a stride, y = -x (C5: the sum is NOT stored)
+    both = (x != 0) & (y != 0)
+    sel = both & (torch.arange(n) % 3 == 0)
+    y = torch.where(sel, -x, y)
+    xo, yo = po.compress(_bits(x), "f32"), po.compress(_bits(y), "f32")
+    want = po.reduce_ss(xo, yo)
+    out = pk.alloc_pici(n, pk.F32)
+    out.B.fill_(-1); out.I.fill_(-1)
+    pk.reduce_ss(_upload(pk, xo), _upload(pk, yo), out, pk.alloc_workspace(n))
+    _assert_pici_equal(pk, out, want)
+
+
+def test_reduce_ss_special_values(pk):
+    n = 4096 + 50
+    sp = wl.special_values_f32()
+    x = sp.repeat((n + sp.numel() - 1) // sp.numel())[:n].contiguous()
+    y = torch.roll(x, 5).contiguous()
+    xo, yo = po.compress(_bits(x), "f32"), po.compress(_bits(y), "f32")
+    want = po.reduce_ss(xo, yo)
+    out = pk.alloc_pici(n, pk.F32)
+    pk.reduce_ss(_upload(pk, xo), _upload(pk, yo), out, pk.alloc_workspace(n))
+    B, I, A = out.to_host()
+    assert np.array_equal(B[:want.B.size], want.B) and np.array_equal(I[:want.I.size], want.I)
+    _assert_bits_equal_nan_aware(A, want.A)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("n", (1, 4097, (1 << 20) + 3))
+def test_nnz_and_maybe_densify(pk, n, dtype):
+    host = wl.sparse_buffer(n, 0.03, seed=n, dtype=dtype)
+    want = po.compress(_bits(host), dtype)
+    dev = host.cuda()
+    cnt = torch.full((1,), -1, dtype=torch.int32, device="cuda")
+    pk.nnz_dense(dev, cnt)
+    assert int(cnt.item()) == want.nnz == po.nnz_dense(_bits(host), dtype)
+    xd = _upload(pk, want)
+    cnt.fill_(-1)
+    pk.nnz(xd, cnt)
+    assert int(cnt.item()) == po.nnz_pici(want)
+    for nnz_switch in (0, want.nnz, want.nnz + 1, n + 1):
+        flag = torch.full((1,), -7, dtype=torch.int32, device="cuda")
+        out = torch.full_like(dev, 9.0)
+        pk.maybe_densify(xd, nnz_switch, out, flag)
+        switched = want.nnz >= nnz_switch
+        assert int(flag.item()) == int(switched)
+        if switched:
+            assert np.array_equal(_bits(out), po.decompress(want))
+        else:
+            assert bool((out == 9.0).all())        # untouched
+
+
+def test_gates_leave_outputs_untouched(pk):
+    n = 8192
+    host = wl.sparse_buffer(n, 0.1, seed=3)
+    dev = host.cuda()
+    gate = torch.tensor([1], dtype=torch.int32, device="cuda")
+    out = pk.alloc_pici(n, pk.F32)
+    out.B.fill_(-1); out.I.fill_(-1)
+    ws = pk.alloc_workspace(n)
+    pk.compress(dev, out, ws, gate=gate, gate_value=0)          # closed
+    assert bool((out.I == -1).all()) and bool((out.B == -1).all())
+    pk.compress(dev, out, ws, gate=gate, gate_value=1)          # open
+    _assert_pici_equal(pk, out, po.compress(_bits(host), "f32"))
+    d = torch.full((n,), 5.0, device="cuda")
+    pk.decompress(out, d, gate=gate, gate_value=0)
+    assert bool((d == 5.0).all())
+    pk.dense_add(dev, dev, d, gate=gate, gate_value=0)
+    assert bool((d == 5.0).all())
+    pk.dense_add(dev, dev, d, gate=gate, gate_value=1)
+    assert np.array_equal(_bits(d), po.dense_add(host.numpy(), host.numpy()).view(np.uint32))
+
+
+def test_errors_are_codes_not_crashes(pk):
+    n = 4096
+    dev = torch.zeros(n, device="cuda")
+    out = pk.alloc_pici(n, pk.F32)
+    ws = pk.alloc_workspace(n)
+    with pytest.raises(pk.PiciError) as e:
+        pk.compress(dev, out, ws[:16])
+    assert e.value.code == -5
+    with pytest.raises(pk.PiciError) as e:
+        pk.compress(torch.zeros(n + 1, device="cuda")[1:], out, ws)       # 4-byte offset pointer
+    assert e.value.code == -3
+    small = pk.alloc_pici(n, pk.F32)
+    small.A = small.A[: n // 2]
+    with pytest.raises(pk.PiciError) as e:
+        pk.compress(dev, small, ws)
+    assert e.value.code == -4
+
+
+def test_host_end_to_end_forms(pk):
+    n = (1 << 18) + 77
+    host = wl.sparse_buffer(n, 0.02, seed=9).pin_memory()
+    want = po.compress(_bits(host), "f32")
+    h = pk.alloc_host_pici(n, pk.F32)
+    scratch = pk.alloc_pici(n, pk.F32)
+    d_dense = torch.empty(n, device="cuda")
+    pk.compress_host(host, h, d_dense, scratch, pk.alloc_workspace(n))
+    assert h.nnz == want.nnz
+    assert np.array_equal(h.I.numpy().view(np.uint32)[:want.I.size], want.I)
+    assert np.array_equal(h.B.numpy().view(np.uint64)[:want.B.size], want.B)
+    assert np.array_equal(_bits(h.A[:h.nnz]), want.A)
+    back = torch.empty(n).pin_memory()
+    pk.decompress_host(h, back, scratch, d_dense)
+    assert np.array_equal(_bits(back), po.decompress(want))
