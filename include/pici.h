@@ -157,6 +157,11 @@ int pici_reduce_sd_out_gated(const uint64_t *B, const uint32_t *I, const void *A
                              uint64_t n, int dtype, void *out, const int32_t *d_gate,
                              int32_t gate_value, void *stream);
 
+/* dst[i] = src[i] (bit copy of n elements) if the gate is open: a DENSE message landing in its
+ * all-gather slot.  src and dst must not overlap. */
+int pici_dense_copy_gated(const void *src, void *dst, uint64_t n, int dtype, const int32_t *d_gate,
+                          int32_t gate_value, void *stream);
+
 /* decompress that runs only if the gate is open. */
 int pici_decompress_gated(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
                           void *dense_out, const int32_t *d_gate, int32_t gate_value, void *stream);

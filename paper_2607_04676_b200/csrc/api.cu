@@ -180,6 +180,15 @@ int pici_dense_add_gated(const void *recv, const void *local, uint64_t n, int dt
                                     static_cast<cudaStream_t>(stream)));
 }
 
+int pici_dense_copy_gated(const void *src, void *dst, uint64_t n, int dtype, const int32_t *d_gate, int32_t gate_value,
+                          void *stream) {
+    if (bad_dtype(dtype)) return PICI_ERR_DTYPE;
+    if (n >= kMaxN || (n != 0 && (src == nullptr || dst == nullptr))) return PICI_ERR_INVALID_ARG;
+    if (!aligned(src, 16) || !aligned(dst, 16)) return PICI_ERR_ALIGN;
+    if (n == 0) return PICI_OK;
+    return cuda_rc(launch_dense_copy(src, dst, n * esize(dtype), Gate{d_gate, gate_value}, static_cast<cudaStream_t>(stream)));
+}
+
 int pici_compress_host(const void *h_dense, uint64_t n, int dtype, uint64_t *h_B, uint32_t *h_I, void *h_A,
                        uint64_t *h_nnz, void *d_dense, uint64_t *d_B, uint32_t *d_I, void *d_A, void *ws,
                        uint64_t ws_bytes, void *stream) {

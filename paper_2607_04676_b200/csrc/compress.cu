@@ -49,51 +49,76 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
     const int warp = threadIdx.x >> 5;
     Elem *stage = reinterpret_cast<Elem *>(smem_raw) + warp * kTile;
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
+    if (blockIdx.x == 0) {  // block 0 is the Phase-2 scanner
+        if (warp == 0) scanner_warp(status, T, I, lane);
+        return;
+    }
     const uint32_t Tfull = (uint32_t)(n / kTile);
     Elem *Aout = reinterpret_cast<Elem *>(A);
 
-    uint32_t t = next_ticket(ticket, lane);
-    while (t < T) {
-        uint32_t t_next = 0;  // prefetch the next ticket: its latency hides behind this tile
-        if (lane == 0) t_next = atomicAdd(ticket, 1u);
-
-        const size_t base = (size_t)t * kTile;
-        uint32_t v[Cfg::kRegs];
-
-        // ---- load the whole tile into registers (row r of the tile = one coalesced request) -----
-        if (t < Tfull) {
-            if constexpr (DT == PICI_F32) {
-                const uint2 *p = reinterpret_cast<const uint2 *>(reinterpret_cast<const uint32_t *>(dense) + base) + lane;
+    // Loads of a full tile: row r of the tile is one coalesced request; all 64 are issued back to back.
+    auto load_full = [&](uint32_t tt, uint32_t (&v)[Cfg::kRegs]) {
+        const size_t base = (size_t)tt * kTile;
+        if constexpr (DT == PICI_F32) {
+            const uint2 *p = reinterpret_cast<const uint2 *>(reinterpret_cast<const uint32_t *>(dense) + base) + lane;
 #pragma unroll
-                for (int r = 0; r < kSide; ++r) {
-                    uint2 x = ldg_stream_u2(p + 32 * r);
-                    v[2 * r] = x.x;
-                    v[2 * r + 1] = x.y;
-                }
-            } else {
-                const uint32_t *p = reinterpret_cast<const uint32_t *>(reinterpret_cast<const uint16_t *>(dense) + base) + lane;
-#pragma unroll
-                for (int r = 0; r < kSide; ++r) v[r] = ldg_stream_u32(p + 32 * r);
+            for (int r = 0; r < kSide; ++r) {
+                uint2 x = ldg_stream_u2(p + 32 * r);
+                v[2 * r] = x.x;
+                v[2 * r + 1] = x.y;
             }
-        } else {  // ragged last tile: elements >= n are virtual zeros (C9 #4); pad through the stage
-            const Elem *p = reinterpret_cast<const Elem *>(dense);
-            for (int i = lane; i < kTile; i += 32) stage[i] = (base + i < n) ? p[base + i] : (Elem)0;
-            __syncwarp();
-            if constexpr (DT == PICI_F32) {
-                const uint2 *q = reinterpret_cast<const uint2 *>(stage) + lane;
+        } else {
+            const uint32_t *p = reinterpret_cast<const uint32_t *>(reinterpret_cast<const uint16_t *>(dense) + base) + lane;
 #pragma unroll
-                for (int r = 0; r < kSide; ++r) {
-                    uint2 x = q[32 * r];
-                    v[2 * r] = x.x;
-                    v[2 * r + 1] = x.y;
-                }
-            } else {
-                const uint32_t *q = reinterpret_cast<const uint32_t *>(stage) + lane;
-#pragma unroll
-                for (int r = 0; r < kSide; ++r) v[r] = q[32 * r];
-            }
-            __syncwarp();
+            for (int r = 0; r < kSide; ++r) v[r] = ldg_stream_u32(p + 32 * r);
         }
+    };
+    // Ragged last tile: elements >= n are virtual zeros (C9 #4); padded through the stage.
+    auto load_ragged = [&](uint32_t tt, uint32_t (&v)[Cfg::kRegs]) {
+        const size_t base = (size_t)tt * kTile;
+        const Elem *p = reinterpret_cast<const Elem *>(dense);
+        for (int i = lane; i < kTile; i += 32) stage[i] = (base + i < n) ? p[base + i] : (Elem)0;
+        __syncwarp();
+        if constexpr (DT == PICI_F32) {
+            const uint2 *q = reinterpret_cast<const uint2 *>(stage) + lane;
+#pragma unroll
+            for (int r = 0; r < kSide; ++r) {
+                uint2 x = q[32 * r];
+                v[2 * r] = x.x;
+                v[2 * r + 1] = x.y;
+            }
+        } else {
+            const uint32_t *q = reinterpret_cast<const uint32_t *>(stage) + lane;
+#pragma unroll
+            for (int r = 0; r < kSide; ++r) v[r] = q[32 * r];
+        }
+        __syncwarp();
+    };
+
+    uint32_t v[Cfg::kRegs];
+    uint32_t t = next_ticket(ticket, lane);
+    if (t < Tfull) load_full(t, v);
+    else if (t < T) load_ragged(t, v);
+
+    // Per-warp software pipeline.  A tile's count is published as soon as its data has arrived and
+    // Phase 1 is done; the wait for its prefix (and the flush of its compacted values) is deferred
+    // until AFTER the next tile's count has been published, so no ticket is ever held across a wait
+    // and the scanner sees counts in near ticket order.
+    bool pending = false;       // stage holds the compacted values of tile pt, not yet flushed
+    uint32_t pt = 0, pnnz = 0;
+    auto flush_pending = [&]() {
+        if (pending) {
+            const uint32_t excl = wait_prefix(status, pt, lane);
+            Elem *dst = Aout + excl;
+            for (uint32_t i = lane; i < pnnz; i += 32) dst[i] = stage[i];
+            __syncwarp();
+            pending = false;
+        }
+    };
+
+    while (t < T) {
+        uint32_t t_next = 0;  // next ticket: its latency hides behind this tile
+        if (lane == 0) t_next = atomicAdd(ticket, 1u);
 
         // ---- Phase 1: column words (bit r <-> row r) and counts --------------------------------
         uint32_t w0lo = 0, w0hi = 0, w1lo = 0, w1hi = 0;
@@ -116,8 +141,8 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
         const uint32_t incl = warp_incl_scan(cnt0 + cnt1, lane);
         const uint32_t tile_nnz = __shfl_sync(kFull, incl, 31);
 
-        // ---- Phase 2a: publish this tile's count for the device-wide scan -----------------------
-        publish_aggregate(status, t, tile_nnz, lane);
+        // ---- Phase 2: publish this tile's count; the scanner warp turns it into I[t] -------------
+        publish_count(status, t, tile_nnz, lane);
 
         // B: lane l holds words 2l, 2l+1 -> one 16-byte store per lane, 512 contiguous bytes per warp
         {
@@ -126,6 +151,9 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
             w.y = ((uint64_t)w1hi << 32) | w1lo;
             reinterpret_cast<ulonglong2 *>(B + (size_t)t * kSide)[lane] = w;
         }
+
+        // ---- Phase 3b of the PREVIOUS tile: its prefix has had a whole iteration to arrive --------
+        flush_pending();
 
         // ---- Phase 3a: compact into the warp's stage (tile-local offsets; order: column, row) ---
         {
@@ -147,24 +175,21 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
                 }
             }
         }
-
-        // ---- Phase 2b: exclusive prefix over all earlier tiles = I[t] ---------------------------
-        const uint32_t excl = lookback_exclusive(status, t, tile_nnz, lane);
-        if (lane == 0) {
-            I[t] = excl;
-            if (t == T - 1) I[T] = excl + tile_nnz;  // trailing entry = total nnz
-        }
         __syncwarp();
+        pending = true;
+        pt = t;
+        pnnz = tile_nnz;
 
-        // ---- Phase 3b: coalesced copy stage -> A[I[t] ...) ---------------------------------------
-        {
-            Elem *dst = Aout + excl;
-            for (uint32_t i = lane; i < tile_nnz; i += 32) dst[i] = stage[i];
+        const uint32_t tn = __shfl_sync(kFull, t_next, 0);
+        if (tn < Tfull) {
+            load_full(tn, v);
+        } else if (tn < T) {  // the ragged tile is padded through the stage: flush first
+            flush_pending();
+            load_ragged(tn, v);
         }
-        __syncwarp();
-
-        t = __shfl_sync(kFull, t_next, 0);
+        t = tn;
     }
+    flush_pending();
 }
 
 int num_sms() {
@@ -199,8 +224,8 @@ static cudaError_t launch_compress_t(const void *dense, uint64_t n, uint64_t *B,
     }
     cudaError_t e = cudaMemsetAsync(ws, 0, scan_workspace_bytes(n), s);
     if (e != cudaSuccess) return e;
-    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
-    const uint64_t cap = (uint64_t)num_sms() * Cfg::kMinBlocks;
+    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps + 1;  // + the scanner block
+    const uint64_t cap = (uint64_t)num_sms() * Cfg::kMinBlocks;           // the whole grid is resident
     if (blocks > cap) blocks = cap;
     uint32_t *ticket = reinterpret_cast<uint32_t *>(ws);
     uint64_t *status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);

@@ -38,6 +38,7 @@ cudaError_t launch_nnz_pici(const uint32_t *I, uint64_t n, uint32_t *d_nnz, cuda
 cudaError_t launch_nnz_dense(const void *dense, uint64_t n, int dtype, uint32_t *d_nnz, cudaStream_t s);
 cudaError_t launch_dense_add(const void *recv, const void *local, uint64_t n, void *out, int32_t *d_fmt_out,
                              Gate g, cudaStream_t s);
+cudaError_t launch_dense_copy(const void *src, void *dst, uint64_t nbytes, Gate g, cudaStream_t s);
 cudaError_t launch_set_u32(uint32_t *p, uint32_t v, Gate g, cudaStream_t s);
 
 }  // namespace pici

@@ -37,6 +37,10 @@ reduce_ss_kernel(const uint64_t *__restrict__ Bx, const uint32_t *__restrict__ I
     uint32_t *sx = so + kTile;
     uint32_t *sy = sx + kMergePass;
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
+    if (blockIdx.x == 0) {  // block 0 is the Phase-2 scanner
+        if (warp == 0) scanner_warp(status, T, Io, lane);
+        return;
+    }
 
     uint32_t t = next_ticket(ticket, lane);
     while (t < T) {
@@ -100,17 +104,13 @@ reduce_ss_kernel(const uint64_t *__restrict__ Bx, const uint32_t *__restrict__ I
         const uint32_t n0 = q01 & 0xFFFFu, n1 = q01 >> 16, n2 = q23 & 0xFFFFu, n3 = q23 >> 16;
         const uint32_t tile_nnz = n0 + n1 + n2 + n3;
 
-        publish_aggregate(status, t, tile_nnz, lane);
+        publish_count(status, t, tile_nnz, lane);
 
         uint32_t *Bow = reinterpret_cast<uint32_t *>(Bo + (size_t)t * kSide);
 #pragma unroll
         for (int p = 0; p < 4; ++p) Bow[32 * p + lane] = wo[p];
 
-        const uint32_t excl = lookback_exclusive(status, t, tile_nnz, lane);
-        if (lane == 0) {
-            Io[t] = excl;
-            if (t == T - 1) Io[T] = excl + tile_nnz;
-        }
+        const uint32_t excl = wait_prefix(status, t, lane);
 
         uint32_t *dst = Ao + excl;
         if (tile_nnz == cand_base) {  // no cancellation anywhere in the tile: the stage is already packed
@@ -143,8 +143,8 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
     cudaError_t e = cudaMemsetAsync(ws, 0, scan_workspace_bytes(n), s);
     if (e != cudaSuccess) return e;
     const uint64_t per_sm = (227u * 1024u) / (smem + 1024);
-    uint64_t blocks = (T + kMergeWarps - 1) / kMergeWarps;
-    const uint64_t cap = (uint64_t)num_sms() * per_sm;
+    uint64_t blocks = (T + kMergeWarps - 1) / kMergeWarps + 1;  // + the scanner block
+    const uint64_t cap = (uint64_t)num_sms() * per_sm;             // the whole grid is resident
     if (blocks > cap) blocks = cap;
     uint32_t *ticket = reinterpret_cast<uint32_t *>(ws);
     uint64_t *status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);

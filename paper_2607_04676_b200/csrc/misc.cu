@@ -117,4 +117,38 @@ cudaError_t launch_dense_add(const void *recv, const void *local, uint64_t n, vo
     return cudaGetLastError();
 }
 
+// dst[i] = src[i] (bit copy), gated: a dense message landing in its all-gather slot.
+__global__ void __launch_bounds__(256) dense_copy_kernel(const uint4 *src, uint4 *dst, uint64_t nbytes, const int32_t *gate,
+                                                         int32_t gate_value) {
+    if (gate_closed(gate, gate_value)) return;
+    const uint64_t nvec = nbytes / 16;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3 * stride < nvec; i += 4 * stride) {
+        uint4 a = ldg_stream_u4(src + i), b = ldg_stream_u4(src + i + stride), c = ldg_stream_u4(src + i + 2 * stride),
+              d = ldg_stream_u4(src + i + 3 * stride);
+        stg_stream_u4(dst + i, a);
+        stg_stream_u4(dst + i + stride, b);
+        stg_stream_u4(dst + i + 2 * stride, c);
+        stg_stream_u4(dst + i + 3 * stride, d);
+    }
+    for (; i < nvec; i += stride) stg_stream_u4(dst + i, ldg_stream_u4(src + i));
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        const unsigned char *s8 = reinterpret_cast<const unsigned char *>(src);
+        unsigned char *d8 = reinterpret_cast<unsigned char *>(dst);
+        for (uint64_t j = nvec * 16; j < nbytes; ++j) d8[j] = s8[j];
+    }
+}
+
+cudaError_t launch_dense_copy(const void *src, void *dst, uint64_t nbytes, Gate g, cudaStream_t s) {
+    const uint64_t nvec = nbytes / 16;
+    uint64_t blocks = (nvec + 256 * 4 - 1) / (256 * 4);
+    const uint64_t cap = (uint64_t)num_sms() * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks == 0) blocks = 1;
+    dense_copy_kernel<<<(unsigned)blocks, 256, 0, s>>>(reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), nbytes,
+                                                       g.ptr, g.value);
+    return cudaGetLastError();
+}
+
 }  // namespace pici

@@ -76,14 +76,24 @@ __device__ __forceinline__ bool gate_closed(const int32_t *gate, int32_t gate_va
     return gate != nullptr && *reinterpret_cast<const volatile int32_t *>(gate) != gate_value;
 }
 
-// ---- single-pass device-wide exclusive scan of per-tile counts: decoupled look-back ------------
-// One 64-bit status word per tile: high 32 bits = flag, low 32 bits = value.  Flag and value travel
-// in ONE 64-bit access, so relaxed gpu-scope accesses are sufficient (no other data is published
-// through the flag).  Workspace header word 0 is the dynamic tile ticket: a warp only ever waits on
-// tiles with a SMALLER ticket, all of which are already owned by running warps, so forward progress
-// does not depend on how many CTAs are co-resident.
-constexpr uint64_t kStEmpty = 0, kStAggregate = 1, kStPrefix = 2;
+// ---- single-pass device-wide exclusive scan of per-tile counts (Phase 2) ------------------------
+// One 64-bit status word per tile: high 32 bits = flag, low 32 bits = value; flag and value travel in
+// ONE 64-bit access, so relaxed gpu-scope accesses suffice (nothing else is published through it).
+//
+// Decoupled look-back, with the look-back itself decoupled from the workers: every worker warp only
+// PUBLISHES its tile count (flag kStCount) and later waits on its OWN word; one dedicated scanner warp
+// (block 0) walks the status array in tile order, kScanRows*32 words per round, and replaces each
+// count by the tile's exclusive prefix (flag kStPrefix), writing I[] as it goes.  The scan is
+// ~T additions in total, so one warp keeps up with tiles retiring at HBM speed, and the polling
+// traffic is one word per waiting warp instead of a 32-word window per warp.
+// Tiles are handed out by a dynamic ticket, so every tile below the highest ticket is owned by a
+// resident warp; the scanner block is block 0 of a grid that is sized to be fully resident.
+constexpr uint64_t kStEmpty = 0, kStCount = 1, kStPrefix = 2;
 constexpr int kWsHeaderBytes = 128;
+#ifndef PICI_SCAN_ROWS
+#define PICI_SCAN_ROWS 4
+#endif
+constexpr int kScanRows = PICI_SCAN_ROWS;
 
 __device__ __forceinline__ uint64_t ld_status(const uint64_t *p) {
     uint64_t v;
@@ -95,49 +105,72 @@ __device__ __forceinline__ void st_status(uint64_t *p, uint64_t flag, uint32_t v
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-// Warp-collective, step 1: make tile t's count visible to its successors as early as possible
-// (tile 0 publishes its inclusive prefix straight away).
-__device__ __forceinline__ void publish_aggregate(uint64_t *status, uint32_t t, uint32_t count, int lane) {
-    if (lane == 0) st_status(status + t, t == 0 ? kStPrefix : kStAggregate, count);
+// Worker, step 1 (warp-collective): make tile t's count visible to the scanner.
+__device__ __forceinline__ void publish_count(uint64_t *status, uint32_t t, uint32_t count, int lane) {
+    if (lane == 0) st_status(status + t, kStCount, count);
 }
 
-// Warp-collective, step 2 (after publish_aggregate): returns the exclusive prefix (sum of the counts
-// of tiles 0..t-1) and publishes tile t's inclusive prefix.  All 32 lanes call it with the same
-// arguments.
-__device__ __forceinline__ uint32_t lookback_exclusive(uint64_t *status, uint32_t t, uint32_t count,
-                                                       int lane) {
-    if (t == 0) return 0;
+// Worker, step 2 (warp-collective): the exclusive prefix of tile t (sum of the counts of tiles 0..t-1).
+__device__ __forceinline__ uint32_t wait_prefix(const uint64_t *status, uint32_t t, int lane) {
     uint32_t excl = 0;
-    int64_t pos = (int64_t)t - 1;  // nearest predecessor examined by lane 0
-    for (;;) {
-        const int64_t idx = pos - lane;
-        uint32_t sum = 0;
-        bool found_prefix = false;
-        for (;;) {
-            uint64_t s = (idx >= 0) ? ld_status(status + idx) : (kStPrefix << 32);
-            const uint32_t flag = (uint32_t)(s >> 32);
-            const unsigned ready = __ballot_sync(kFull, flag != (uint32_t)kStEmpty);
-            const unsigned pref = __ballot_sync(kFull, flag == (uint32_t)kStPrefix);
-            if (pref != 0) {
-                const int first = __ffs(pref) - 1;  // nearest predecessor that carries a prefix
-                const unsigned need = (first == 31) ? kFull : ((2u << first) - 1u);
-                if ((ready & need) == need) {
-                    sum = warp_sum(lane <= first ? (uint32_t)s : 0u);
-                    found_prefix = true;
-                    break;
-                }
-            } else if (ready == kFull) {
-                sum = warp_sum((uint32_t)s);
-                break;
-            }
-            __nanosleep(32);
+    if (lane == 0) {
+        uint64_t s = ld_status(status + t);
+        unsigned ns = 20;
+        while ((uint32_t)(s >> 32) != (uint32_t)kStPrefix) {
+            __nanosleep(ns);
+            if (ns < 160) ns += ns;
+            s = ld_status(status + t);
         }
-        excl += sum;
-        if (found_prefix) break;
-        pos -= 32;
+        excl = (uint32_t)s;
     }
-    if (lane == 0) st_status(status + t, kStPrefix, excl + count);
-    return excl;
+    return __shfl_sync(kFull, excl, 0);
+}
+
+// The scanner warp.  Writes I[0..T] (I[T] = total nnz).
+__device__ __forceinline__ void scanner_warp(uint64_t *status, uint32_t T, uint32_t *__restrict__ I, int lane) {
+    uint32_t pos = 0, run = 0;
+    unsigned ns = 20;
+    while (pos < T) {
+        uint64_t st[kScanRows];
+#pragma unroll
+        for (int j = 0; j < kScanRows; ++j) {
+            const uint32_t idx = pos + 32 * j + lane;
+            st[j] = idx < T ? ld_status(status + idx) : 0ull;
+        }
+        uint32_t nready = 0;
+        bool open = true;
+#pragma unroll
+        for (int j = 0; j < kScanRows; ++j) {
+            const unsigned m = __ballot_sync(kFull, (uint32_t)(st[j] >> 32) == (uint32_t)kStCount);
+            if (open) {
+                const uint32_t lead = (m == kFull) ? 32u : (uint32_t)(__ffs(~m) - 1);
+                nready += lead;
+                open = (lead == 32u);
+            }
+        }
+        if (nready == 0) {
+            __nanosleep(ns);
+            if (ns < 80) ns += ns;
+            continue;
+        }
+        ns = 20;
+#pragma unroll
+        for (int j = 0; j < kScanRows; ++j) {
+            if (32u * j < nready) {  // warp-uniform
+                const uint32_t k = 32 * j + lane;
+                const uint32_t c = k < nready ? (uint32_t)st[j] : 0u;
+                const uint32_t incl = warp_incl_scan(c, lane);
+                if (k < nready) {
+                    const uint32_t excl = run + incl - c;
+                    st_status(status + pos + k, kStPrefix, excl);
+                    I[pos + k] = excl;
+                }
+                run += __shfl_sync(kFull, incl, 31);
+            }
+        }
+        pos += nready;
+    }
+    if (lane == 0) I[T] = run;
 }
 
 // Dynamic tile ticket (one atomic per tile, issued by lane 0 and broadcast).

@@ -25,7 +25,7 @@ EXPORTS = (
     "pici_version", "pici_strerror", "pici_sizes", "pici_compress", "pici_decompress", "pici_reduce_sd",
     "pici_reduce_ss", "pici_nnz", "pici_nnz_dense", "pici_maybe_densify", "pici_compress_gated",
     "pici_reduce_ss_gated", "pici_maybe_densify_gated", "pici_dense_add_gated", "pici_reduce_sd_out_gated",
-    "pici_decompress_gated", "pici_compress_host", "pici_decompress_host",
+    "pici_decompress_gated", "pici_dense_copy_gated", "pici_compress_host", "pici_decompress_host",
 )
 
 _lib = None
@@ -65,6 +65,7 @@ def lib() -> ctypes.CDLL:
             "pici_maybe_densify": ([p, p, p, u64, ci, u64, p, p, p], ci),
             "pici_maybe_densify_gated": ([p, p, p, u64, ci, u64, p, p, p, i32, p], ci),
             "pici_dense_add_gated": ([p, p, u64, ci, p, p, p, i32, p], ci),
+            "pici_dense_copy_gated": ([p, p, u64, ci, p, i32, p], ci),
             "pici_compress_host": ([p, u64, ci, p, p, p, p, p, p, p, p, p, u64, p], ci),
             "pici_decompress_host": ([p, p, p, u64, u64, ci, p, p, p, p, p, p], ci),
         }
@@ -247,6 +248,14 @@ def dense_add(recv: torch.Tensor, local: torch.Tensor, out: torch.Tensor, d_fmt_
     _check(lib().pici_dense_add_gated(_p(recv), _p(local), out.numel(), _DT[out.dtype], _p(out), _p(d_fmt_out),
                                       _p(gate), gate_value, _stream(stream)), "pici_dense_add_gated")
     return out
+
+
+def dense_copy(src: torch.Tensor, dst: torch.Tensor, stream=None, gate=None, gate_value: int = 0) -> torch.Tensor:
+    _dev(src, dst, gate)
+    assert src.numel() == dst.numel() and src.dtype == dst.dtype and src.is_contiguous() and dst.is_contiguous()
+    _check(lib().pici_dense_copy_gated(_p(src), _p(dst), dst.numel(), _DT[dst.dtype], _p(gate), gate_value,
+                                       _stream(stream)), "pici_dense_copy_gated")
+    return dst
 
 
 @dataclass
