@@ -1,0 +1,478 @@
+#!/usr/bin/env python
+"""bench.py - the Pici hot path on B200: one JSON line (contract in the task statement).
+
+A STEP is one pass of the whole hot path over one batch of synthetic input of
+BASELINE.json configs[1] (N = 2^28 single buffer, fp32, unstructured Bernoulli sparsity, N(0,1) values):
+
+    compress(X) -> PX ; compress(Y) -> PY          a1-a3   (X, Y: seeds 0 and 1 of the config)
+    reduce_ss(PX, PY) -> PO                        a6      sparse + sparse merge
+    nnz(PO)                                        a7      on-device count
+    maybe_densify(PO, nnz_switch = 0) -> D         a8 + a4 the switch is taken: a full decompress
+    reduce_sd(PX, D)                               a5      scatter-add into the dense buffer
+
+`value` = dense-equivalent GB/s = (5 buffers of N*s bytes handled per step) * K / time, inputs resident in
+HBM.  `e2e` = the same metric through the C ABI's HOST-buffer calls (pici_compress_host +
+pici_decompress_host, pinned host memory, copies inside the timed region): 2 buffers of N*s per step.
+`roofline` = the dominant kernel (largest share of the timed region), algorithmic bytes (DESIGN.md
+"Algorithmic bytes") / its CUDA-event duration measured inside the timed region, against the measured
+HBM copy peak of MEASURED_PEAKS.json.  `sweep` = every kernel at every sparsity of the config (fp32 and
+bf16), timed alone with CUDA events after the K steps.  `cpu_baseline` = oracle/ (single-threaded C,
+as it stands) on a bounded sample of the same workload, on this box's host cores.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--sparsity 0.99] [--no-sweep]
+    python bench.py --impl reference ...     # the oracle timed on the host cores (same metric)
+Under torchrun (N > 1) every rank runs the same per-GPU workload on its own GPU (weak scaling; the path
+has no data-path collective on one node: SURVEY.md S8(e) "replicas only"), time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+import workloads as wl  # noqa: E402
+
+METRIC = "Pici compress/decompress/merge GB/s (dense-equiv) and % of B200 HBM peak vs sparsity"
+UNIT = "GB/s (dense-equivalent)"
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+OPS_PER_STEP = 5                   # N-element buffers handled per step (2 compress, merge, densify, scatter-add)
+TILE = 4096
+
+
+def measured_peak() -> tuple[float, str]:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            with open(p) as f:
+                return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy burst)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic() -> dict:
+    """Per-launch DRAM bytes of each kernel from the committed ncu --set full capture (text)."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f)
+    return {}
+
+
+# ---------------------------------------------------------------------------------------------------
+# algorithmic bytes; n multiple of 4096 here
+# ---------------------------------------------------------------------------------------------------
+def meta_bytes(n: int) -> int:
+    T = (n + TILE - 1) // TILE
+    return 8 * 64 * T + 4 * (T + 1)
+
+
+def bytes_compress(n, s, nnz):          # read dense, write B + I + A
+    return n * s + meta_bytes(n) + s * nnz
+
+
+def bytes_decompress(n, s, nnz):        # read B + I + A, write dense
+    return n * s + meta_bytes(n) + s * nnz
+
+
+def bytes_reduce_ss(n, nx, ny, no):     # read 2 x (B, I, A), write (B, I, A)
+    return 3 * meta_bytes(n) + 4 * (nx + ny + no)
+
+
+def bytes_reduce_sd(n, nnz, touched_sectors=None):
+    """Sparse operand + the cheaper of (a) streaming the dense buffer through (read + write n*4) and
+    (b) read-modify-write of only the touched 32-byte sectors (2 x 32 B each)."""
+    stream = 8 * n
+    if touched_sectors is None:
+        return meta_bytes(n) + 4 * nnz + stream
+    return meta_bytes(n) + 4 * nnz + min(stream, 64 * touched_sectors)
+
+
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for _, r in self.rows]
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except Exception:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores, same metric/config/unit."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    import numpy as np
+    from oracle import pici_oracle as po
+    n = args.ref_n
+    d = 1.0 - args.sparsity
+    x = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 0)).numpy()
+    y = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 1)).numpy()
+
+    def step():
+        px = po.compress(x.view(np.uint32), "f32")
+        py = po.compress(y.view(np.uint32), "f32")
+        pz = po.reduce_ss(px, py)
+        po.nnz_pici(pz)
+        dense = np.empty(n, np.uint32)
+        po.maybe_densify(pz, 0, dense)
+        po.reduce_sd(px, dense.view(np.float32))
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    val = OPS_PER_STEP * n * 4 * args.steps / dt / 1e9
+    sample = f"first-principles sample: N=2^{n.bit_length() - 1} elements of the same recipe per step (full workload N=2^28)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"configs[1] Pici hot path, fp32, sparsity {args.sparsity}, seeds 0/1; oracle on host cores",
+                   "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "host_cores_available": os.cpu_count()},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+class HotPath:
+    """Buffers + the step of the hot path for one (n, dtype=f32, sparsity)."""
+
+    def __init__(self, pk, n: int, density: float, seed_x: int, seed_y: int, device):
+        self.pk, self.n = pk, n
+        self.x = wl.sparse_buffer(n, density, seed=seed_x, device=device)
+        self.y = wl.sparse_buffer(n, density, seed=seed_y, device=device)
+        self.px, self.py, self.po = (pk.alloc_pici(n, pk.F32, device) for _ in range(3))
+        self.ws = pk.alloc_workspace(n, device)
+        self.dense = torch.empty(n, dtype=torch.float32, device=device)
+        self.cnt = torch.zeros(1, dtype=torch.int32, device=device)
+        self.flag = torch.zeros(1, dtype=torch.int32, device=device)
+        self.launches_per_step = 6
+
+    OPS = ("compress", "compress", "reduce_ss", "nnz", "maybe_densify", "reduce_sd")
+
+    def step(self, ev=None):
+        pk = self.pk
+        calls = (
+            lambda: pk.compress(self.x, self.px, self.ws),
+            lambda: pk.compress(self.y, self.py, self.ws),
+            lambda: pk.reduce_ss(self.px, self.py, self.po, self.ws),
+            lambda: pk.nnz(self.po, self.cnt),
+            lambda: pk.maybe_densify(self.po, 0, self.dense, self.flag),
+            lambda: pk.reduce_sd(self.px, self.dense),
+        )
+        if ev is None:
+            for c in calls:
+                c()
+            return
+        for i, c in enumerate(calls):
+            ev[i][0].record()
+            c()
+            ev[i][1].record()
+
+    def counts(self):
+        torch.cuda.synchronize()
+        return self.px.nnz_host(), self.py.nnz_host(), self.po.nnz_host()
+
+
+def touched_sectors_f32(mask_dense: torch.Tensor) -> int:
+    """Number of 32-byte sectors (8 fp32) of a dense buffer holding at least one nonzero."""
+    n8 = mask_dense.numel() // 8 * 8
+    return int((mask_dense[:n8].view(-1, 8) != 0).any(dim=1).sum().item())
+
+
+def time_op(fn, iters: int, warm: int = 2):
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+    for a, b in evs:
+        a.record(); fn(); b.record()
+    torch.cuda.synchronize()
+    ts = sorted(a.elapsed_time(b) for a, b in evs)
+    return ts[len(ts) // 2], ts[0]
+
+
+def run_sweep(pk, n: int, peak: float, iters: int, device) -> list[dict]:
+    """Every kernel alone at every sparsity of configs[1] (seed 0; fp32: all ops, bf16: compress/decompress)."""
+    rows = []
+    for dtype in ("f32", "bf16"):
+        s = 4 if dtype == "f32" else 2
+        D = pk.F32 if dtype == "f32" else pk.BF16
+        for sp in wl.CONFIG2_SPARSITIES:
+            d = 1.0 - sp
+            x = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 0), dtype=dtype, device=device)
+            px = pk.alloc_pici(n, D, device)
+            ws = pk.alloc_workspace(n, device)
+            out = torch.empty_like(x)
+
+            def row(op, ms, ms_min, nbytes):
+                rows.append({"dtype": dtype, "sparsity": sp, "op": op, "ms": round(ms, 4), "ms_min": round(ms_min, 4),
+                             "dense_equiv_gbs": round(n * s / ms / 1e6, 1), "bytes_moved_gbs": round(nbytes / ms / 1e6, 1),
+                             "frac": round(nbytes / ms / 1e6 / peak, 3)})
+
+            ms, mn = time_op(lambda: pk.compress(x, px, ws), iters)
+            nx = px.nnz_host()
+            row("compress", ms, mn, bytes_compress(n, s, nx))
+            ms, mn = time_op(lambda: pk.decompress(px, out), iters)
+            row("decompress", ms, mn, bytes_decompress(n, s, nx))
+            if dtype == "f32":
+                y = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 1), dtype=dtype, device=device)
+                py, po = pk.alloc_pici(n, D, device), pk.alloc_pici(n, D, device)
+                pk.compress(y, py, ws)
+                pk.reduce_ss(px, py, po, ws)
+                ny, no = py.nnz_host(), po.nnz_host()
+                ms, mn = time_op(lambda: pk.reduce_ss(px, py, po, ws), iters)
+                row("reduce_ss", ms, mn, bytes_reduce_ss(n, nx, ny, no))
+                sect = touched_sectors_f32(x)
+                ms, mn = time_op(lambda: pk.reduce_sd(px, y), iters)      # in place into a 2^28 dense buffer
+                row("reduce_sd", ms, mn, bytes_reduce_sd(n, nx, sect))
+                rows[-1]["touched_sector_frac"] = round(sect / (n / 8), 4)
+                del y, py, po
+            del x, px, out, ws
+            torch.cuda.empty_cache()
+    return rows
+
+
+def run_e2e(pk, n: int, density: float, steps: int, device, seed: int) -> dict:
+    """HOST buffers in, HOST buffers out, through pici_compress_host / pici_decompress_host."""
+    h_x = wl.sparse_buffer(n, density, seed=seed).pin_memory()
+    h_back = torch.empty(n, dtype=torch.float32).pin_memory()
+    h_p = pk.alloc_host_pici(n, pk.F32)
+    d_dense = torch.empty(n, dtype=torch.float32, device=device)
+    d_p = pk.alloc_pici(n, pk.F32, device)
+    ws = pk.alloc_workspace(n, device)
+
+    def step():
+        pk.compress_host(h_x, h_p, d_dense, d_p, ws)
+        pk.decompress_host(h_p, h_back, d_p, d_dense)
+
+    step()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step()
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    ok = bool(torch.equal(h_back.view(torch.int32), h_x.view(torch.int32)))
+    m = meta_bytes(n) + 4 * h_p.nnz
+    return {"value": 2 * n * 4 * steps / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": n * 4 + m,
+            "d2h_bytes_per_step": n * 4 + m, "ms_per_step": dt / steps * 1e3, "steps": steps, "round_trip_ok": ok,
+            "path": "pici_compress_host + pici_decompress_host (pinned host buffers; 2 buffers of N*4 bytes per step)"}
+
+
+def run_cpu_baseline(n: int, density: float) -> dict:
+    import numpy as np
+    from oracle import pici_oracle as po
+    x = wl.sparse_buffer(n, density, seed=wl.stream_seed(0, 0)).numpy()
+    y = wl.sparse_buffer(n, density, seed=wl.stream_seed(0, 1)).numpy()
+    best = None
+    t_all = time.perf_counter()
+    reps = 0
+    while reps < 2 or (time.perf_counter() - t_all < 8.0 and reps < 6):
+        t0 = time.perf_counter()
+        px = po.compress(x.view(np.uint32), "f32")
+        py = po.compress(y.view(np.uint32), "f32")
+        pz = po.reduce_ss(px, py)
+        po.nnz_pici(pz)
+        dense = np.empty(n, np.uint32)
+        po.maybe_densify(pz, 0, dense)
+        po.reduce_sd(px, dense.view(np.float32))
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+        reps += 1
+    return {"value": OPS_PER_STEP * n * 4 / best / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"same step on N=2^{n.bit_length() - 1} elements of the same recipe (fp32, same sparsity, seeds 0/1), "
+                      f"best of {reps}; oracle/pici_oracle.c single thread, gcc -O2",
+            "host_cores_available": os.cpu_count()}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="pici", choices=["pici", "reference"])
+    ap.add_argument("--sparsity", type=float, default=0.99)
+    ap.add_argument("--log2n", type=int, default=28, help="elements per buffer (configs[1]: 2^28)")
+    ap.add_argument("--ref-n", type=int, default=1 << 26, help="--impl reference: elements per step (bounded sample)")
+    ap.add_argument("--cpu-n", type=int, default=1 << 26, help="cpu_baseline sample size")
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweep-iters", type=int, default=7)
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the Pici path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    from paper_2607_04676_b200 import pici as pk
+    pk.lib()
+
+    n = 1 << args.log2n
+    density = 1.0 - args.sparsity
+    peak, peak_src = measured_peak()
+    from paper_2607_04676_b200 import replicas
+    seed_x, seed_y = replicas.rank_seeds(0, rank, 2)
+    hp = HotPath(pk, n, density, seed_x, seed_y, device)
+    for _ in range(args.warmup):
+        hp.step()
+    nx, ny, no = hp.counts()
+
+    K = args.steps
+    nops = len(HotPath.OPS)
+    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nops)]
+           for _ in range(K)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    barrier()
+    w0 = time.time()
+    e0.record()
+    for k in range(K):
+        hp.step(evs[k])
+    e1.record()
+    barrier()
+    w1 = time.time()
+    units_per_s, ms_total = replicas.whole_job_throughput(OPS_PER_STEP * n * 4 * K, e0.elapsed_time(e1), device)
+    clocks = sampler.stop(w0, w1) if rank == 0 else None
+
+    # per-kernel durations inside the timed region
+    per_op = {}
+    for i, name in enumerate(HotPath.OPS):
+        per_op.setdefault(name, []).extend(evs[k][i][0].elapsed_time(evs[k][i][1]) for k in range(K))
+    sect = touched_sectors_f32(hp.x)
+    alg = {"compress": (bytes_compress(n, 4, nx) + bytes_compress(n, 4, ny)) / 2,
+           "reduce_ss": bytes_reduce_ss(n, nx, ny, no),
+           "maybe_densify": bytes_decompress(n, 4, no),
+           "reduce_sd": bytes_reduce_sd(n, nx, sect),
+           "nnz": 8}
+    traffic = ncu_traffic()
+    kernels = {}
+    for name, ts in per_op.items():
+        avg = sum(ts) / len(ts)
+        kernels[name] = {"avg_ms": round(avg, 4), "launches": len(ts), "share": round(sum(ts) / ms_total, 3),
+                         "alg_bytes": int(alg[name]), "achieved_gbs": round(alg[name] / avg / 1e6, 1),
+                         "frac": round(alg[name] / avg / 1e6 / peak, 3)}
+    dom = max((k for k in kernels if k != "nnz"), key=lambda k: kernels[k]["avg_ms"] * kernels[k]["launches"])
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "traffic": traffic.get(dom), "peak_source": peak_src,
+                "alg_bytes_per_launch": kernels[dom]["alg_bytes"], "avg_launch_ms": kernels[dom]["avg_ms"]}
+
+    e2e = None
+    if not args.no_e2e:
+        del hp.dense
+        torch.cuda.empty_cache()
+        e2e = run_e2e(pk, n, density, max(2, min(K, 5)), device, seed_x)
+        thr, ms = replicas.whole_job_throughput(2 * n * 4 * e2e["steps"], e2e["ms_per_step"] * e2e["steps"], device)
+        e2e["value"], e2e["ms_per_step"] = thr / 1e9, ms / e2e["steps"]
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    value = units_per_s / 1e9
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"configs[1]: Pici hot path (2x compress, reduce_ss, nnz, maybe_densify->decompress, reduce_sd) "
+                               f"on N=2^{args.log2n} fp32 buffers, Bernoulli sparsity {args.sparsity}, N(0,1), seeds 0/1",
+                   "n": n, "sparsity": args.sparsity, "nnz": [nx, ny, no],
+                   "l2": "inputs larger than L2 (1 GiB dense buffers, 126 MB L2); no explicit flush",
+                   "parallelism": f"replicas x{world}, no data-path collective"},
+        "gpu_launches": hp.launches_per_step * K,
+        "kernels": kernels, "roofline": roofline, "clocks": clocks,
+    }
+    if e2e is not None:
+        out["e2e"] = e2e
+    if not args.no_sweep and world == 1:
+        del hp
+        torch.cuda.empty_cache()
+        out["sweep"] = run_sweep(pk, n, peak, args.sweep_iters, device)
+    if not args.no_cpu and world == 1:
+        out["cpu_baseline"] = run_cpu_baseline(args.cpu_n, density)
+    print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
