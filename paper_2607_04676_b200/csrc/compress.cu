@@ -9,7 +9,8 @@
 //     of the tile are in flight at once, and the tile is read from HBM exactly ONCE: its values stay
 //     in registers between Phase 1 and Phase 3;
 //   * Phase 2 is a device-wide single-pass decoupled look-back over per-tile status words (the paper
-//     scans block-locally per NCCLX segment); tiles are handed out by a dynamic ticket;
+//     scans block-locally per NCCLX segment); tiles are handed out by a dynamic ticket
+//     and a tile's look-back is deferred behind the next tile's loads;
 //   * Phase 3 compacts into a per-warp shared-memory stage (lane l's values are one contiguous run),
 //     which is then written to A with coalesced stores.
 #include "launch.h"
@@ -49,10 +50,6 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
     const int warp = threadIdx.x >> 5;
     Elem *stage = reinterpret_cast<Elem *>(smem_raw) + warp * kTile;
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
-    if (blockIdx.x == 0) {  // block 0 is the Phase-2 scanner
-        if (warp == 0) scanner_warp(status, T, I, lane);
-        return;
-    }
     const uint32_t Tfull = (uint32_t)(n / kTile);
     Elem *Aout = reinterpret_cast<Elem *>(A);
 
@@ -101,14 +98,14 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
     else if (t < T) load_ragged(t, v);
 
     // Per-warp software pipeline.  A tile's count is published as soon as its data has arrived and
-    // Phase 1 is done; the wait for its prefix (and the flush of its compacted values) is deferred
-    // until AFTER the next tile's count has been published, so no ticket is ever held across a wait
-    // and the scanner sees counts in near ticket order.
+    // Phase 1 is done; its look-back (and the flush of its compacted values) is deferred until AFTER
+    // the next tile's count has been published, so the look-back latency hides behind the next tile
+    // and no count is ever held back by a wait.
     bool pending = false;       // stage holds the compacted values of tile pt, not yet flushed
     uint32_t pt = 0, pnnz = 0;
     auto flush_pending = [&]() {
         if (pending) {
-            const uint32_t excl = wait_prefix(status, pt, lane);
+            const uint32_t excl = lookback_prefix(status, pt, pnnz, T, I, lane);
             Elem *dst = Aout + excl;
             for (uint32_t i = lane; i < pnnz; i += 32) dst[i] = stage[i];
             __syncwarp();
@@ -141,7 +138,7 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
         const uint32_t incl = warp_incl_scan(cnt0 + cnt1, lane);
         const uint32_t tile_nnz = __shfl_sync(kFull, incl, 31);
 
-        // ---- Phase 2: publish this tile's count; the scanner warp turns it into I[t] -------------
+        // ---- Phase 2: publish this tile's count (the look-back itself is deferred, see above) ----
         publish_count(status, t, tile_nnz, lane);
 
         // B: lane l holds words 2l, 2l+1 -> one 16-byte store per lane, 512 contiguous bytes per warp
@@ -224,8 +221,8 @@ static cudaError_t launch_compress_t(const void *dense, uint64_t n, uint64_t *B,
     }
     cudaError_t e = cudaMemsetAsync(ws, 0, scan_workspace_bytes(n), s);
     if (e != cudaSuccess) return e;
-    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps + 1;  // + the scanner block
-    const uint64_t cap = (uint64_t)num_sms() * Cfg::kMinBlocks;           // the whole grid is resident
+    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
+    const uint64_t cap = (uint64_t)num_sms() * Cfg::kMinBlocks;           // persistent: one resident wave
     if (blocks > cap) blocks = cap;
     uint32_t *ticket = reinterpret_cast<uint32_t *>(ws);
     uint64_t *status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);

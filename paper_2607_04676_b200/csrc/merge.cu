@@ -37,10 +37,6 @@ reduce_ss_kernel(const uint64_t *__restrict__ Bx, const uint32_t *__restrict__ I
     uint32_t *sx = so + kTile;
     uint32_t *sy = sx + kMergePass;
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
-    if (blockIdx.x == 0) {  // block 0 is the Phase-2 scanner
-        if (warp == 0) scanner_warp(status, T, Io, lane);
-        return;
-    }
 
     uint32_t t = next_ticket(ticket, lane);
     while (t < T) {
@@ -110,7 +106,7 @@ reduce_ss_kernel(const uint64_t *__restrict__ Bx, const uint32_t *__restrict__ I
 #pragma unroll
         for (int p = 0; p < 4; ++p) Bow[32 * p + lane] = wo[p];
 
-        const uint32_t excl = wait_prefix(status, t, lane);
+        const uint32_t excl = lookback_prefix(status, t, tile_nnz, T, Io, lane);
 
         uint32_t *dst = Ao + excl;
         if (tile_nnz == cand_base) {  // no cancellation anywhere in the tile: the stage is already packed
@@ -143,8 +139,8 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
     cudaError_t e = cudaMemsetAsync(ws, 0, scan_workspace_bytes(n), s);
     if (e != cudaSuccess) return e;
     const uint64_t per_sm = (227u * 1024u) / (smem + 1024);
-    uint64_t blocks = (T + kMergeWarps - 1) / kMergeWarps + 1;  // + the scanner block
-    const uint64_t cap = (uint64_t)num_sms() * per_sm;             // the whole grid is resident
+    uint64_t blocks = (T + kMergeWarps - 1) / kMergeWarps;
+    const uint64_t cap = (uint64_t)num_sms() * per_sm;             // persistent: one resident wave
     if (blocks > cap) blocks = cap;
     uint32_t *ticket = reinterpret_cast<uint32_t *>(ws);
     uint64_t *status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);

@@ -77,23 +77,20 @@ __device__ __forceinline__ bool gate_closed(const int32_t *gate, int32_t gate_va
 }
 
 // ---- single-pass device-wide exclusive scan of per-tile counts (Phase 2) ------------------------
+// Decoupled look-back at TILE granularity (one partition = one 64x64 tile = one warp's unit of work).
 // One 64-bit status word per tile: high 32 bits = flag, low 32 bits = value; flag and value travel in
 // ONE 64-bit access, so relaxed gpu-scope accesses suffice (nothing else is published through it).
-//
-// Decoupled look-back, with the look-back itself decoupled from the workers: every worker warp only
-// PUBLISHES its tile count (flag kStCount) and later waits on its OWN word; one dedicated scanner warp
-// (block 0) walks the status array in tile order, kScanRows*32 words per round, and replaces each
-// count by the tile's exclusive prefix (flag kStPrefix), writing I[] as it goes.  The scan is
-// ~T additions in total, so one warp keeps up with tiles retiring at HBM speed, and the polling
-// traffic is one word per waiting warp instead of a 32-word window per warp.
-// Tiles are handed out by a dynamic ticket, so every tile below the highest ticket is owned by a
-// resident warp; the scanner block is block 0 of a grid that is sized to be fully resident.
-constexpr uint64_t kStEmpty = 0, kStCount = 1, kStPrefix = 2;
+//   kStAggregate : value = nnz of the tile               (published right after Phase 1)
+//   kStPrefix    : value = nnz of tiles 0..t inclusive   (published after the tile's look-back)
+// A tile's look-back reads the 32 status words before it in one coalesced request (lane l <-> tile
+// pos-1-l), takes everything up to the closest kStPrefix, or - if the window holds aggregates only -
+// adds all 32 and moves one window further back.  Aggregates do not depend on any other tile, so a
+// look-back never waits on another look-back, only on Phase 1 of earlier tiles; tiles are handed out
+// by a dynamic ticket, so every earlier tile is owned by a warp that is already running (forward
+// progress without any residency assumption).  All sums are integers: the result does not depend on
+// scheduling.
+constexpr uint64_t kStEmpty = 0, kStAggregate = 1, kStPrefix = 2;
 constexpr int kWsHeaderBytes = 128;
-#ifndef PICI_SCAN_ROWS
-#define PICI_SCAN_ROWS 4
-#endif
-constexpr int kScanRows = PICI_SCAN_ROWS;
 
 __device__ __forceinline__ uint64_t ld_status(const uint64_t *p) {
     uint64_t v;
@@ -105,72 +102,47 @@ __device__ __forceinline__ void st_status(uint64_t *p, uint64_t flag, uint32_t v
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-// Worker, step 1 (warp-collective): make tile t's count visible to the scanner.
+// Step 1 (warp-collective): make tile t's count visible.  Tile 0 has no predecessor: its aggregate
+// is its inclusive prefix.
 __device__ __forceinline__ void publish_count(uint64_t *status, uint32_t t, uint32_t count, int lane) {
-    if (lane == 0) st_status(status + t, kStCount, count);
+    if (lane == 0) st_status(status + t, t == 0 ? kStPrefix : kStAggregate, count);
 }
 
-// Worker, step 2 (warp-collective): the exclusive prefix of tile t (sum of the counts of tiles 0..t-1).
-__device__ __forceinline__ uint32_t wait_prefix(const uint64_t *status, uint32_t t, int lane) {
+// Step 2 (warp-collective): exclusive prefix of tile t = sum of the counts of tiles 0..t-1; publishes
+// the tile's inclusive prefix and writes I[t] (and I[T] from the last tile).
+__device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t t, uint32_t count, uint32_t T,
+                                                    uint32_t *__restrict__ I, int lane) {
     uint32_t excl = 0;
+    int64_t pos = t;  // tiles [0, pos) are not yet accounted for
+    while (pos > 0) {  // warp-uniform
+        const int64_t idx = pos - 1 - lane;
+        uint64_t s;
+        unsigned pm, em;
+        unsigned ns = 8;
+        for (;;) {
+            s = idx >= 0 ? ld_status(status + idx) : (kStPrefix << 32);
+            const uint32_t flag = (uint32_t)(s >> 32);
+            pm = __ballot_sync(kFull, flag == (uint32_t)kStPrefix);
+            em = __ballot_sync(kFull, flag == (uint32_t)kStEmpty);
+            // lanes that matter: up to and including the closest prefix (all 32 if there is none)
+            const unsigned rel = pm ? ((pm & (0u - pm)) | ((pm & (0u - pm)) - 1u)) : kFull;
+            if ((em & rel) == 0u) {
+                const uint32_t v = ((1u << lane) & rel) ? (uint32_t)s : 0u;
+                excl += warp_sum(v);
+                break;
+            }
+            __nanosleep(ns);
+            if (ns < 64) ns += ns;
+        }
+        if (pm) break;
+        pos -= 32;
+    }
     if (lane == 0) {
-        uint64_t s = ld_status(status + t);
-        unsigned ns = 20;
-        while ((uint32_t)(s >> 32) != (uint32_t)kStPrefix) {
-            __nanosleep(ns);
-            if (ns < 160) ns += ns;
-            s = ld_status(status + t);
-        }
-        excl = (uint32_t)s;
+        if (t != 0) st_status(status + t, kStPrefix, excl + count);
+        I[t] = excl;
+        if (t + 1 == T) I[T] = excl + count;
     }
-    return __shfl_sync(kFull, excl, 0);
-}
-
-// The scanner warp.  Writes I[0..T] (I[T] = total nnz).
-__device__ __forceinline__ void scanner_warp(uint64_t *status, uint32_t T, uint32_t *__restrict__ I, int lane) {
-    uint32_t pos = 0, run = 0;
-    unsigned ns = 20;
-    while (pos < T) {
-        uint64_t st[kScanRows];
-#pragma unroll
-        for (int j = 0; j < kScanRows; ++j) {
-            const uint32_t idx = pos + 32 * j + lane;
-            st[j] = idx < T ? ld_status(status + idx) : 0ull;
-        }
-        uint32_t nready = 0;
-        bool open = true;
-#pragma unroll
-        for (int j = 0; j < kScanRows; ++j) {
-            const unsigned m = __ballot_sync(kFull, (uint32_t)(st[j] >> 32) == (uint32_t)kStCount);
-            if (open) {
-                const uint32_t lead = (m == kFull) ? 32u : (uint32_t)(__ffs(~m) - 1);
-                nready += lead;
-                open = (lead == 32u);
-            }
-        }
-        if (nready == 0) {
-            __nanosleep(ns);
-            if (ns < 80) ns += ns;
-            continue;
-        }
-        ns = 20;
-#pragma unroll
-        for (int j = 0; j < kScanRows; ++j) {
-            if (32u * j < nready) {  // warp-uniform
-                const uint32_t k = 32 * j + lane;
-                const uint32_t c = k < nready ? (uint32_t)st[j] : 0u;
-                const uint32_t incl = warp_incl_scan(c, lane);
-                if (k < nready) {
-                    const uint32_t excl = run + incl - c;
-                    st_status(status + pos + k, kStPrefix, excl);
-                    I[pos + k] = excl;
-                }
-                run += __shfl_sync(kFull, incl, 31);
-            }
-        }
-        pos += nready;
-    }
-    if (lane == 0) I[T] = run;
+    return excl;
 }
 
 // Dynamic tile ticket (one atomic per tile, issued by lane 0 and broadcast).
