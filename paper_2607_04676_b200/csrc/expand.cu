@@ -1,39 +1,58 @@
 // expand.cu - the "Phase 3 reversed" family: pici_decompress, pici_reduce_sd (the
 // scatter-add "decompression"), pici_maybe_densify.
 //
-// One warp owns one 64x64 tile.  The 512-byte block of B that belongs to the tile is read as 128
-// 32-bit HALF-COLUMN words: in pass p (0..3) lane l holds word 32p+l = column 16p + l/2, rows
-// 32(l&1) .. 32(l&1)+31.  Read that way the words are in exactly the order of A (tile -> column ->
-// row), so a value's slot is   I[t] + (popc of all earlier words of the tile) + popc(lower bits),
-// the warp scan runs on 32-bit popcounts, and every lane has the same amount of work.
-//
-//   decompress : the tile is assembled in shared memory (zero-fill, scatter the values) and leaves
-//                as ONE contiguous 16 KB (fp32) / 8 KB (bf16) block -> fully coalesced 128-bit stores.
-//   add, stream: same, but the shared tile starts as a copy of `local`, values are added in place in
-//                shared memory (each element is owned by exactly one lane) and the tile is stored to
-//                `out`.  Elements without a bit keep their bits exactly (a -0.0 survives).
-//   add, sparse: in place and few nonzeros in the tile: read-modify-write of only the touched
-//                elements straight in global memory (sector-granular traffic).
-// A values of a pass (<= 1024) are staged through shared memory with coalesced loads, so slot lookups
-// never become per-lane strided global loads.
+// One warp owns one 64x64 tile at a time; lane l owns the ADJACENT columns 2l and 2l+1 (the paper's
+// Phase-3 mapping), i.e. the two 64-bit words B[64t+2l], B[64t+2l+1] - one 16-byte load
+// per lane, 512 contiguous bytes per warp.  Because A is ordered tile -> column -> row, the values of
+// lane l's two columns are ONE contiguous run of A that starts at
+//     I[t] + (exclusive warp scan of popc(word 2l) + popc(word 2l+1)).
+// The kernel is written as a GATHER over rows, not a scatter over set bits:
+//   * the tile's segment of A, A[I[t] .. I[t+1]), is staged in shared memory by ONE 1-D TMA bulk copy
+//     (cp.async.bulk on a 16-byte aligned window; the < 16-byte tail goes through plain loads so
+//     nothing past the segment is ever read) - no per-value global latency;
+//   * for row r = 0..63 (fully unrolled) the lane tests bit r of its two words, reads the next value
+//     of the column's run from the stage if the bit is set (running cursor), and the warp writes the
+//     row as one coalesced 256-byte (fp32) / 128-byte (bf16) streaming store straight to global
+//     memory.  No tile buffer, no zero fill, no shared-memory scatter, no copy-out.
+//   * reduce_sd, streaming form (out != local, or a tile with many values): same walk, the row of
+//     `local` is loaded 16 rows ahead and `a` is added where the bit is set; elements without a bit
+//     keep their bits exactly (a -0.0 survives).
+//   * reduce_sd, sparse form (in place and <= kSparseTileNnz values in the tile): the lanes first turn
+//     their words into a tile-local index list in shared memory (A order), then the warp walks that
+//     list 32 values at a time - coalesced loads of A, gather of the touched elements, add, scatter -
+//     with every load of the tile in flight before the first store (sector-granular traffic,
+//     SURVEY.md S7 #4).
+// The next tile's words and I[t] are prefetched into registers while the current tile is processed.
 #include "launch.h"
 #include "pici_common.cuh"
 #include "../../include/pici.h"
 
 namespace pici {
 
-constexpr int kExpandWarps = 2;
-constexpr int kPassElems = 1024;           // 16 columns x 64 rows
-constexpr uint32_t kSparseTileNnz = 256;   // in-place add: tiles with <= this many values use RMW
+constexpr int kExpandWarps = 1;
+#ifndef PICI_SPARSE_TILE_NNZ
+#define PICI_SPARSE_TILE_NNZ 128
+#endif
+constexpr uint32_t kSparseTileNnz = PICI_SPARSE_TILE_NNZ;   // in-place add: tiles with <= this many values use RMW
+static_assert(kSparseTileNnz % 32 == 0 && kSparseTileNnz <= 1024, "sparse list is walked 32 values at a time");
 
 enum { kModeDecompress = 0, kModeAdd = 1 };
 
-template <typename Elem>
-__device__ __forceinline__ void zero_fill(Elem *tile, int lane) {
-    uint4 *q = reinterpret_cast<uint4 *>(tile);
-    constexpr int kVec = kTile * sizeof(Elem) / 16;
-#pragma unroll 8
-    for (int i = lane; i < kVec; i += 32) q[i] = make_uint4(0, 0, 0, 0);
+template <int DT>
+struct ExpandCfg {
+    using Elem = typename ElemOf<DT>::type;
+    static constexpr uint32_t kStageBytes = kTile * sizeof(Elem) + 32;   // segment + alignment slack
+};
+
+__device__ __forceinline__ uint2 ld_coherent_u2(const uint2 *p) {
+    uint2 v;
+    asm volatile("ld.global.L1::no_allocate.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ ulonglong2 ldg_nc_u64x2(const uint64_t *p) {
+    ulonglong2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "l"(p));
+    return v;
 }
 
 template <int DT, int MODE>
@@ -41,8 +60,10 @@ __global__ void __launch_bounds__(kExpandWarps * 32)
 expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, const void *__restrict__ A,
               uint64_t n, const void *local, void *out, DensifyCtl ctl, const int32_t *gate,
               int32_t gate_value) {
-    using Elem = typename ElemOf<DT>::type;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    using Elem = typename ExpandCfg<DT>::Elem;
+    constexpr uint32_t ES = sizeof(Elem);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t mbar_mem[kExpandWarps];
     if (gate_closed(gate, gate_value)) return;
 
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
@@ -54,114 +75,200 @@ expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, co
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    Elem *tile = reinterpret_cast<Elem *>(smem_raw) + (size_t)warp * (kTile + kPassElems);
-    Elem *stage = tile + kTile;
+    unsigned char *stage_raw = smem_raw + (size_t)warp * ExpandCfg<DT>::kStageBytes;
+    Elem *stage = reinterpret_cast<Elem *>(stage_raw);
+    const uint32_t stage_s = smem_u32(stage_raw);
+    const uint32_t bar = smem_u32(&mbar_mem[warp]);
+    if (lane == 0) mbar_init(bar, 1);
+    __syncwarp();
+    uint32_t parity = 0;
+
     const Elem *Ain = reinterpret_cast<const Elem *>(A);
     const Elem *Lin = reinterpret_cast<const Elem *>(local);
     Elem *Dout = reinterpret_cast<Elem *>(out);
     const bool in_place = (MODE == kModeAdd) && (local == out);
+    const uint32_t Tfull = (uint32_t)(n / kTile);
+    const uint32_t stride = gridDim.x * kExpandWarps;
 
-    const uint32_t warps_total = gridDim.x * kExpandWarps;
-    for (uint32_t t = blockIdx.x * kExpandWarps + warp; t < T; t += warps_total) {
-        const size_t base = (size_t)t * kTile;
-        const uint32_t valid = (uint32_t)((n - base) < (uint64_t)kTile ? (n - base) : (uint64_t)kTile);
-        const uint32_t *Bw = reinterpret_cast<const uint32_t *>(B + (size_t)t * kSide);
-        uint32_t w[4];
-#pragma unroll
-        for (int p = 0; p < 4; ++p) w[p] = __ldg(Bw + 32 * p + lane);
-        const uint32_t seg = __ldg(I + t);
-
-        // exclusive offsets of this lane's four words inside the tile's segment of A
-        const uint32_t c0 = __popc(w[0]), c1 = __popc(w[1]), c2 = __popc(w[2]), c3 = __popc(w[3]);
-        const uint32_t s01 = warp_incl_scan(c0 | (c1 << 16), lane);
-        const uint32_t s23 = warp_incl_scan(c2 | (c3 << 16), lane);
-        const uint32_t t01 = __shfl_sync(kFull, s01, 31), t23 = __shfl_sync(kFull, s23, 31);
-        uint32_t tot[4] = {t01 & 0xFFFFu, t01 >> 16, t23 & 0xFFFFu, t23 >> 16};
-        uint32_t excl[4] = {(s01 & 0xFFFFu) - c0, (s01 >> 16) - c1, (s23 & 0xFFFFu) - c2, (s23 >> 16) - c3};
-        const uint32_t tile_nnz = tot[0] + tot[1] + tot[2] + tot[3];
-
-        const bool sparse_rmw = in_place && tile_nnz <= kSparseTileNnz;  // warp-uniform
-        if (MODE == kModeAdd && sparse_rmw && tile_nnz == 0) continue;
-
-        // ---- initialise the shared tile ------------------------------------------------------------
-        if (MODE == kModeDecompress) {
-            zero_fill(tile, lane);
-        } else if (!sparse_rmw) {
-            if (valid == kTile) {
-                const uint4 *src = reinterpret_cast<const uint4 *>(Lin + base);
-                uint4 *dst = reinterpret_cast<uint4 *>(tile);
-                constexpr int kVec = kTile * sizeof(Elem) / 16;
-#pragma unroll 8
-                for (int i = lane; i < kVec; i += 32) dst[i] = ldg_stream_u4(src + i);
-            } else {
-                for (uint32_t i = lane; i < valid; i += 32) tile[i] = Lin[base + i];
-            }
+    uint32_t t = blockIdx.x * kExpandWarps + warp;
+    ulonglong2 wn = make_ulonglong2(0, 0);
+    uint32_t segn = 0;
+    if (t < T) {
+        wn = ldg_nc_u64x2(B + (size_t)t * kSide + 2 * lane);
+        segn = __ldg(I + t);
+    }
+    for (; t < T; t += stride) {
+        const ulonglong2 w = wn;
+        const uint32_t seg = segn;
+        if (t + stride < T) {  // prefetch the next tile's words and segment start
+            wn = ldg_nc_u64x2(B + (size_t)(t + stride) * kSide + 2 * lane);
+            segn = __ldg(I + t + stride);
         }
-        __syncwarp();
+        const uint32_t cnt0 = __popcll(w.x), cnt1 = __popcll(w.y);
+        const uint32_t incl = warp_incl_scan(cnt0 + cnt1, lane);
+        const uint32_t tile_nnz = __shfl_sync(kFull, incl, 31);
+        const uint32_t excl = incl - cnt0 - cnt1;   // tile-local slot of this lane's first value
+        const size_t base = (size_t)t * kTile;
+        const bool full = t < Tfull;
 
-        // ---- scatter the values, pass by pass -------------------------------------------------------
-        uint32_t pass_base = seg;
-#pragma unroll
-        for (int p = 0; p < 4; ++p) {
-            const uint32_t cnt = tot[p];
-            if (cnt != 0) {  // warp-uniform
-                for (uint32_t i = lane; i < cnt; i += 32) stage[i] = Ain[pass_base + i];
-                __syncwarp();
-                const uint32_t col = 16 * p + (lane >> 1);
-                const uint32_t row0 = 32 * (lane & 1);
-                uint32_t u = w[p], k = excl[p];
+        if constexpr (MODE == kModeAdd) {
+            if (in_place && tile_nnz == 0) continue;
+            if (in_place && tile_nnz <= kSparseTileNnz) {
+                // ---- sparse form: index list, then batched gather / add / scatter ------------------
+                uint16_t *list = reinterpret_cast<uint16_t *>(stage_raw);
+                uint32_t k = excl;
+                uint64_t u = w.x;
                 while (u) {
-                    const uint32_t r = __ffs(u) - 1;
+                    const uint32_t r = __ffsll((long long)u) - 1;
                     u &= u - 1;
-                    const uint32_t idx = (row0 + r) * kSide + col;
-                    if (MODE == kModeDecompress) {
-                        tile[idx] = stage[k++];
-                    } else {
-                        if constexpr (DT == PICI_F32) {
-                            const float a = __uint_as_float(stage[k++]);
-                            if (sparse_rmw) {
-                                uint32_t *d = reinterpret_cast<uint32_t *>(Dout) + base + idx;
-                                *d = __float_as_uint(__fadd_rn(__uint_as_float(*d), a));
-                            } else {
-                                tile[idx] = __float_as_uint(__fadd_rn(__uint_as_float(tile[idx]), a));
-                            }
-                        }
-                    }
+                    list[k++] = (uint16_t)(r * kSide + 2 * lane);
+                }
+                u = w.y;
+                while (u) {
+                    const uint32_t r = __ffsll((long long)u) - 1;
+                    u &= u - 1;
+                    list[k++] = (uint16_t)(r * kSide + 2 * lane + 1);
                 }
                 __syncwarp();
-                pass_base += cnt;
+                constexpr int kIt = kSparseTileNnz / 32;
+                const uint32_t *Au = reinterpret_cast<const uint32_t *>(A) + seg;
+                uint32_t *Du = reinterpret_cast<uint32_t *>(out) + base;
+                uint32_t av[kIt], dv[kIt], ix[kIt];
+#pragma unroll
+                for (int j = 0; j < kIt; ++j) {
+                    const uint32_t jj = 32 * j + lane;
+                    if (jj < tile_nnz) {
+                        ix[j] = list[jj];
+                        av[j] = ldg_stream_u32(Au + jj);
+                        dv[j] = Du[ix[j]];
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < kIt; ++j) {
+                    const uint32_t jj = 32 * j + lane;
+                    if (jj < tile_nnz)
+                        Du[ix[j]] = __float_as_uint(__fadd_rn(__uint_as_float(dv[j]), __uint_as_float(av[j])));
+                }
+                __syncwarp();
+                continue;
+            }
+        }
+        if constexpr (MODE == kModeDecompress) {
+            if (tile_nnz == 0 && full) {  // an empty tile: 16 KB / 8 KB of +0.0
+                uint4 *dst = reinterpret_cast<uint4 *>(Dout + base);
+                constexpr int kVec = kTile * ES / 16;
+#pragma unroll
+                for (int i = 0; i < kVec / 32; ++i) stg_stream_u4(dst + 32 * i + lane, make_uint4(0, 0, 0, 0));
+                continue;
             }
         }
 
-        // ---- store the tile -------------------------------------------------------------------------
-        if (!(MODE == kModeAdd && sparse_rmw)) {
-            if (valid == kTile) {
-                const uint4 *src = reinterpret_cast<const uint4 *>(tile);
-                uint4 *dst = reinterpret_cast<uint4 *>(Dout + base);
-                constexpr int kVec = kTile * sizeof(Elem) / 16;
-#pragma unroll 8
-                for (int i = lane; i < kVec; i += 32) stg_stream_u4(dst + i, src[i]);
-            } else {
-                for (uint32_t i = lane; i < valid; i += 32) Dout[base + i] = tile[i];
+        // ---- stage the tile's segment of A: one TMA bulk copy + a < 16-byte tail ---------------------
+        const uint64_t a_beg = (uint64_t)seg * ES, a_end = a_beg + (uint64_t)tile_nnz * ES;
+        const uint64_t start_al = a_beg & ~15ull, end_dn = a_end & ~15ull;
+        const uint32_t bulk = end_dn > start_al ? (uint32_t)(end_dn - start_al) : 0u;
+        if (tile_nnz != 0) {
+            if (bulk != 0 && lane == 0) {
+                fence_proxy_async_smem();
+                mbar_expect_tx(bar, bulk);
+                bulk_g2s(stage_s, reinterpret_cast<const unsigned char *>(A) + start_al, bulk, bar);
+            }
+            const uint64_t tail_beg = bulk != 0 ? end_dn : a_beg;
+            const uint32_t tail_cnt = (uint32_t)(a_end - tail_beg) / ES;
+            if ((uint32_t)lane < tail_cnt)
+                stage[(uint32_t)(tail_beg - start_al) / ES + lane] = Ain[tail_beg / ES + lane];
+        }
+        uint32_t k0 = (uint32_t)(a_beg - start_al) / ES + excl;   // cursor of column 2l in the stage
+        uint32_t k1 = k0 + cnt0;                                  // cursor of column 2l+1
+        const uint32_t w0lo = (uint32_t)w.x, w0hi = (uint32_t)(w.x >> 32);
+        const uint32_t w1lo = (uint32_t)w.y, w1hi = (uint32_t)(w.y >> 32);
+
+        if (full) {
+            constexpr int kChunk = 16;
+#pragma unroll
+            for (int c = 0; c < kSide / kChunk; ++c) {
+                uint2 loc[kChunk];
+                if constexpr (MODE == kModeAdd) {
+                    const uint2 *src = reinterpret_cast<const uint2 *>(Lin + base) + lane;
+#pragma unroll
+                    for (int j = 0; j < kChunk; ++j) loc[j] = ld_coherent_u2(src + 32 * (kChunk * c + j));
+                }
+                if (c == 0) {
+                    if (bulk != 0) {
+                        mbar_wait(bar, parity);
+                        parity ^= 1u;
+                    }
+                    __syncwarp();
+                }
+#pragma unroll
+                for (int j = 0; j < kChunk; ++j) {
+                    const int r = kChunk * c + j;
+                    const uint32_t m = 1u << (r & 31);
+                    const bool b0 = ((r < 32 ? w0lo : w0hi) & m) != 0u;
+                    const bool b1 = ((r < 32 ? w1lo : w1hi) & m) != 0u;
+                    if constexpr (MODE == kModeDecompress) {
+                        uint32_t v0 = 0, v1 = 0;
+                        if (b0) v0 = stage[k0++];
+                        if (b1) v1 = stage[k1++];
+                        if constexpr (DT == PICI_F32) {
+                            stg_stream_u2(reinterpret_cast<uint2 *>(Dout + base) + lane + 32 * r, make_uint2(v0, v1));
+                        } else {
+                            stg_stream_u32(reinterpret_cast<uint32_t *>(Dout + base) + lane + 32 * r, v0 | (v1 << 16));
+                        }
+                    } else if constexpr (DT == PICI_F32) {
+                        uint2 v = loc[j];
+                        if (b0) v.x = __float_as_uint(__fadd_rn(__uint_as_float(v.x), __uint_as_float(stage[k0++])));
+                        if (b1) v.y = __float_as_uint(__fadd_rn(__uint_as_float(v.y), __uint_as_float(stage[k1++])));
+                        stg_stream_u2(reinterpret_cast<uint2 *>(Dout + base) + lane + 32 * r, v);
+                    }
+                }
+            }
+        } else {
+            // ---- ragged last tile: elements >= n do not exist (their bits are 0, C9 #4) -------------
+            const uint32_t valid = (uint32_t)(n - base);
+            if (bulk != 0) {
+                mbar_wait(bar, parity);
+                parity ^= 1u;
             }
             __syncwarp();
+            for (uint32_t r = 0; r < (uint32_t)kSide; ++r) {
+                const uint32_t i0 = r * kSide + 2 * lane;
+                const bool b0 = (w.x >> r) & 1ull, b1 = (w.y >> r) & 1ull;
+                Elem a0 = 0, a1 = 0;
+                if (b0) a0 = stage[k0++];
+                if (b1) a1 = stage[k1++];
+                if constexpr (MODE == kModeDecompress) {
+                    if (i0 < valid) Dout[base + i0] = a0;
+                    if (i0 + 1 < valid) Dout[base + i0 + 1] = a1;
+                } else if constexpr (DT == PICI_F32) {
+                    if (i0 < valid) {
+                        const uint32_t l0 = Lin[base + i0];
+                        Dout[base + i0] = b0 ? __float_as_uint(__fadd_rn(__uint_as_float(l0), __uint_as_float(a0))) : l0;
+                    }
+                    if (i0 + 1 < valid) {
+                        const uint32_t l1 = Lin[base + i0 + 1];
+                        Dout[base + i0 + 1] = b1 ? __float_as_uint(__fadd_rn(__uint_as_float(l1), __uint_as_float(a1))) : l1;
+                    }
+                }
+            }
         }
+        __syncwarp();  // every lane is done with the stage before the next tile's copy lands in it
     }
 }
 
 template <int DT, int MODE>
 static cudaError_t launch_expand_t(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n,
                                    const void *local, void *out, DensifyCtl ctl, Gate g, cudaStream_t s) {
-    using Elem = typename ElemOf<DT>::type;
     const uint64_t T = (n + kTile - 1) / kTile;
-    const size_t smem = (size_t)kExpandWarps * (kTile + kPassElems) * sizeof(Elem);
+    const size_t smem = (size_t)kExpandWarps * ExpandCfg<DT>::kStageBytes;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(expand_kernel<DT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    const uint64_t per_sm = (227u * 1024u) / (smem + 1024);
+    uint64_t per_sm = (227u * 1024u) / (smem + 1024);
+    if (per_sm > 32) per_sm = 32;
     uint64_t blocks = (T + kExpandWarps - 1) / kExpandWarps;
     const uint64_t cap = (uint64_t)num_sms() * (per_sm ? per_sm : 1);
     if (blocks > cap) blocks = cap;
