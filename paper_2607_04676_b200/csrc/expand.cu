@@ -38,6 +38,19 @@ static_assert(kSparseTileNnz % 32 == 0 && kSparseTileNnz <= 1024, "sparse list i
 
 enum { kModeDecompress = 0, kModeAdd = 1 };
 
+// In-place scatter-add picks its kernel ON THE DEVICE from the measured total I[T] (no host sync): with
+// at most kSparseAvgNnz values per tile on average the launch is a read-modify-write of the touched
+// elements only (scatter_add_sparse_kernel, sector-granular traffic); above it the
+// dense buffer is streamed through (expand_kernel).  Both kernels are enqueued, one returns at once.
+#ifndef PICI_SPARSE_AVG_NNZ
+#define PICI_SPARSE_AVG_NNZ 224
+#endif
+constexpr uint32_t kSparseAvgNnz = PICI_SPARSE_AVG_NNZ;
+constexpr uint32_t kSparseListMax = 256;   // values of one tile that fit the per-warp index list
+__device__ __forceinline__ bool sparse_regime(const uint32_t *__restrict__ I, uint32_t T) {
+    return (uint64_t)__ldg(I + T) <= (uint64_t)kSparseAvgNnz * T;
+}
+
 template <int DT>
 struct ExpandCfg {
     using Elem = typename ElemOf<DT>::type;
@@ -67,6 +80,9 @@ expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, co
     if (gate_closed(gate, gate_value)) return;
 
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
+    if constexpr (MODE == kModeAdd) {  // in place: the sparse regime belongs to scatter_add_sparse_kernel
+        if (local == out && sparse_regime(I, T)) return;
+    }
     if (ctl.d_flag != nullptr) {  // maybe_densify: integer compare on the measured nnz (C9 #9/#10)
         const bool switched = (uint64_t)I[T] >= ctl.nnz_switch;
         if (blockIdx.x == 0 && threadIdx.x == 0) *ctl.d_flag = switched ? ctl.on_value : ctl.off_value;
@@ -256,6 +272,93 @@ expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, co
     }
 }
 
+// ---- reduce_sd, sparse regime (in place) ---------------------------------------------------------
+// One warp per tile, 8 warps per CTA and only 512 bytes of shared memory per warp, so ~40 warps per SM
+// keep enough read-modify-writes in flight to cover HBM latency (the 16 KB stage of expand_kernel
+// limits it to 13 warps per SM; profiles/r1b: 52 % long-scoreboard stalls at 15 % issue activity).
+// Per tile: the lanes turn their two column words into a tile-local index list in A order (shared
+// memory), then the warp walks the list 32 values at a time - coalesced loads of A, gather of the
+// touched elements, one __fadd_rn each, scatter - with up to 128 gathers in flight per warp before the
+// first store.  Tiles are disjoint ranges of the dense buffer and a tile's list has no duplicates, so
+// no two threads touch the same element.  A tile with more than kSparseListMax values (rare here:
+// the regime is chosen from the average) is walked lane by lane without the list.
+constexpr int kSparseWarps = 8;
+__global__ void __launch_bounds__(kSparseWarps * 32, 5)
+scatter_add_sparse_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I,
+                          const uint32_t *__restrict__ A, uint64_t n, uint32_t *dense, const int32_t *gate,
+                          int32_t gate_value) {
+    __shared__ uint16_t lists[kSparseWarps][kSparseListMax];
+    if (gate_closed(gate, gate_value)) return;
+    const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
+    if (!sparse_regime(I, T)) return;
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    uint16_t *list = lists[warp];
+    const uint32_t stride = gridDim.x * kSparseWarps;
+    uint32_t t = blockIdx.x * kSparseWarps + warp;
+    // lanes 0 and 1 hold I[t], I[t+1] of the NEXT tile (prefetched one iteration ahead)
+    uint32_t inext = (t < T && lane < 2) ? __ldg(I + t + lane) : 0u;
+    for (; t < T; t += stride) {
+        const uint32_t seg = __shfl_sync(kFull, inext, 0);
+        const uint32_t tile_nnz = __shfl_sync(kFull, inext, 1) - seg;
+        if (t + stride < T && lane < 2) inext = __ldg(I + t + stride + lane);
+        if (tile_nnz == 0) continue;
+        const ulonglong2 w = ldg_nc_u64x2(B + (size_t)t * kSide + 2 * lane);
+        const uint32_t cnt0 = __popcll(w.x), cnt1 = __popcll(w.y);
+        const uint32_t excl = warp_incl_scan(cnt0 + cnt1, lane) - cnt0 - cnt1;
+        const uint32_t *Au = A + seg;
+        uint32_t *Du = dense + (size_t)t * kTile;
+        if (tile_nnz > kSparseListMax) {   // outlier tile: every lane walks its own two columns
+            uint32_t k = excl;
+            for (uint64_t u = w.x; u; u &= u - 1) {
+                const uint32_t i = (__ffsll((long long)u) - 1) * kSide + 2 * lane;
+                Du[i] = __float_as_uint(__fadd_rn(__uint_as_float(Du[i]), __uint_as_float(Au[k++])));
+            }
+            for (uint64_t u = w.y; u; u &= u - 1) {
+                const uint32_t i = (__ffsll((long long)u) - 1) * kSide + 2 * lane + 1;
+                Du[i] = __float_as_uint(__fadd_rn(__uint_as_float(Du[i]), __uint_as_float(Au[k++])));
+            }
+            continue;
+        }
+        {
+            uint32_t k = excl;
+            for (uint64_t u = w.x; u; u &= u - 1) list[k++] = (uint16_t)((__ffsll((long long)u) - 1) * kSide + 2 * lane);
+            for (uint64_t u = w.y; u; u &= u - 1) list[k++] = (uint16_t)((__ffsll((long long)u) - 1) * kSide + 2 * lane + 1);
+        }
+        __syncwarp();
+        for (uint32_t b0 = 0; b0 < tile_nnz; b0 += 128) {
+            uint32_t av[4], dv[4], ix[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t jj = b0 + 32 * j + lane;
+                if (jj < tile_nnz) {
+                    ix[j] = list[jj];
+                    av[j] = ldg_stream_u32(Au + jj);
+                    dv[j] = Du[ix[j]];
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t jj = b0 + 32 * j + lane;
+                if (jj < tile_nnz) Du[ix[j]] = __float_as_uint(__fadd_rn(__uint_as_float(dv[j]), __uint_as_float(av[j])));
+            }
+        }
+        __syncwarp();   // the list is rebuilt by the next tile
+    }
+}
+
+cudaError_t launch_scatter_add_sparse(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, void *dense,
+                                      Gate g, cudaStream_t s) {
+    const uint64_t T = (n + kTile - 1) / kTile;
+    uint64_t blocks = (T + kSparseWarps - 1) / kSparseWarps;
+    const uint64_t cap = (uint64_t)num_sms() * 5;
+    if (blocks > cap) blocks = cap;
+    if (blocks == 0) return cudaSuccess;
+    scatter_add_sparse_kernel<<<(unsigned)blocks, kSparseWarps * 32, 0, s>>>(
+        B, I, reinterpret_cast<const uint32_t *>(A), n, reinterpret_cast<uint32_t *>(dense), g.ptr, g.value);
+    return cudaGetLastError();
+}
+
 template <int DT, int MODE>
 static cudaError_t launch_expand_t(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n,
                                    const void *local, void *out, DensifyCtl ctl, Gate g, cudaStream_t s) {
@@ -280,7 +383,13 @@ static cudaError_t launch_expand_t(const uint64_t *B, const uint32_t *I, const v
 cudaError_t launch_expand(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
                           const void *local, void *out, int mode, DensifyCtl ctl, Gate g, cudaStream_t s) {
     if (n == 0 && ctl.d_flag == nullptr) return cudaSuccess;
-    if (mode == kModeAdd) return launch_expand_t<PICI_F32, kModeAdd>(B, I, A, n, local, out, ctl, g, s);
+    if (mode == kModeAdd) {
+        if (local == out) {  // in place: the sparse-regime kernel and the streaming kernel pick on the device
+            cudaError_t e = launch_scatter_add_sparse(B, I, A, n, out, g, s);
+            if (e != cudaSuccess) return e;
+        }
+        return launch_expand_t<PICI_F32, kModeAdd>(B, I, A, n, local, out, ctl, g, s);
+    }
     return dtype == PICI_F32 ? launch_expand_t<PICI_F32, kModeDecompress>(B, I, A, n, local, out, ctl, g, s)
                              : launch_expand_t<PICI_BF16, kModeDecompress>(B, I, A, n, local, out, ctl, g, s);
 }

@@ -202,14 +202,19 @@ __device__ __forceinline__ WalkOut span_walk(const MergeArgs &a, uint32_t *pool,
     return r;
 }
 
-// Phase 2 for the mt tiles of a span (one warp; lane i < mt holds tc = survivors of tile ts + i):
-// publish the aggregates, look back from tile ts, publish the inclusive prefixes, write Io.
+// Phase 2 for a span (one warp; lane i < mt holds tc = survivors of tile ts + i).  ONE status word per
+// SPAN (index g): the aggregate is the span's survivor total, so a 32-entry look-back window covers
+// 32 * m tiles and the chain of hops a look-back has to walk is m times shorter than with per-tile
+// words (profiles/r1b: 49 % of reduce_ss's stall samples sat behind this look-back).  Publishes the
+// aggregate, looks back from span g, publishes the inclusive prefix, writes Io for the span's tiles.
 // Returns the number of survivors before tile ts.
-__device__ __forceinline__ uint32_t span_lookback(const MergeArgs &a, uint32_t ts, uint32_t mt, uint32_t tc, int lane) {
-    if ((uint32_t)lane < mt) st_status(a.status + ts + lane, kStAggregate, tc);
+__device__ __forceinline__ uint32_t span_lookback(const MergeArgs &a, uint32_t g, uint32_t ts, uint32_t mt, uint32_t tc,
+                                                  int lane) {
     const uint32_t tincl = warp_incl_scan((uint32_t)lane < mt ? tc : 0u, lane);
+    const uint32_t total = __shfl_sync(kFull, tincl, 31);
+    if (lane == 0) st_status(a.status + g, g == 0 ? kStPrefix : kStAggregate, total);
     uint32_t excl = 0;
-    int64_t pos = ts;
+    int64_t pos = g;
     while (pos > 0) {
         const int64_t idx = pos - 1 - lane;
         uint64_t st;
@@ -230,8 +235,8 @@ __device__ __forceinline__ uint32_t span_lookback(const MergeArgs &a, uint32_t t
         if (pm) break;
         pos -= 32;
     }
+    if (lane == 0 && g != 0) st_status(a.status + g, kStPrefix, excl + total);
     if ((uint32_t)lane < mt) {
-        st_status(a.status + ts + lane, kStPrefix, excl + tincl);
         a.Io[ts + lane] = excl + tincl - tc;
         if (ts + lane + 1 == a.T) a.Io[a.T] = excl + tincl;
     }
@@ -314,7 +319,7 @@ reduce_ss_kernel(MergeArgs a, uint32_t *ticket, const int32_t *gate, int32_t gat
                 uint32_t tc = 0;
                 if ((uint32_t)lane < mt)
                     for (uint32_t w = 0; w < wpt; ++w) tc += sh.ws[lane * wpt + w];
-                const uint32_t excl = span_lookback(a, ts, mt, tc, lane);
+                const uint32_t excl = span_lookback(a, g, ts, mt, tc, lane);
                 if (lane == 0) sh.span_excl = excl;
             }
             if (tid == 0) sh.ticket = next_ticket;
@@ -338,7 +343,7 @@ reduce_ss_kernel(MergeArgs a, uint32_t *ticket, const int32_t *gate, int32_t gat
             }
             if (warp == 0) {
                 const uint32_t tc = (uint32_t)lane < mt ? sh.tc[lane] : 0u;
-                const uint32_t excl = span_lookback(a, ts, mt, tc, lane);
+                const uint32_t excl = span_lookback(a, g, ts, mt, tc, lane);
                 if (lane == 0) sh.span_excl = excl;
             }
             if (tid == 0) sh.ticket = next_ticket;

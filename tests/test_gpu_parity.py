@@ -109,6 +109,41 @@ def test_reduce_sd_matches_oracle(pk, n, dens):
     assert np.array_equal(_bits(out), want.view(np.uint32))
 
 
+def _clustered(n, lo, hi, every, seed):
+    """Buffer whose tiles alternate between two densities: every `every`-th tile has density `hi`,
+    the others `lo` - the per-tile path decisions (list / lane walk / streaming, span fits / does not)
+    all occur inside one launch."""
+    a, b = wl.sparse_buffer(n, lo, seed=seed), wl.sparse_buffer(n, hi, seed=seed + 1)
+    tile = torch.arange(n) // wl.TILE
+    return torch.where(tile % every == every - 1, b, a)
+
+
+@pytest.mark.parametrize("lo,hi,every", ((0.002, 1.0, 16), (0.0, 0.3, 5), (0.6, 0.0, 2), (0.9, 0.01, 3)))
+def test_reduce_sd_mixed_tiles(pk, lo, hi, every):
+    n = 37 * wl.TILE + 1234
+    x = _clustered(n, lo, hi, every, seed=77)
+    local = wl.sparse_buffer(n, 0.5, seed=79)
+    xo = po.compress(_bits(x), "f32")
+    want = local.numpy().copy()
+    po.reduce_sd(xo, want)
+    got = local.cuda()
+    pk.reduce_sd(_upload(pk, xo), got)
+    assert np.array_equal(_bits(got), want.view(np.uint32))
+
+
+@pytest.mark.parametrize("lo,hi,every", ((0.002, 1.0, 16), (0.0, 0.5, 5), (0.7, 0.0, 2), (0.01, 0.9, 9)))
+def test_reduce_ss_mixed_tiles(pk, lo, hi, every):
+    n = 133 * wl.TILE + 77
+    x = _clustered(n, lo, hi, every, seed=81)
+    y = _clustered(n, lo, hi, every + 1, seed=83)
+    xo, yo = po.compress(_bits(x), "f32"), po.compress(_bits(y), "f32")
+    want = po.reduce_ss(xo, yo)
+    out = pk.alloc_pici(n, pk.F32)
+    out.B.fill_(-1); out.I.fill_(-1)
+    pk.reduce_ss(_upload(pk, xo), _upload(pk, yo), out, pk.alloc_workspace(n))
+    _assert_pici_equal(pk, out, want)
+
+
 @pytest.mark.parametrize("n", (1, 64, 4097, 3 * 4096 + 17, 1 << 20))
 @pytest.mark.parametrize("dx,dy", ((0.0, 0.0), (0.01, 0.01), (0.0, 0.2), (0.3, 0.02), (0.6, 0.6), (1.0, 1.0)))
 def test_reduce_ss_matches_oracle(pk, n, dx, dy):
