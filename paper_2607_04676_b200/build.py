@@ -44,7 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(os.path.join(_HERE, "build"), exist_ok=True)
     for src in SOURCES:
         obj = os.path.join(_HERE, "build", src.replace(".cu", ".o"))
-        cmd = [_nvcc()] + NVCC_FLAGS + \
+        cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("PICI_NVCC_EXTRA", "").split() + \
               (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)

@@ -202,9 +202,11 @@ int num_sms() {
     return cached[dev];
 }
 
+// Scratch for the scans: compress uses one status word per tile; reduce_ss uses one word per span plus
+// its per-iteration and per-group accumulators (merge.cu), bounded by T + 4096 more words.
 uint64_t scan_workspace_bytes(uint64_t n) {
     const uint64_t T = (n + kTile - 1) / kTile;
-    return (uint64_t)kWsHeaderBytes + ((T * 8 + 15) / 16) * 16;
+    return (uint64_t)kWsHeaderBytes + (2 * T + 4096) * 8;
 }
 
 template <int DT>
@@ -219,7 +221,7 @@ static cudaError_t launch_compress_t(const void *dense, uint64_t n, uint64_t *B,
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    cudaError_t e = cudaMemsetAsync(ws, 0, scan_workspace_bytes(n), s);
+    cudaError_t e = cudaMemsetAsync(ws, 0, (size_t)kWsHeaderBytes + T * 8, s);
     if (e != cudaSuccess) return e;
     uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
     const uint64_t cap = (uint64_t)num_sms() * Cfg::kMinBlocks;           // persistent: one resident wave

@@ -62,6 +62,13 @@ __device__ __forceinline__ uint2 ld_coherent_u2(const uint2 *p) {
     asm volatile("ld.global.L1::no_allocate.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p) : "memory");
     return v;
 }
+// Gather load of the scatter-add: a miss fetches 64 bytes from DRAM instead of the default 128-byte
+// line pair (probe on B200: 185 MB instead of 403 MB of DRAM reads for 2.7 M random 4-byte gathers).
+__device__ __forceinline__ uint32_t ld_gather_u32(const uint32_t *p) {
+    uint32_t v;
+    asm volatile("ld.global.L2::64B.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ ulonglong2 ldg_nc_u64x2(const uint64_t *p) {
     ulonglong2 v;
     asm volatile("ld.global.nc.L1::no_allocate.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "l"(p));
@@ -156,7 +163,7 @@ expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, co
                     if (jj < tile_nnz) {
                         ix[j] = list[jj];
                         av[j] = ldg_stream_u32(Au + jj);
-                        dv[j] = Du[ix[j]];
+                        dv[j] = ld_gather_u32(Du + ix[j]);
                     }
                 }
 #pragma unroll
@@ -334,7 +341,7 @@ scatter_add_sparse_kernel(const uint64_t *__restrict__ B, const uint32_t *__rest
                 if (jj < tile_nnz) {
                     ix[j] = list[jj];
                     av[j] = ldg_stream_u32(Au + jj);
-                    dv[j] = Du[ix[j]];
+                    dv[j] = ld_gather_u32(Du + ix[j]);
                 }
             }
 #pragma unroll

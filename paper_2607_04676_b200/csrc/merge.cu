@@ -11,36 +11,63 @@
 // B read as ONE little-endian bit string ARE the order of A.  The merge therefore never needs a dense
 // position: it is a 1-D merge of two (bit string, value stream) pairs, and I[t] is the number of
 // survivors before bit 4096*t.  The kernel works on SPANS of that string:
-//   * a CTA of 256 threads takes a group of 8 consecutive tiles by dynamic ticket and cuts it into
-//     spans of m = 8, 4, 2 or 1 tiles - the largest m whose X values, Y values and worst-case output
-//     all fit the CTA's shared-memory pool (read from Ix, Iy; one tile always fits).  Sparse inputs
-//     run 8 tiles per span (many tiles in flight, one look-back per 8 tiles), dense ones 1 tile per
-//     span with all 256 threads on it;
-//   * thread j owns the 16m-bit piece j of the span (128 / 64 / 32 / 16 bits: one coalesced load of
-//     consecutive pieces); the span's X and Y values are contiguous in Ax / Ay and are staged in the
-//     pool by two 1-D TMA bulk copies (16-byte aligned window, < 16-byte tail by plain loads);
-//   * x's and y's cursors come from the block-wide popc prefix of their own pieces, the candidate
-//     cursor from the popc prefix of the OR; every thread walks the set bits of its piece, adds, tests
-//     the predicate and packs its surviving sums into its own run of the pool's output region (runs
-//     start at the OR-prefix, so they never overlap);
-//   * the span's per-tile survivor counts go through the same per-tile decoupled look-back as compress
-//     (Phase 2), and the output region is written to Ao with coalesced stores.  Only spans that
-//     actually had a cancellation take the thread-by-thread copy.
+//   * a span is m = 16, 8, 4, 2 or 1 consecutive tiles, the same m for the whole launch: the largest
+//     whose AVERAGE contents fit one shared-memory stage (read on the device from Ix[T] + Iy[T]),
+//     halved while the launch has fewer than two spans per CTA;
+//   * the launch is COOPERATIVE with G CTAs of 512 threads (two per SM); CTA c takes spans c, c + G,
+//     c + 2G, ... and runs a two-stage software pipeline: while span i is walked, the whole of span
+//     i+1 - its Bx / By words (contiguous) and its X / Y value runs (contiguous in Ax / Ay) - is in
+//     flight into the other stage as four 1-D TMA bulk copies on one mbarrier; index entries are
+//     loaded two spans ahead so the copies never wait on them;
+//   * thread j owns the 8m-bit piece j of the span; x's and y's cursors come from the block-wide popc
+//     prefix of their own pieces, the candidate cursor from the popc prefix of the OR; every thread
+//     walks the set bits of its piece, adds, tests the predicate and packs its surviving sums into its
+//     own run of an output region (runs start at the OR-prefix, so they never overlap);
+//   * Phase 2 (exclusive scan of the counts) uses the round-robin structure: iteration
+//     `it` of the grid covers spans [it*G, (it+1)*G).  A CTA publishes its span's survivor count as
+//     (a) a per-span word, (b) an atomic add into the word of its group of 32 spans, (c) an atomic add
+//     into the word of its iteration; each word carries (how many have added, sum).  The prefix of
+//     span (it, c) = running sum of complete iterations + complete groups below c + the spans of its
+//     own group below c: three independent loads, ONE L2 round trip, 64 words per look-back (a flat
+//     decoupled look-back walks up to G/32 dependent hops here because the CTAs run in lock-step and
+//     nobody below has a prefix yet; a block-wide flat read hot-spots a few L2 lines - both measured);
+//   * a span's look-back and flush are DEFERRED behind the next span's walk (second output region),
+//     so one iteration of skew between CTAs is absorbed;
+//   * a span denser than the stage (the average said it would fit) is processed tile by tile in two
+//     sweeps (count, then emit) - one tile always fits.
 #include "launch.h"
 #include "pici_common.cuh"
 #include "../../include/pici.h"
 
 namespace pici {
 
-constexpr int kMergeWarps = 8;
+#ifdef PICI_MERGE_TRACE   // debug only: per-CTA, per-iteration %globaltimer stamps
+__device__ uint64_t *g_merge_trace;
+#define PICI_TR(it, k)                                                                      \
+    do {                                                                                    \
+        if (threadIdx.x == 0 && (it) < 16u) {                                               \
+            uint64_t t_;                                                                    \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                          \
+            g_merge_trace[((size_t)blockIdx.x * 16 + (it)) * 8 + (k)] = t_;                 \
+        }                                                                                   \
+    } while (0)
+#else
+#define PICI_TR(it, k) do { } while (0)
+#endif
+
+constexpr int kMergeWarps = 16;
 constexpr int kMergeThreads = kMergeWarps * 32;
-constexpr int kMaxSpan = 8;                             // tiles per ticket: 8, 4, 2 or 1
-constexpr uint32_t kPoolWords = 3 * kTile + 16;         // X window + Y window + output region of ONE tile
-constexpr int kMergeMinBlocks = 4;
+constexpr int kMaxSpan = 16;                            // tiles per span: 16, 8, 4, 2 or 1
+constexpr uint32_t kTileWords = 2 * kSide;              // u32 words of B per tile
+// stage = [Bx words of the span][By words][X window][Y window]; one full tile always fits
+constexpr uint32_t kStageWords = 2 * kTileWords + 2 * kTile + 16;
+constexpr uint32_t kOutWords = kTile;                   // candidates (bits of x | y) of a span
+constexpr uint32_t kPoolWords = 2 * kStageWords + 2 * kOutWords;   // two stages, two output regions
+constexpr int kMergeMinBlocks = 2;
+constexpr uint32_t kMaxGrid = 1024;                     // groups of 32 spans per iteration fit one warp
 
 struct MergeShared {
-    uint64_t mbar;
-    uint32_t ticket;
+    uint64_t mbar[2];
     uint32_t span_excl;               // exclusive prefix (survivors before the span) from the look-back
     uint32_t wxy[kMergeWarps];        // per-warp totals: popc(x piece) | popc(y piece) << 16
     uint32_t wu[kMergeWarps];         // per-warp totals: popc(x | y)
@@ -48,94 +75,143 @@ struct MergeShared {
     uint32_t tc[kMaxSpan];            // per-tile survivors of a span walked tile by tile
 };
 
-// Stage A[beg .. beg+cnt) (4-byte elements) at pool word `dstw` (a multiple of 4): element i lands at
-// pool[dstw + (beg & 3) + i].  Called by one warp; lane 0 issues the bulk copy (the caller has posted
-// the expected byte count), lanes 0..2 move the tail.
-__device__ __forceinline__ uint32_t bulk_bytes_of(uint32_t beg, uint32_t cnt) {
-    const uint64_t a_beg = (uint64_t)beg * 4, a_end = a_beg + (uint64_t)cnt * 4;
-    const uint64_t start_al = a_beg & ~15ull, end_dn = a_end & ~15ull;
-    return end_dn > start_al ? (uint32_t)(end_dn - start_al) : 0u;
-}
-__device__ __forceinline__ void stage_values(uint32_t *pool, uint32_t dstw, const uint32_t *__restrict__ A,
-                                             uint32_t beg, uint32_t cnt, uint32_t bar, int lane) {
-    if (cnt == 0) return;
-    const uint64_t a_beg = (uint64_t)beg * 4, a_end = a_beg + (uint64_t)cnt * 4;
-    const uint64_t start_al = a_beg & ~15ull, end_dn = a_end & ~15ull;
-    const uint32_t bulk = end_dn > start_al ? (uint32_t)(end_dn - start_al) : 0u;
-    if (bulk != 0 && lane == 0)
-        bulk_g2s(smem_u32(pool + dstw), reinterpret_cast<const unsigned char *>(A) + start_al, bulk, bar);
-    const uint64_t tail_beg = bulk != 0 ? end_dn : a_beg;
-    const uint32_t tail_cnt = (uint32_t)(a_end - tail_beg) / 4;
-    if ((uint32_t)lane < tail_cnt) pool[dstw + (uint32_t)(tail_beg - start_al) / 4 + lane] = A[tail_beg / 4 + lane];
-}
-
-
 struct MergeArgs {
     const uint64_t *Bx, *By;
     const uint32_t *Ix, *Iy, *Ax, *Ay;
     uint64_t *Bo;
     uint32_t *Io, *Ao;
-    uint64_t *status;
-    uint32_t T;
+    uint64_t *span_word;   // [spans]          (1 << 32) | survivors once published
+    uint64_t *grp_word;    // [iterations][ngrp] (adds << 48) + sum
+    uint64_t *iter_word;   // [iterations]       (adds << 48) + sum
+    uint32_t T, ngrp;
+    uint64_t a_limit;      // bytes of Ax / Ay that may be read: (n * 4) & ~15 (capacity >= n elements)
 };
+
+// ---- staging ------------------------------------------------------------------------------------
+// The values A[beg .. beg+cnt) are copied as ONE bulk copy of the 16-byte aligned window around them
+// (up to 12 bytes before and after belong to neighbouring spans of the same buffer; the window never
+// passes a_limit, so nothing outside the caller's capacity is read).  Only a run that ends in the last
+// < 16 bytes of a completely full buffer keeps a tail, moved by plain loads.
+struct Window {
+    uint64_t g_beg;    // byte offset in A of the window start
+    uint32_t bulk;     // bytes of the bulk copy (multiple of 16, may be 0)
+    uint32_t words;    // window length in words, multiple of 4 (what the stage reserves)
+    uint32_t first;    // word index inside the window of element 0
+    uint32_t tail_beg; // element index (relative to beg) where the plain-load tail starts; == cnt if none
+};
+__device__ __forceinline__ Window window_of(uint32_t beg, uint32_t cnt, uint64_t a_limit) {
+    Window w;
+    const uint64_t a_beg = (uint64_t)beg * 4, a_end = a_beg + (uint64_t)cnt * 4;
+    w.g_beg = a_beg & ~15ull;
+    const uint64_t end_up = (a_end + 15ull) & ~15ull;
+    const uint64_t end_bulk = cnt == 0 ? w.g_beg : (end_up <= a_limit ? end_up : (a_end & ~15ull));
+    w.bulk = end_bulk > w.g_beg ? (uint32_t)(end_bulk - w.g_beg) : 0u;
+    w.words = (uint32_t)((end_up - w.g_beg) / 4);
+    w.first = (uint32_t)(a_beg - w.g_beg) / 4;
+    const uint64_t covered = w.g_beg + w.bulk;   // bytes below this are in the bulk copy
+    w.tail_beg = covered >= a_end ? cnt : (covered > a_beg ? (uint32_t)((covered - a_beg) / 4) : 0u);
+    return w;
+}
+
+// Layout of a span inside a stage (m tiles per span).
+struct SpanLayout {
+    uint32_t By0;      // word of the span's By words (Bx words start at 0)
+    uint32_t Xb, Yb;   // word of the first x / y value
+    uint32_t tx;       // bytes the bulk copies signal on the mbarrier
+};
+__device__ __forceinline__ bool span_fits(uint32_t m, uint32_t nx, uint32_t ny, uint32_t mt) {
+    return 2u * m * kTileWords + nx + ny + 16u <= kStageWords && min(nx + ny, (uint32_t)kTile * mt) <= kOutWords;
+}
+
+// Warp 0: start the copies of the span of mt tiles at tile ts (m tiles per span) into `stage`; returns
+// its layout.  Other callers pass issue = false to get the layout only.
+__device__ __forceinline__ SpanLayout span_stage(const MergeArgs &a, uint32_t *stage, uint32_t bar, uint32_t ts, uint32_t m,
+                                                 uint32_t mt, uint32_t xs, uint32_t nx, uint32_t ys, uint32_t ny,
+                                                 bool issue, int lane) {
+    const Window wx = window_of(xs, nx, a.a_limit), wy = window_of(ys, ny, a.a_limit);
+    SpanLayout L;
+    L.By0 = m * kTileWords;
+    const uint32_t V = 2u * m * kTileWords;
+    L.Xb = V + wx.first;
+    L.Yb = V + wx.words + wy.first;
+    const uint32_t bbytes = mt * kTileWords * 4u;
+    L.tx = 2u * bbytes + wx.bulk + wy.bulk;
+    if (issue) {
+        if (lane == 0) {
+            fence_proxy_async_smem();
+            mbar_expect_tx(bar, L.tx);
+            bulk_g2s(smem_u32(stage), a.Bx + (size_t)ts * kSide, bbytes, bar);
+            bulk_g2s(smem_u32(stage + L.By0), a.By + (size_t)ts * kSide, bbytes, bar);
+            if (wx.bulk) bulk_g2s(smem_u32(stage + V), reinterpret_cast<const unsigned char *>(a.Ax) + wx.g_beg, wx.bulk, bar);
+            if (wy.bulk)
+                bulk_g2s(smem_u32(stage + V + wx.words), reinterpret_cast<const unsigned char *>(a.Ay) + wy.g_beg, wy.bulk, bar);
+        }
+        if (wx.tail_beg + lane < nx) stage[L.Xb + wx.tail_beg + lane] = a.Ax[xs + wx.tail_beg + lane];   // < 4 elements
+        if (wy.tail_beg + lane < ny) stage[L.Yb + wy.tail_beg + lane] = a.Ay[ys + wy.tail_beg + lane];
+    }
+    return L;
+}
+
+// This thread's 8*m-bit piece of the staged Bx / By words.  Pieces past the span's last tile are 0.
+__device__ __forceinline__ void read_piece(const uint32_t *stage, uint32_t By0, uint32_t m, uint32_t mt, int tid,
+                                           uint32_t (&ax)[4], uint32_t (&ay)[4]) {
+    ax[0] = ax[1] = ax[2] = ax[3] = 0u;
+    ay[0] = ay[1] = ay[2] = ay[3] = 0u;
+    if ((uint32_t)tid * m >= (uint32_t)kMergeThreads * mt) return;
+    const uint32_t *bx = stage, *by = stage + By0;
+    if (m == 16) {
+        const uint4 p = reinterpret_cast<const uint4 *>(bx)[tid], q = reinterpret_cast<const uint4 *>(by)[tid];
+        ax[0] = p.x; ax[1] = p.y; ax[2] = p.z; ax[3] = p.w;
+        ay[0] = q.x; ay[1] = q.y; ay[2] = q.z; ay[3] = q.w;
+    } else if (m == 8) {
+        const uint2 p = reinterpret_cast<const uint2 *>(bx)[tid], q = reinterpret_cast<const uint2 *>(by)[tid];
+        ax[0] = p.x; ax[1] = p.y;
+        ay[0] = q.x; ay[1] = q.y;
+    } else if (m == 4) {
+        ax[0] = bx[tid];
+        ay[0] = by[tid];
+    } else if (m == 2) {
+        ax[0] = reinterpret_cast<const uint16_t *>(bx)[tid];
+        ay[0] = reinterpret_cast<const uint16_t *>(by)[tid];
+    } else {
+        ax[0] = reinterpret_cast<const uint8_t *>(bx)[tid];
+        ay[0] = reinterpret_cast<const uint8_t *>(by)[tid];
+    }
+}
+__device__ __forceinline__ void store_piece(const MergeArgs &a, uint32_t ts, uint32_t m, uint32_t mt, int tid,
+                                            const uint32_t (&ao)[4]) {
+    if ((uint32_t)tid * m >= (uint32_t)kMergeThreads * mt) return;
+    const size_t wbase = (size_t)ts * kSide;
+    if (m == 16) reinterpret_cast<uint4 *>(a.Bo + wbase)[tid] = make_uint4(ao[0], ao[1], ao[2], ao[3]);
+    else if (m == 8) reinterpret_cast<uint2 *>(a.Bo + wbase)[tid] = make_uint2(ao[0], ao[1]);
+    else if (m == 4) reinterpret_cast<uint32_t *>(a.Bo + wbase)[tid] = ao[0];
+    else if (m == 2) reinterpret_cast<uint16_t *>(a.Bo + wbase)[tid] = (uint16_t)ao[0];
+    else reinterpret_cast<uint8_t *>(a.Bo + wbase)[tid] = (uint8_t)ao[0];
+}
 
 // What a thread keeps from one walk of a span.
 struct WalkOut {
     uint32_t k;            // this thread's survivors
-    uint32_t ko0;          // pool word of this thread's run in the output region
+    uint32_t ko0;          // word of this thread's run in the output region
     uint32_t sk;           // inclusive warp scan of k
-    uint32_t Ob;           // pool word where the span's output region starts
     uint32_t cand_total;   // candidates (bits of x | y) in the span
 };
 
-// One pass over the span of mt (<= m) tiles that starts at tile ts: stage the span's X and Y values,
-// load this thread's 16*m-bit piece of Bx / By, block-wide popc prefixes, walk the set bits.  With
-// EMIT the surviving sums are packed into the pool's output region and the piece of Bo is written;
-// without it only the survivors are counted (first sweep of a span that does not fit the pool).
-// On return sh.ws[] holds the per-warp survivor totals (after a __syncthreads()).
-template <bool EMIT>
-__device__ __forceinline__ WalkOut span_walk(const MergeArgs &a, uint32_t *pool, MergeShared &sh, uint32_t ts,
-                                             uint32_t m, uint32_t mt, uint32_t xs, uint32_t xe, uint32_t ys,
-                                             uint32_t ye, uint32_t bar, uint32_t &parity, int tid) {
+// Wait for the span's copies, read this thread's piece, block-wide popc prefixes, then the walk of the
+// piece's set bits: add, re-test, pack.  after_barrier1 is a caller hook run right behind the first
+// barrier (the pipelined caller starts the NEXT span's copies there).  With EMIT the surviving sums go
+// to `out` and ao[] receives the piece of Bo; without it the survivors are only counted.  Contains two
+// __syncthreads(); on return sh.ws[] holds the per-warp survivor totals and the stage is free.
+template <bool EMIT, typename Hook>
+__device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *out, MergeShared &sh, const SpanLayout &L,
+                                             uint32_t m, uint32_t mt, uint32_t (&ao)[4], uint32_t bar, uint32_t &parity,
+                                             int tid, Hook after_barrier1, uint32_t trace_it = 99u) {
     const int lane = tid & 31, warp = tid >> 5;
-    const uint32_t nx = xe - xs, ny = ye - ys;
-    const uint32_t xw = ((xs & 3u) + nx + 3u) & ~3u;              // X window (words)
-    const uint32_t yw = ((ys & 3u) + ny + 3u) & ~3u;              // Y window (words)
-    const uint32_t Xb = (xs & 3u), Yb = xw + (ys & 3u), Ob = xw + yw;   // first x / y / output word
-    const uint32_t tx = bulk_bytes_of(xs, nx) + bulk_bytes_of(ys, ny);
-
-    if (warp == 0) {
-        if (lane == 0 && tx != 0) {
-            fence_proxy_async_smem();
-            mbar_expect_tx(bar, tx);
-        }
-        stage_values(pool, 0, a.Ax, xs, nx, bar, lane);
-        stage_values(pool, xw, a.Ay, ys, ny, bar, lane);
-    }
-
-    // ---- this thread's piece of the span: 16*m bits of Bx, By ---------------------------------------
-    uint32_t ax[4] = {0, 0, 0, 0}, ay[4] = {0, 0, 0, 0};
-    const bool valid = (uint32_t)tid * m < (uint32_t)kMergeThreads * mt;   // piece inside the span's tiles
-    const size_t wbase = (size_t)ts * kSide;
-    if (valid) {
-        if (m == 8) {
-            const uint4 p = __ldg(reinterpret_cast<const uint4 *>(a.Bx + wbase) + tid);
-            const uint4 q = __ldg(reinterpret_cast<const uint4 *>(a.By + wbase) + tid);
-            ax[0] = p.x; ax[1] = p.y; ax[2] = p.z; ax[3] = p.w;
-            ay[0] = q.x; ay[1] = q.y; ay[2] = q.z; ay[3] = q.w;
-        } else if (m == 4) {
-            const uint2 p = __ldg(reinterpret_cast<const uint2 *>(a.Bx + wbase) + tid);
-            const uint2 q = __ldg(reinterpret_cast<const uint2 *>(a.By + wbase) + tid);
-            ax[0] = p.x; ax[1] = p.y;
-            ay[0] = q.x; ay[1] = q.y;
-        } else if (m == 2) {
-            ax[0] = __ldg(reinterpret_cast<const uint32_t *>(a.Bx + wbase) + tid);
-            ay[0] = __ldg(reinterpret_cast<const uint32_t *>(a.By + wbase) + tid);
-        } else {
-            ax[0] = __ldg(reinterpret_cast<const uint16_t *>(a.Bx + wbase) + tid);
-            ay[0] = __ldg(reinterpret_cast<const uint16_t *>(a.By + wbase) + tid);
-        }
-    }
+    mbar_wait(bar, parity);
+    parity ^= 1u;
+    PICI_TR(trace_it, 1);
+    uint32_t ax[4], ay[4];
+    read_piece(stage, L.By0, m, mt, tid, ax, ay);
     const uint32_t cx = __popc(ax[0]) + __popc(ax[1]) + __popc(ax[2]) + __popc(ax[3]);
     const uint32_t cy = __popc(ay[0]) + __popc(ay[1]) + __popc(ay[2]) + __popc(ay[3]);
     const uint32_t cu = __popc(ax[0] | ay[0]) + __popc(ax[1] | ay[1]) + __popc(ax[2] | ay[2]) + __popc(ax[3] | ay[3]);
@@ -145,28 +221,24 @@ __device__ __forceinline__ WalkOut span_walk(const MergeArgs &a, uint32_t *pool,
         sh.wxy[warp] = sxy;
         sh.wu[warp] = su;
     }
-    __syncthreads();  // #1: warp totals and the tail words of the staged values are visible
+    __syncthreads();  // #1: warp totals and any tail words of the staged values are visible
+    PICI_TR(trace_it, 2);
+    after_barrier1();
+    PICI_TR(trace_it, 3);
     uint32_t bxy = 0, bu = 0, cand_total = 0;
 #pragma unroll
-    for (int w = 0; w < kMergeWarps; ++w) {
-        const uint32_t p = sh.wxy[w], q = sh.wu[w];
-        if (w < warp) {
+    for (int q = 0; q < kMergeWarps; ++q) {
+        const uint32_t p = sh.wxy[q], u = sh.wu[q];
+        if (q < warp) {
             bxy += p;
-            bu += q;
+            bu += u;
         }
-        cand_total += q;
+        cand_total += u;
     }
-    uint32_t kx = Xb + (bxy & 0xFFFFu) + (sxy & 0xFFFFu) - cx;
-    uint32_t ky = Yb + (bxy >> 16) + (sxy >> 16) - cy;
-    const uint32_t ko0 = Ob + bu + su - cu;
+    uint32_t kx = L.Xb + (bxy & 0xFFFFu) + (sxy & 0xFFFFu) - cx;
+    uint32_t ky = L.Yb + (bxy >> 16) + (sxy >> 16) - cy;
+    const uint32_t ko0 = bu + su - cu;
     uint32_t ko = ko0;
-    if (tx != 0) {
-        mbar_wait(bar, parity);
-        parity ^= 1u;
-    }
-
-    // ---- walk the set bits of the piece: add, re-test, pack ------------------------------------------
-    uint32_t ao[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
         uint32_t u = ax[q] | ay[q], o = 0;
@@ -174,89 +246,123 @@ __device__ __forceinline__ WalkOut span_walk(const MergeArgs &a, uint32_t *pool,
             const uint32_t bit = u & (0u - u);
             u ^= bit;
             float x = 0.0f, y = 0.0f;
-            if (ax[q] & bit) x = __uint_as_float(pool[kx++]);
-            if (ay[q] & bit) y = __uint_as_float(pool[ky++]);
+            if (ax[q] & bit) x = __uint_as_float(stage[kx++]);
+            if (ay[q] & bit) y = __uint_as_float(stage[ky++]);
             const uint32_t sum = __float_as_uint(__fadd_rn(x, y));   // received + local (C9 #7)
             if (nz32(sum)) {
                 o |= bit;
-                if (EMIT) pool[ko] = sum;
+                if (EMIT) out[ko] = sum;
                 ++ko;
             }
         }
         ao[q] = o;
     }
-    if (EMIT && valid) {
-        if (m == 8) reinterpret_cast<uint4 *>(a.Bo + wbase)[tid] = make_uint4(ao[0], ao[1], ao[2], ao[3]);
-        else if (m == 4) reinterpret_cast<uint2 *>(a.Bo + wbase)[tid] = make_uint2(ao[0], ao[1]);
-        else if (m == 2) reinterpret_cast<uint32_t *>(a.Bo + wbase)[tid] = ao[0];
-        else reinterpret_cast<uint16_t *>(a.Bo + wbase)[tid] = (uint16_t)ao[0];
-    }
     WalkOut r;
     r.k = ko - ko0;
     r.ko0 = ko0;
     r.sk = warp_incl_scan(r.k, lane);
-    r.Ob = Ob;
     r.cand_total = cand_total;
     if (lane == 31) sh.ws[warp] = r.sk;
-    __syncthreads();  // #2: survivor totals and the output region are visible
+    __syncthreads();  // #2: survivor totals and the output region are visible; the stage is free
+    PICI_TR(trace_it, 4);
     return r;
 }
 
-// Phase 2 for a span (one warp; lane i < mt holds tc = survivors of tile ts + i).  ONE status word per
-// SPAN (index g): the aggregate is the span's survivor total, so a 32-entry look-back window covers
-// 32 * m tiles and the chain of hops a look-back has to walk is m times shorter than with per-tile
-// words (profiles/r1b: 49 % of reduce_ss's stall samples sat behind this look-back).  Publishes the
-// aggregate, looks back from span g, publishes the inclusive prefix, writes Io for the span's tiles.
-// Returns the number of survivors before tile ts.
-__device__ __forceinline__ uint32_t span_lookback(const MergeArgs &a, uint32_t g, uint32_t ts, uint32_t mt, uint32_t tc,
-                                                  int lane) {
-    const uint32_t tincl = warp_incl_scan((uint32_t)lane < mt ? tc : 0u, lane);
-    const uint32_t total = __shfl_sync(kFull, tincl, 31);
-    if (lane == 0) st_status(a.status + g, g == 0 ? kStPrefix : kStAggregate, total);
-    uint32_t excl = 0;
-    int64_t pos = g;
-    while (pos > 0) {
-        const int64_t idx = pos - 1 - lane;
-        uint64_t st;
-        unsigned pm, em, ns = 8;
-        for (;;) {
-            st = idx >= 0 ? ld_status(a.status + idx) : (kStPrefix << 32);
-            const uint32_t flag = (uint32_t)(st >> 32);
-            pm = __ballot_sync(kFull, flag == (uint32_t)kStPrefix);
-            em = __ballot_sync(kFull, flag == (uint32_t)kStEmpty);
-            const unsigned rel = pm ? ((pm & (0u - pm)) | ((pm & (0u - pm)) - 1u)) : kFull;
-            if ((em & rel) == 0u) {
-                excl += warp_sum(((1u << lane) & rel) ? (uint32_t)st : 0u);
-                break;
-            }
-            __nanosleep(ns);
-            if (ns < 64) ns += ns;
-        }
-        if (pm) break;
-        pos -= 32;
+// ---- Phase 2: counts -> exclusive prefix ------------------------------------------------------------
+constexpr uint64_t kOneAdd = 1ull << 48;
+__device__ __forceinline__ void red_add_u64(uint64_t *p, uint64_t v) {
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// One thread: make span (it, c)'s survivor count visible in its three words.  Every word is
+// self-contained (count and sum travel in one 64-bit access), so relaxed gpu-scope accesses suffice.
+__device__ __forceinline__ void publish_span(const MergeArgs &a, uint32_t g, uint32_t it, uint32_t c, uint32_t total) {
+    st_status(a.span_word + g, 1u, total);
+    red_add_u64(a.grp_word + (size_t)it * a.ngrp + (c >> 5), kOneAdd + total);
+    red_add_u64(a.iter_word + it, kOneAdd + total);
+}
+// Warp 0: survivors before span (it, c).  E = running sum of the complete iterations [0, E_it), carried
+// by the CTA from look-back to look-back (a CTA's `it` advances by one each time, so at most one
+// iteration word is read; the loop covers the general case).  All G spans of an iteration below `it`
+// exist, and so do all 32 spans of a group below c's.
+__device__ __forceinline__ uint32_t iter_lookback(const MergeArgs &a, uint32_t G, uint32_t it, uint32_t c, uint32_t &E,
+                                                  uint32_t &E_it, int lane) {
+    const uint32_t nfull = c >> 5, rem = c & 31u;
+    const uint64_t *gw = a.grp_word + (size_t)it * a.ngrp;
+    const uint64_t *sw = a.span_word + (size_t)it * G + (size_t)nfull * 32;
+    while (E_it + 1 < it) {   // not taken in the round-robin schedule
+        uint64_t v;
+        do { v = ld_status(a.iter_word + E_it); } while ((uint32_t)(v >> 48) != G);
+        E += (uint32_t)v;
+        ++E_it;
     }
-    if (lane == 0 && g != 0) st_status(a.status + g, kStPrefix, excl + total);
+    const bool need_iter = E_it < it;   // uniform
+    uint64_t vi, vg, vs;
+    unsigned ns = 8;
+    for (;;) {
+        vi = (need_iter && lane == 0) ? ld_status(a.iter_word + E_it) : ((uint64_t)G << 48);
+        vg = (uint32_t)lane < nfull ? ld_status(gw + lane) : (32ull << 48);
+        vs = (uint32_t)lane < rem ? ld_status(sw + lane) : (1ull << 32);
+        const bool ok = (uint32_t)(vi >> 48) == G && (uint32_t)(vg >> 48) == 32u && (uint32_t)(vs >> 32) != 0u;
+        if (__all_sync(kFull, ok)) break;
+        __nanosleep(ns);
+        if (ns < 128) ns += ns;
+    }
+    if (need_iter) {
+        E += __shfl_sync(kFull, (uint32_t)vi, 0);
+        ++E_it;
+    }
+    return E + warp_sum((uint32_t)vg + (uint32_t)vs);
+}
+
+// Io for the mt tiles of a span (one warp; lane i < mt holds tc = survivors of tile ts + i).
+__device__ __forceinline__ void write_index(const MergeArgs &a, uint32_t ts, uint32_t mt, uint32_t tc, uint32_t excl, int lane) {
+    const uint32_t tincl = warp_incl_scan((uint32_t)lane < mt ? tc : 0u, lane);
     if ((uint32_t)lane < mt) {
         a.Io[ts + lane] = excl + tincl - tc;
         if (ts + lane + 1 == a.T) a.Io[a.T] = excl + tincl;
     }
-    return excl;
 }
 
-// Write a walked span's output region to Ao + off.  packed: no cancellation happened, the region is
+// Write a walked span's output region to Ao + off.  Packed (no cancellation happened): the region is
 // contiguous; otherwise every thread moves its own run (before = survivors of earlier threads).
-__device__ __forceinline__ void span_flush(uint32_t *__restrict__ Ao, const uint32_t *pool, const WalkOut &r,
-                                           uint32_t off, uint32_t surv_total, uint32_t before, int tid) {
+__device__ __forceinline__ void span_flush(uint32_t *__restrict__ Ao, const uint32_t *out, const WalkOut &r, uint32_t off,
+                                           uint32_t surv_total, uint32_t before, int tid) {
     uint32_t *dst = Ao + off;
     if (surv_total == r.cand_total) {
-        for (uint32_t i = tid; i < surv_total; i += kMergeThreads) dst[i] = pool[r.Ob + i];
+        for (uint32_t i = tid; i < surv_total; i += kMergeThreads) dst[i] = out[i];
     } else {
-        for (uint32_t i = 0; i < r.k; ++i) dst[before + i] = pool[r.ko0 + i];
+        for (uint32_t i = 0; i < r.k; ++i) dst[before + i] = out[r.ko0 + i];
     }
 }
 
+// Survivors of earlier warps / of the whole block, from sh.ws[] (after walk_span's last barrier).
+__device__ __forceinline__ void survivor_sums(const MergeShared &sh, int warp, uint32_t &before, uint32_t &total) {
+    before = 0;
+    total = 0;
+#pragma unroll
+    for (int q = 0; q < kMergeWarps; ++q) {
+        const uint32_t v = sh.ws[q];
+        if (q < warp) before += v;
+        total += v;
+    }
+}
+
+// One tile (a span of m = 1) end to end, copies included: the slow path of a span that does not fit.
+// Starts with a __syncthreads() (the stage may still be read by the caller's previous step).
+template <bool EMIT>
+__device__ __forceinline__ WalkOut tile_pass(const MergeArgs &a, uint32_t *stage, uint32_t *out, MergeShared &sh,
+                                             uint32_t t, uint32_t x0, uint32_t x1, uint32_t y0, uint32_t y1, uint32_t bar,
+                                             uint32_t &parity, int tid) {
+    __syncthreads();
+    const SpanLayout L = span_stage(a, stage, bar, t, 1u, 1u, x0, x1 - x0, y0, y1 - y0, tid < 32, tid & 31);
+    uint32_t ao[4];
+    const WalkOut r = walk_span<EMIT>(stage, out, sh, L, 1u, 1u, ao, bar, parity, tid, [] {});
+    if (EMIT) store_piece(a, t, 1u, 1u, tid, ao);
+    return r;
+}
+
 __global__ void __launch_bounds__(kMergeThreads, kMergeMinBlocks)
-reduce_ss_kernel(MergeArgs a, uint32_t *ticket, const int32_t *gate, int32_t gate_value) {
+reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     extern __shared__ __align__(128) uint32_t pool[];
     __shared__ MergeShared sh;
     if (gate_closed(gate, gate_value)) return;
@@ -265,107 +371,171 @@ reduce_ss_kernel(MergeArgs a, uint32_t *ticket, const int32_t *gate, int32_t gat
     const int lane = tid & 31;
     const int warp = tid >> 5;
     const uint32_t T = a.T;
+    const uint32_t G = gridDim.x;
 
-    // ---- span length of this launch: the largest m in {8, 4, 2, 1} whose AVERAGE span (plus 1/16
-    // margin) fits the pool; read from the totals Ix[T], Iy[T].  A span that still does not fit is
-    // processed tile by tile in two sweeps (count, then emit), see below.
+    // ---- span length of this launch: the largest m whose AVERAGE span (plus 1/16 margin) fits a stage
+    // and the output region, from the totals Ix[T], Iy[T]; halved while the launch has fewer than two
+    // spans per CTA (ring chunks are a few thousand tiles).
     uint32_t m = 1;
     {
-        const uint64_t tot = (uint64_t)a.Ix[T] + (uint64_t)a.Iy[T];
+        const uint64_t tot = (uint64_t)__ldg(a.Ix + T) + (uint64_t)__ldg(a.Iy + T);
         const uint64_t avg = (tot + T - 1) / T;   // values per tile, X and Y together
 #pragma unroll
-        for (uint32_t mm = 8; mm >= 2; mm /= 2) {
-            const uint64_t need = avg * mm + min(avg, (uint64_t)kTile) * mm + 8;   // values + worst-case output
-            if (m == 1 && need + need / 16 <= kPoolWords) m = mm;
+        for (uint32_t mm = kMaxSpan; mm >= 2; mm /= 2) {
+            const uint64_t vals = avg * mm + 16, cand = min(avg, (uint64_t)kTile) * mm;
+            if (m == 1 && 2u * mm * kTileWords + vals + vals / 16 <= kStageWords && cand + cand / 16 <= kOutWords) m = mm;
         }
+        while (m > 1 && (T + m - 1) / m < 2u * G) m /= 2;
     }
     const uint32_t spans = (T + m - 1) / m;
-    const uint32_t bar = smem_u32(&sh.mbar);
+    uint32_t *const out = pool + 2 * kStageWords;
+    const uint32_t bar0 = smem_u32(&sh.mbar[0]), bar1 = smem_u32(&sh.mbar[1]);
     if (tid == 0) {
-        mbar_init(bar, 1);
-        sh.ticket = atomicAdd(ticket, 1u);
+        mbar_init(bar0, 1);
+        mbar_init(bar1, 1);
     }
     __syncthreads();
-    uint32_t parity = 0;
+    // Spans are dealt round-robin: CTA c takes spans c, c + G, c + 2G, ...  The launch is cooperative
+    // (all G CTAs are co-resident), so every span a look-back waits on belongs to a running CTA, and
+    // iteration i of a CTA only depends on iterations <= i of the others.
+    const uint32_t c = blockIdx.x;
+    uint32_t g = c, gn = c + G;
+    uint32_t par0 = 0, par1 = 0;
 
-    for (;;) {
-        const uint32_t g = sh.ticket;
-        if (g >= spans) break;
-        uint32_t next_ticket = 0;
-        if (tid == 0) next_ticket = atomicAdd(ticket, 1u);   // its latency hides behind this span
+    // lanes 0..mt of every warp hold the span's index entries I[ts .. ts+mt]
+    auto load_index = [&](uint32_t gg, uint32_t &ixl, uint32_t &iyl) {
+        ixl = 0;
+        iyl = 0;
+        if (gg < spans) {
+            const uint32_t ts = gg * m, j = min((uint32_t)lane, min(m, T - ts));
+            ixl = __ldg(a.Ix + ts + j);
+            iyl = __ldg(a.Iy + ts + j);
+        }
+    };
+    // warp 0: start the copies of span gg (index entries in ixl / iyl) unless it takes the slow path
+    auto start_copies = [&](uint32_t gg, uint32_t ixl, uint32_t iyl, uint32_t *stage, uint32_t bar) {
+        if (warp != 0 || gg >= spans) return;
+        const uint32_t ts = gg * m, mt = min(m, T - ts);
+        const uint32_t xs = __shfl_sync(kFull, ixl, 0), xe = __shfl_sync(kFull, ixl, mt);
+        const uint32_t ys = __shfl_sync(kFull, iyl, 0), ye = __shfl_sync(kFull, iyl, mt);
+        if (span_fits(m, xe - xs, ye - ys, mt)) span_stage(a, stage, bar, ts, m, mt, xs, xe - xs, ys, ye - ys, true, lane);
+    };
+
+    uint32_t ixl, iyl, ixn, iyn;
+    load_index(g, ixl, iyl);
+    load_index(gn, ixn, iyn);   // index entries run TWO spans ahead: the copies of span i+1 never wait on them
+    start_copies(g, ixl, iyl, pool, bar0);
+
+    // A walked span whose look-back and flush are deferred behind the next span's walk.
+    bool pending = false;
+    WalkOut pr = {0, 0, 0, 0};
+    uint32_t p_before = 0, p_total = 0, p_tc = 0, p_it = 0;
+    uint32_t E = 0, E_it = 0;   // warp 0: survivors of the complete iterations [0, E_it)
+    auto finish_pending = [&]() {   // contains one __syncthreads()
+        if (!pending) return;
+        const uint32_t pg = p_it * G + c, pts = pg * m, pmt = min(m, T - pts);
+        if (warp == 0) {
+            const uint32_t excl = iter_lookback(a, G, p_it, c, E, E_it, lane);
+            write_index(a, pts, pmt, p_tc, excl, lane);
+            if (lane == 0) sh.span_excl = excl;
+        }
+        __syncthreads();
+        PICI_TR(p_it + 1u, 5);
+        span_flush(a.Ao, out + (p_it & 1u) * kOutWords, pr, sh.span_excl, p_total, p_before, tid);
+        pending = false;
+    };
+
+    for (uint32_t it = 0; g < spans; ++it) {
+        const uint32_t s = it & 1u;
+        uint32_t *const stage = pool + s * kStageWords;
+        uint32_t *const stage_n = pool + (s ^ 1u) * kStageWords;
+        uint32_t *const out_s = out + s * kOutWords;
+        const uint32_t bar = s ? bar1 : bar0, bar_n = s ? bar0 : bar1;
+        uint32_t par = s ? par1 : par0;
+        PICI_TR(it, 0);
+
+        uint32_t ix2, iy2;
+        load_index(gn + G, ix2, iy2);
+        auto prefetch_span = [&] { start_copies(gn, ixn, iyn, stage_n, bar_n); };
 
         const uint32_t ts = g * m;
         const uint32_t mt = min(m, T - ts);
-        // lanes 0..mt of every warp hold the span's index entries
-        const uint32_t ixl = a.Ix[ts + min((uint32_t)lane, mt)];
-        const uint32_t iyl = a.Iy[ts + min((uint32_t)lane, mt)];
         const uint32_t xs = __shfl_sync(kFull, ixl, 0), xe = __shfl_sync(kFull, ixl, mt);
         const uint32_t ys = __shfl_sync(kFull, iyl, 0), ye = __shfl_sync(kFull, iyl, mt);
-        const uint32_t nxy = (xe - xs) + (ye - ys);
-        const bool fits = nxy + min(nxy, (uint32_t)kTile * mt) + 8u <= kPoolWords;   // uniform over the CTA
 
-        if (fits) {
-            // ---- one sweep: walk, Phase 2, flush ---------------------------------------------------------
-            const WalkOut r = span_walk<true>(a, pool, sh, ts, m, mt, xs, xe, ys, ye, bar, parity, tid);
-            uint32_t before = 0, surv_total = 0;
-#pragma unroll
-            for (int w = 0; w < kMergeWarps; ++w) {
-                const uint32_t v = sh.ws[w];
-                if (w < warp) before += v;
-                surv_total += v;
+        if (span_fits(m, xe - xs, ye - ys, mt)) {
+            // ---- walk now, publish the count, finish the PREVIOUS span, leave this one pending ----------
+            const SpanLayout L = span_stage(a, stage, bar, ts, m, mt, xs, xe - xs, ys, ye - ys, false, lane);
+            uint32_t ao[4];
+            const WalkOut r = walk_span<true>(stage, out_s, sh, L, m, mt, ao, bar, par, tid, prefetch_span, it);
+            uint32_t before, surv_total;
+            survivor_sums(sh, warp, before, surv_total);
+            if (tid == 0) publish_span(a, g, it, c, surv_total);
+            store_piece(a, ts, m, mt, tid, ao);
+            uint32_t tc = 0;
+            if (warp == 0 && (uint32_t)lane < mt) {
+                const uint32_t wpt = (uint32_t)kMergeWarps / m;   // a tile is covered by 16/m consecutive warps
+                for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
             }
-            if (warp == 0) {
-                const uint32_t wpt = (uint32_t)kMergeWarps / m;   // a tile is covered by 8/m consecutive warps
-                uint32_t tc = 0;
-                if ((uint32_t)lane < mt)
-                    for (uint32_t w = 0; w < wpt; ++w) tc += sh.ws[lane * wpt + w];
-                const uint32_t excl = span_lookback(a, g, ts, mt, tc, lane);
-                if (lane == 0) sh.span_excl = excl;
-            }
-            if (tid == 0) sh.ticket = next_ticket;
-            __syncthreads();  // #3: the span's offset in Ao is known
-            span_flush(a.Ao, pool, r, sh.span_excl, surv_total, before + r.sk - r.k, tid);
-            __syncthreads();  // #4: the pool may be reused
+            finish_pending();
+            PICI_TR(it, 6);
+            pending = true;
+            pr = r;
+            p_before = before + r.sk - r.k;
+            p_total = surv_total;
+            p_tc = tc;
+            p_it = it;
         } else {
             // ---- the span does not fit: tile by tile (one tile always fits), two sweeps -----------------
-            // Sweep 1 counts the survivors of every tile so that all aggregates are published before
+            // Sweep 1 counts the survivors of every tile so that the span's count is published before
             // anything waits (no other CTA ever waits on a half-processed span); sweep 2 emits.
+            __syncthreads();
+            finish_pending();
+            prefetch_span();
             for (uint32_t i = 0; i < mt; ++i) {
                 const uint32_t x0 = __shfl_sync(kFull, ixl, i), x1 = __shfl_sync(kFull, ixl, i + 1);
                 const uint32_t y0 = __shfl_sync(kFull, iyl, i), y1 = __shfl_sync(kFull, iyl, i + 1);
-                span_walk<false>(a, pool, sh, ts + i, 1u, 1u, x0, x1, y0, y1, bar, parity, tid);
+                tile_pass<false>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, bar, par, tid);
                 if (tid == 0) {
-                    uint32_t c = 0;
-                    for (int w = 0; w < kMergeWarps; ++w) c += sh.ws[w];
-                    sh.tc[i] = c;
+                    uint32_t cnt = 0;
+                    for (int q = 0; q < kMergeWarps; ++q) cnt += sh.ws[q];
+                    sh.tc[i] = cnt;
                 }
-                __syncthreads();
             }
+            __syncthreads();
+            uint32_t span_total = 0;
+            for (uint32_t i = 0; i < mt; ++i) span_total += sh.tc[i];
+            if (tid == 0) publish_span(a, g, it, c, span_total);
             if (warp == 0) {
-                const uint32_t tc = (uint32_t)lane < mt ? sh.tc[lane] : 0u;
-                const uint32_t excl = span_lookback(a, g, ts, mt, tc, lane);
+                const uint32_t excl = iter_lookback(a, G, it, c, E, E_it, lane);
+                write_index(a, ts, mt, (uint32_t)lane < mt ? sh.tc[lane] : 0u, excl, lane);
                 if (lane == 0) sh.span_excl = excl;
             }
-            if (tid == 0) sh.ticket = next_ticket;
             __syncthreads();
             uint32_t off = sh.span_excl;
             for (uint32_t i = 0; i < mt; ++i) {
                 const uint32_t x0 = __shfl_sync(kFull, ixl, i), x1 = __shfl_sync(kFull, ixl, i + 1);
                 const uint32_t y0 = __shfl_sync(kFull, iyl, i), y1 = __shfl_sync(kFull, iyl, i + 1);
-                const WalkOut r = span_walk<true>(a, pool, sh, ts + i, 1u, 1u, x0, x1, y0, y1, bar, parity, tid);
-                uint32_t before = 0, surv_total = 0;
-#pragma unroll
-                for (int w = 0; w < kMergeWarps; ++w) {
-                    const uint32_t v = sh.ws[w];
-                    if (w < warp) before += v;
-                    surv_total += v;
-                }
-                span_flush(a.Ao, pool, r, off, surv_total, before + r.sk - r.k, tid);
+                const WalkOut r = tile_pass<true>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, bar, par, tid);
+                uint32_t before, surv_total;
+                survivor_sums(sh, warp, before, surv_total);
+                span_flush(a.Ao, out_s, r, off, surv_total, before + r.sk - r.k, tid);
                 off += surv_total;
-                __syncthreads();
             }
+            __syncthreads();
         }
+
+        // ---- rotate the pipeline -------------------------------------------------------------------------
+        if (s) par1 = par; else par0 = par;
+        g = gn;
+        gn += G;
+        ixl = ixn;
+        iyl = iyn;
+        ixn = ix2;
+        iyn = iy2;
     }
+    __syncthreads();
+    finish_pending();
 }
 
 cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void *Ax, const uint64_t *By,
@@ -375,25 +545,45 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
     const uint64_t T = (n + kTile - 1) / kTile;
     const size_t smem = (size_t)kPoolWords * sizeof(uint32_t);
     static bool configured = false;
+    static int per_sm = 0;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(reduce_ss_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
+        int v = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, reduce_ss_kernel, kMergeThreads, smem);
+        if (e != cudaSuccess) return e;
+        per_sm = v > 0 ? v : 1;
         configured = true;
     }
-    cudaError_t e = cudaMemsetAsync(ws, 0, scan_workspace_bytes(n), s);
-    if (e != cudaSuccess) return e;
-    uint64_t blocks = T;   // the span length is chosen on the device; surplus CTAs find no ticket and exit
-    const uint64_t cap = (uint64_t)num_sms() * kMergeMinBlocks;   // persistent: one resident wave
+    uint64_t blocks = T;   // the span length is chosen on the device; surplus CTAs find no span and exit
+    uint64_t cap = (uint64_t)num_sms() * per_sm;   // cooperative: exactly one co-resident wave
+    if (cap > kMaxGrid) cap = kMaxGrid;
     if (blocks > cap) blocks = cap;
-    uint32_t *ticket = reinterpret_cast<uint32_t *>(ws);
-    uint64_t *status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);
+    // workspace: [header][span words: T][iteration words: iters][group words: iters * ngrp], all zero
+    const uint64_t iters = (T + blocks - 1) / blocks, ngrp = (blocks + 31) / 32;
+    const uint64_t words = T + iters * (1 + ngrp);
+    if ((uint64_t)kWsHeaderBytes + words * 8 > scan_workspace_bytes(n)) return cudaErrorInvalidValue;   // cannot happen
+    cudaError_t e = cudaMemsetAsync(ws, 0, (size_t)kWsHeaderBytes + words * 8, s);
+    if (e != cudaSuccess) return e;
+    uint64_t *base = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);
     MergeArgs a;
     a.Bx = Bx; a.By = By; a.Ix = Ix; a.Iy = Iy;
     a.Ax = reinterpret_cast<const uint32_t *>(Ax); a.Ay = reinterpret_cast<const uint32_t *>(Ay);
     a.Bo = Bo; a.Io = Io; a.Ao = reinterpret_cast<uint32_t *>(Ao);
-    a.status = status; a.T = (uint32_t)T;
-    reduce_ss_kernel<<<(unsigned)blocks, kMergeThreads, smem, s>>>(a, ticket, g.ptr, g.value);
-    return cudaGetLastError();
+    a.span_word = base; a.iter_word = base + T; a.grp_word = base + T + iters;
+    a.T = (uint32_t)T; a.ngrp = (uint32_t)ngrp;
+    a.a_limit = (n * 4) & ~15ull;
+#ifdef PICI_MERGE_TRACE
+    {
+        uint64_t *tr = base + words;   // needs a workspace with 296 * 16 * 8 spare words
+        cudaMemcpyToSymbolAsync(g_merge_trace, &tr, sizeof(tr), 0, cudaMemcpyHostToDevice, s);
+    }
+#endif
+    const int32_t *gate_ptr = g.ptr;
+    int32_t gate_value = g.value;
+    void *params[] = {&a, &gate_ptr, &gate_value};
+    return cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(reduce_ss_kernel), dim3((unsigned)blocks),
+                                       dim3(kMergeThreads), params, smem, s);
 }
 
 }  // namespace pici
