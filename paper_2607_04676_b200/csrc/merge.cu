@@ -66,14 +66,39 @@ constexpr uint32_t kPoolWords = 2 * kStageWords + 2 * kOutWords;   // two stages
 constexpr int kMergeMinBlocks = 2;
 constexpr uint32_t kMaxGrid = 1024;                     // groups of 32 spans per iteration fit one warp
 
+// What the staging warp tells the walkers about the span in a stage.
+struct SpanInfo {
+    uint32_t fits;      // 0: the span takes the slow path (nothing was copied)
+    uint32_t Xb, Yb;    // stage word of the first x / y value
+    uint32_t xs, ys;    // Ix[ts], Iy[ts]
+};
 struct MergeShared {
-    uint64_t mbar[2];
-    uint32_t span_excl;               // exclusive prefix (survivors before the span) from the look-back
+    uint64_t full[2];         // mbarrier: the copies of the span in stage s have landed
+    uint64_t stage_free[2];   // mbarrier: the walkers are done with stage s
+    uint64_t counts[2];       // mbarrier: tcs[s] is written and the span's count is published
+    uint64_t lb_done[2];      // mbarrier: excl[s] is written
+    uint64_t slow_bar;        // mbarrier: copies of the slow path
+    SpanInfo info[2];
+    uint32_t excl[2];                 // survivors before the span (from the look-back)
+    uint32_t tcs[2][kMaxSpan];        // per-tile survivors of the span
     uint32_t wxy[kMergeWarps];        // per-warp totals: popc(x piece) | popc(y piece) << 16
     uint32_t wu[kMergeWarps];         // per-warp totals: popc(x | y)
     uint32_t ws[kMergeWarps];         // per-warp totals: survivors
-    uint32_t tc[kMaxSpan];            // per-tile survivors of a span walked tile by tile
 };
+// Barrier of the 16 walker warps (the staging warp never joins it).
+__device__ __forceinline__ void walkers_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kMergeThreads) : "memory"); }
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0u;
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 
 struct MergeArgs {
     const uint64_t *Bx, *By;
@@ -197,21 +222,18 @@ struct WalkOut {
     uint32_t cand_total;   // candidates (bits of x | y) in the span
 };
 
-// Wait for the span's copies, read this thread's piece, block-wide popc prefixes, then the walk of the
-// piece's set bits: add, re-test, pack.  after_barrier1 is a caller hook run right behind the first
-// barrier (the pipelined caller starts the NEXT span's copies there).  With EMIT the surviving sums go
-// to `out` and ao[] receives the piece of Bo; without it the survivors are only counted.  Contains two
-// __syncthreads(); on return sh.ws[] holds the per-warp survivor totals and the stage is free.
-template <bool EMIT, typename Hook>
-__device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *out, MergeShared &sh, const SpanLayout &L,
-                                             uint32_t m, uint32_t mt, uint32_t (&ao)[4], uint32_t bar, uint32_t &parity,
-                                             int tid, Hook after_barrier1, uint32_t trace_it = 99u) {
+// Read this thread's piece of the staged span, block-wide popc prefixes, then the walk of the piece's
+// set bits: add, re-test, pack.  The caller has waited for the span's copies.  With EMIT the surviving
+// sums go to `out` and ao[] receives the piece of Bo; without it the survivors are only counted.
+// Contains two walkers_sync(); on return sh.ws[] holds the per-warp survivor totals and nobody reads
+// the stage any more.
+template <bool EMIT>
+__device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *out, MergeShared &sh, uint32_t By0, uint32_t Xb,
+                                             uint32_t Yb, uint32_t m, uint32_t mt, uint32_t (&ao)[4], int tid,
+                                             uint32_t trace_it = 99u) {
     const int lane = tid & 31, warp = tid >> 5;
-    mbar_wait(bar, parity);
-    parity ^= 1u;
-    PICI_TR(trace_it, 1);
     uint32_t ax[4], ay[4];
-    read_piece(stage, L.By0, m, mt, tid, ax, ay);
+    read_piece(stage, By0, m, mt, tid, ax, ay);
     const uint32_t cx = __popc(ax[0]) + __popc(ax[1]) + __popc(ax[2]) + __popc(ax[3]);
     const uint32_t cy = __popc(ay[0]) + __popc(ay[1]) + __popc(ay[2]) + __popc(ay[3]);
     const uint32_t cu = __popc(ax[0] | ay[0]) + __popc(ax[1] | ay[1]) + __popc(ax[2] | ay[2]) + __popc(ax[3] | ay[3]);
@@ -221,10 +243,8 @@ __device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *ou
         sh.wxy[warp] = sxy;
         sh.wu[warp] = su;
     }
-    __syncthreads();  // #1: warp totals and any tail words of the staged values are visible
+    walkers_sync();  // #1: warp totals are visible
     PICI_TR(trace_it, 2);
-    after_barrier1();
-    PICI_TR(trace_it, 3);
     uint32_t bxy = 0, bu = 0, cand_total = 0;
 #pragma unroll
     for (int q = 0; q < kMergeWarps; ++q) {
@@ -235,8 +255,8 @@ __device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *ou
         }
         cand_total += u;
     }
-    uint32_t kx = L.Xb + (bxy & 0xFFFFu) + (sxy & 0xFFFFu) - cx;
-    uint32_t ky = L.Yb + (bxy >> 16) + (sxy >> 16) - cy;
+    uint32_t kx = Xb + (bxy & 0xFFFFu) + (sxy & 0xFFFFu) - cx;
+    uint32_t ky = Yb + (bxy >> 16) + (sxy >> 16) - cy;
     const uint32_t ko0 = bu + su - cu;
     uint32_t ko = ko0;
 #pragma unroll
@@ -263,7 +283,7 @@ __device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *ou
     r.sk = warp_incl_scan(r.k, lane);
     r.cand_total = cand_total;
     if (lane == 31) sh.ws[warp] = r.sk;
-    __syncthreads();  // #2: survivor totals and the output region are visible; the stage is free
+    walkers_sync();  // #2: survivor totals and the output region are visible; the stage is no longer read
     PICI_TR(trace_it, 4);
     return r;
 }
@@ -347,21 +367,26 @@ __device__ __forceinline__ void survivor_sums(const MergeShared &sh, int warp, u
     }
 }
 
-// One tile (a span of m = 1) end to end, copies included: the slow path of a span that does not fit.
-// Starts with a __syncthreads() (the stage may still be read by the caller's previous step).
+// One tile (a span of m = 1) end to end, copies included (walker warp 0 issues them on slow_bar): the
+// slow path of a span that does not fit.  Starts with a walkers_sync() (the stage may still be read).
 template <bool EMIT>
 __device__ __forceinline__ WalkOut tile_pass(const MergeArgs &a, uint32_t *stage, uint32_t *out, MergeShared &sh,
                                              uint32_t t, uint32_t x0, uint32_t x1, uint32_t y0, uint32_t y1, uint32_t bar,
                                              uint32_t &parity, int tid) {
-    __syncthreads();
+    walkers_sync();
     const SpanLayout L = span_stage(a, stage, bar, t, 1u, 1u, x0, x1 - x0, y0, y1 - y0, tid < 32, tid & 31);
+    mbar_wait(bar, parity);
+    parity ^= 1u;
     uint32_t ao[4];
-    const WalkOut r = walk_span<EMIT>(stage, out, sh, L, 1u, 1u, ao, bar, parity, tid, [] {});
+    const WalkOut r = walk_span<EMIT>(stage, out, sh, L.By0, L.Xb, L.Yb, 1u, 1u, ao, tid);
     if (EMIT) store_piece(a, t, 1u, 1u, tid, ao);
     return r;
 }
 
-__global__ void __launch_bounds__(kMergeThreads, kMergeMinBlocks)
+
+constexpr int kMergeLaunchThreads = kMergeThreads + 32;   // 16 walker warps + the staging / scan warp
+
+__global__ void __launch_bounds__(kMergeLaunchThreads, kMergeMinBlocks)
 reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     extern __shared__ __align__(128) uint32_t pool[];
     __shared__ MergeShared sh;
@@ -389,152 +414,178 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     }
     const uint32_t spans = (T + m - 1) / m;
     uint32_t *const out = pool + 2 * kStageWords;
-    const uint32_t bar0 = smem_u32(&sh.mbar[0]), bar1 = smem_u32(&sh.mbar[1]);
+    const uint32_t full0 = smem_u32(&sh.full[0]), free0 = smem_u32(&sh.stage_free[0]);
+    const uint32_t cnt0 = smem_u32(&sh.counts[0]), lbd0 = smem_u32(&sh.lb_done[0]);
+    const uint32_t slow_bar = smem_u32(&sh.slow_bar);
     if (tid == 0) {
-        mbar_init(bar0, 1);
-        mbar_init(bar1, 1);
+#pragma unroll
+        for (uint32_t s = 0; s < 2; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(free0 + 8 * s, 1);
+            mbar_init(cnt0 + 8 * s, 1);
+            mbar_init(lbd0 + 8 * s, 1);
+        }
+        mbar_init(slow_bar, 1);
     }
     __syncthreads();
-    // Spans are dealt round-robin: CTA c takes spans c, c + G, c + 2G, ...  The launch is cooperative
-    // (all G CTAs are co-resident), so every span a look-back waits on belongs to a running CTA, and
-    // iteration i of a CTA only depends on iterations <= i of the others.
+    // Spans are dealt round-robin: CTA c takes spans c, c + G, c + 2G, ...; j counts this CTA's spans.
+    // The launch is cooperative (all G CTAs are co-resident), so every span a look-back waits on
+    // belongs to a running CTA, and span j of a CTA only depends on spans <= j of the others.
     const uint32_t c = blockIdx.x;
-    uint32_t g = c, gn = c + G;
-    uint32_t par0 = 0, par1 = 0;
 
-    // lanes 0..mt of every warp hold the span's index entries I[ts .. ts+mt]
-    auto load_index = [&](uint32_t gg, uint32_t &ixl, uint32_t &iyl) {
-        ixl = 0;
-        iyl = 0;
-        if (gg < spans) {
-            const uint32_t ts = gg * m, j = min((uint32_t)lane, min(m, T - ts));
-            ixl = __ldg(a.Ix + ts + j);
-            iyl = __ldg(a.Iy + ts + j);
+    if (warp == kMergeWarps) {
+        // =============================== staging / scan warp ===============================
+        // For this CTA's span j (stage s = j & 1): (A) once the walkers have left stage s, start the
+        // copies of span j + 2 into it; (B) once span j's count is published, take its prefix, write
+        // its index entries and hand the prefix to the walkers.  Whichever is ready first is served.
+        auto load_index = [&](uint32_t gg, uint32_t &ixl, uint32_t &iyl) {   // lanes 0..mt hold I[ts .. ts+mt]
+            ixl = 0;
+            iyl = 0;
+            if (gg < spans) {
+                const uint32_t ts = gg * m, jj = min((uint32_t)lane, min(m, T - ts));
+                ixl = __ldg(a.Ix + ts + jj);
+                iyl = __ldg(a.Iy + ts + jj);
+            }
+        };
+        auto prepare = [&](uint32_t gg, uint32_t ixl, uint32_t iyl, uint32_t s) {
+            if (gg >= spans) return;
+            const uint32_t ts = gg * m, mt = min(m, T - ts);
+            const uint32_t xs = __shfl_sync(kFull, ixl, 0), xe = __shfl_sync(kFull, ixl, mt);
+            const uint32_t ys = __shfl_sync(kFull, iyl, 0), ye = __shfl_sync(kFull, iyl, mt);
+            const bool fits = span_fits(m, xe - xs, ye - ys, mt);
+            const SpanLayout L = span_stage(a, pool + s * kStageWords, full0 + 8 * s, ts, m, mt, xs, xe - xs, ys, ye - ys, false, lane);
+            if (lane == 0) {
+                sh.info[s].fits = fits ? 1u : 0u;
+                sh.info[s].Xb = L.Xb;
+                sh.info[s].Yb = L.Yb;
+                sh.info[s].xs = xs;
+                sh.info[s].ys = ys;
+            }
+            __syncwarp();
+            if (fits) span_stage(a, pool + s * kStageWords, full0 + 8 * s, ts, m, mt, xs, xe - xs, ys, ye - ys, true, lane);
+            else if (lane == 0) mbar_arrive(full0 + 8 * s);   // nothing to copy: the walkers stage tile by tile
+        };
+        uint32_t ixa, iya, ixb, iyb;
+        load_index(c, ixa, iya);
+        load_index(c + G, ixb, iyb);
+        prepare(c, ixa, iya, 0u);
+        prepare(c + G, ixb, iyb, 1u);
+        load_index(c + 2 * G, ixa, iya);   // entries of the next span to prepare, one span ahead
+        uint32_t E = 0, E_it = 0;          // survivors of the complete iterations [0, E_it)
+        for (uint32_t j = 0; c + j * G < spans; ++j) {
+            const uint32_t s = j & 1u, ph = (j >> 1) & 1u;
+            const uint32_t g = c + j * G, ts = g * m, mt = min(m, T - ts);
+            bool issued = false, looked = false;
+            while (!(issued && looked)) {
+                if (!issued && mbar_test(free0 + 8 * s, ph)) {
+                    prepare(g + 2 * G, ixa, iya, s);
+                    load_index(g + 3 * G, ixa, iya);
+                    issued = true;
+                }
+                if (!looked && mbar_test(cnt0 + 8 * s, ph)) {
+                    const uint32_t excl = iter_lookback(a, G, j, c, E, E_it, lane);
+                    write_index(a, ts, mt, (uint32_t)lane < mt ? sh.tcs[s][lane] : 0u, excl, lane);
+                    if (lane == 0) {
+                        sh.excl[s] = excl;
+                        mbar_arrive(lbd0 + 8 * s);
+                    }
+                    looked = true;
+                }
+            }
         }
-    };
-    // warp 0: start the copies of span gg (index entries in ixl / iyl) unless it takes the slow path
-    auto start_copies = [&](uint32_t gg, uint32_t ixl, uint32_t iyl, uint32_t *stage, uint32_t bar) {
-        if (warp != 0 || gg >= spans) return;
-        const uint32_t ts = gg * m, mt = min(m, T - ts);
-        const uint32_t xs = __shfl_sync(kFull, ixl, 0), xe = __shfl_sync(kFull, ixl, mt);
-        const uint32_t ys = __shfl_sync(kFull, iyl, 0), ye = __shfl_sync(kFull, iyl, mt);
-        if (span_fits(m, xe - xs, ye - ys, mt)) span_stage(a, stage, bar, ts, m, mt, xs, xe - xs, ys, ye - ys, true, lane);
-    };
+        return;
+    }
 
-    uint32_t ixl, iyl, ixn, iyn;
-    load_index(g, ixl, iyl);
-    load_index(gn, ixn, iyn);   // index entries run TWO spans ahead: the copies of span i+1 never wait on them
-    start_copies(g, ixl, iyl, pool, bar0);
-
-    // A walked span whose look-back and flush are deferred behind the next span's walk.
+    // ======================================= walker warps =======================================
+    // A walked span whose flush is deferred behind the next span's walk: its count is published at
+    // once, the staging warp takes its prefix meanwhile.
     bool pending = false;
     WalkOut pr = {0, 0, 0, 0};
-    uint32_t p_before = 0, p_total = 0, p_tc = 0, p_it = 0;
-    uint32_t E = 0, E_it = 0;   // warp 0: survivors of the complete iterations [0, E_it)
-    auto finish_pending = [&]() {   // contains one __syncthreads()
+    uint32_t p_before = 0, p_total = 0, p_j = 0;
+    auto finish_pending = [&]() {
         if (!pending) return;
-        const uint32_t pg = p_it * G + c, pts = pg * m, pmt = min(m, T - pts);
-        if (warp == 0) {
-            const uint32_t excl = iter_lookback(a, G, p_it, c, E, E_it, lane);
-            write_index(a, pts, pmt, p_tc, excl, lane);
-            if (lane == 0) sh.span_excl = excl;
-        }
-        __syncthreads();
-        PICI_TR(p_it + 1u, 5);
-        span_flush(a.Ao, out + (p_it & 1u) * kOutWords, pr, sh.span_excl, p_total, p_before, tid);
+        const uint32_t ps = p_j & 1u;
+        mbar_wait(lbd0 + 8 * ps, (p_j >> 1) & 1u);
+        PICI_TR(p_j + 1u, 5);
+        span_flush(a.Ao, out + ps * kOutWords, pr, sh.excl[ps], p_total, p_before, tid);
         pending = false;
     };
+    uint32_t slow_par = 0;
 
-    for (uint32_t it = 0; g < spans; ++it) {
-        const uint32_t s = it & 1u;
+    for (uint32_t j = 0; c + j * G < spans; ++j) {
+        const uint32_t s = j & 1u, ph = (j >> 1) & 1u;
+        const uint32_t g = c + j * G, ts = g * m, mt = min(m, T - ts);
         uint32_t *const stage = pool + s * kStageWords;
-        uint32_t *const stage_n = pool + (s ^ 1u) * kStageWords;
         uint32_t *const out_s = out + s * kOutWords;
-        const uint32_t bar = s ? bar1 : bar0, bar_n = s ? bar0 : bar1;
-        uint32_t par = s ? par1 : par0;
-        PICI_TR(it, 0);
+        PICI_TR(j, 0);
+        mbar_wait(full0 + 8 * s, ph);
+        PICI_TR(j, 1);
+        const SpanInfo info = sh.info[s];
 
-        uint32_t ix2, iy2;
-        load_index(gn + G, ix2, iy2);
-        auto prefetch_span = [&] { start_copies(gn, ixn, iyn, stage_n, bar_n); };
-
-        const uint32_t ts = g * m;
-        const uint32_t mt = min(m, T - ts);
-        const uint32_t xs = __shfl_sync(kFull, ixl, 0), xe = __shfl_sync(kFull, ixl, mt);
-        const uint32_t ys = __shfl_sync(kFull, iyl, 0), ye = __shfl_sync(kFull, iyl, mt);
-
-        if (span_fits(m, xe - xs, ye - ys, mt)) {
-            // ---- walk now, publish the count, finish the PREVIOUS span, leave this one pending ----------
-            const SpanLayout L = span_stage(a, stage, bar, ts, m, mt, xs, xe - xs, ys, ye - ys, false, lane);
+        if (info.fits) {
+            // ---- walk now, publish the count, flush the PREVIOUS span, leave this one pending -----------
             uint32_t ao[4];
-            const WalkOut r = walk_span<true>(stage, out_s, sh, L, m, mt, ao, bar, par, tid, prefetch_span, it);
+            const WalkOut r = walk_span<true>(stage, out_s, sh, m * kTileWords, info.Xb, info.Yb, m, mt, ao, tid, j);
             uint32_t before, surv_total;
             survivor_sums(sh, warp, before, surv_total);
-            if (tid == 0) publish_span(a, g, it, c, surv_total);
-            store_piece(a, ts, m, mt, tid, ao);
-            uint32_t tc = 0;
-            if (warp == 0 && (uint32_t)lane < mt) {
+            if (warp == 0) {
+                if (lane == 0) {
+                    mbar_arrive(free0 + 8 * s);               // every walker is past barrier #2
+                    publish_span(a, g, j, c, surv_total);
+                }
                 const uint32_t wpt = (uint32_t)kMergeWarps / m;   // a tile is covered by 16/m consecutive warps
-                for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
+                uint32_t tc = 0;
+                if ((uint32_t)lane < mt)
+                    for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
+                if (lane < kMaxSpan) sh.tcs[s][lane] = tc;
+                __syncwarp();
+                if (lane == 0) mbar_arrive(cnt0 + 8 * s);
             }
+            store_piece(a, ts, m, mt, tid, ao);
             finish_pending();
-            PICI_TR(it, 6);
+            PICI_TR(j, 6);
             pending = true;
             pr = r;
             p_before = before + r.sk - r.k;
             p_total = surv_total;
-            p_tc = tc;
-            p_it = it;
+            p_j = j;
         } else {
             // ---- the span does not fit: tile by tile (one tile always fits), two sweeps -----------------
             // Sweep 1 counts the survivors of every tile so that the span's count is published before
             // anything waits (no other CTA ever waits on a half-processed span); sweep 2 emits.
-            __syncthreads();
             finish_pending();
-            prefetch_span();
             for (uint32_t i = 0; i < mt; ++i) {
-                const uint32_t x0 = __shfl_sync(kFull, ixl, i), x1 = __shfl_sync(kFull, ixl, i + 1);
-                const uint32_t y0 = __shfl_sync(kFull, iyl, i), y1 = __shfl_sync(kFull, iyl, i + 1);
-                tile_pass<false>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, bar, par, tid);
+                const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
+                const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
+                tile_pass<false>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, slow_bar, slow_par, tid);
                 if (tid == 0) {
                     uint32_t cnt = 0;
                     for (int q = 0; q < kMergeWarps; ++q) cnt += sh.ws[q];
-                    sh.tc[i] = cnt;
+                    sh.tcs[s][i] = cnt;
                 }
             }
-            __syncthreads();
-            uint32_t span_total = 0;
-            for (uint32_t i = 0; i < mt; ++i) span_total += sh.tc[i];
-            if (tid == 0) publish_span(a, g, it, c, span_total);
-            if (warp == 0) {
-                const uint32_t excl = iter_lookback(a, G, it, c, E, E_it, lane);
-                write_index(a, ts, mt, (uint32_t)lane < mt ? sh.tc[lane] : 0u, excl, lane);
-                if (lane == 0) sh.span_excl = excl;
+            walkers_sync();
+            if (tid == 0) {
+                uint32_t span_total = 0;
+                for (uint32_t i = 0; i < mt; ++i) span_total += sh.tcs[s][i];
+                publish_span(a, g, j, c, span_total);
+                mbar_arrive(cnt0 + 8 * s);
             }
-            __syncthreads();
-            uint32_t off = sh.span_excl;
+            mbar_wait(lbd0 + 8 * s, ph);
+            uint32_t off = sh.excl[s];
             for (uint32_t i = 0; i < mt; ++i) {
-                const uint32_t x0 = __shfl_sync(kFull, ixl, i), x1 = __shfl_sync(kFull, ixl, i + 1);
-                const uint32_t y0 = __shfl_sync(kFull, iyl, i), y1 = __shfl_sync(kFull, iyl, i + 1);
-                const WalkOut r = tile_pass<true>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, bar, par, tid);
+                const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
+                const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
+                const WalkOut r = tile_pass<true>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, slow_bar, slow_par, tid);
                 uint32_t before, surv_total;
                 survivor_sums(sh, warp, before, surv_total);
                 span_flush(a.Ao, out_s, r, off, surv_total, before + r.sk - r.k, tid);
                 off += surv_total;
             }
-            __syncthreads();
+            walkers_sync();
+            if (tid == 0) mbar_arrive(free0 + 8 * s);
         }
-
-        // ---- rotate the pipeline -------------------------------------------------------------------------
-        if (s) par1 = par; else par0 = par;
-        g = gn;
-        gn += G;
-        ixl = ixn;
-        iyl = iyn;
-        ixn = ix2;
-        iyn = iy2;
     }
-    __syncthreads();
     finish_pending();
 }
 
@@ -550,7 +601,7 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
         cudaError_t e = cudaFuncSetAttribute(reduce_ss_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         int v = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, reduce_ss_kernel, kMergeThreads, smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, reduce_ss_kernel, kMergeLaunchThreads, smem);
         if (e != cudaSuccess) return e;
         per_sm = v > 0 ? v : 1;
         configured = true;
@@ -583,7 +634,7 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
     int32_t gate_value = g.value;
     void *params[] = {&a, &gate_ptr, &gate_value};
     return cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(reduce_ss_kernel), dim3((unsigned)blocks),
-                                       dim3(kMergeThreads), params, smem, s);
+                                       dim3(kMergeLaunchThreads), params, smem, s);
 }
 
 }  // namespace pici
