@@ -75,15 +75,19 @@ struct SpanInfo {
 struct MergeShared {
     uint64_t full[2];         // mbarrier: the copies of the span in stage s have landed
     uint64_t stage_free[2];   // mbarrier: the walkers are done with stage s
-    uint64_t counts[2];       // mbarrier: tcs[s] is written and the span's count is published
+    uint64_t counts[2];       // mbarrier: out region s, tcs[s], tot[s] are written, the count is published
     uint64_t lb_done[2];      // mbarrier: excl[s] is written
+    uint64_t flushed[2];      // mbarrier: out region s has been written to Ao
     uint64_t slow_bar;        // mbarrier: copies of the slow path
     SpanInfo info[2];
     uint32_t excl[2];                 // survivors before the span (from the look-back)
+    uint32_t tot[2], cand[2];         // survivors / candidates of the span; cand == ~0u: the walkers flush it
     uint32_t tcs[2][kMaxSpan];        // per-tile survivors of the span
     uint32_t wxy[kMergeWarps];        // per-warp totals: popc(x piece) | popc(y piece) << 16
     uint32_t wu[kMergeWarps];         // per-warp totals: popc(x | y)
     uint32_t ws[kMergeWarps];         // per-warp totals: survivors
+    uint16_t run_at[2][kMergeThreads];   // per-thread runs of a span that had cancellations: first word,
+    uint16_t run_k[2][kMergeThreads];    // survivors
 };
 // Barrier of the 16 walker warps (the staging warp never joins it).
 __device__ __forceinline__ void walkers_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kMergeThreads) : "memory"); }
@@ -300,26 +304,26 @@ __device__ __forceinline__ void publish_span(const MergeArgs &a, uint32_t g, uin
     red_add_u64(a.grp_word + (size_t)it * a.ngrp + (c >> 5), kOneAdd + total);
     red_add_u64(a.iter_word + it, kOneAdd + total);
 }
-// Warp 0: survivors before span (it, c).  E = running sum of the complete iterations [0, E_it), carried
-// by the CTA from look-back to look-back (a CTA's `it` advances by one each time, so at most one
-// iteration word is read; the loop covers the general case).  All G spans of an iteration below `it`
-// exist, and so do all 32 spans of a group below c's.
+// One warp: survivors before span (it, c).  E = running sum of the complete iterations [0, E_it),
+// carried by the calling warp from look-back to look-back (a service warp sees every other iteration
+// of its CTA, so two iteration words are read; up to 32 in one go).  All G spans of an iteration below
+// `it` exist, and so do all 32 spans of a group below c's.
 __device__ __forceinline__ uint32_t iter_lookback(const MergeArgs &a, uint32_t G, uint32_t it, uint32_t c, uint32_t &E,
                                                   uint32_t &E_it, int lane) {
     const uint32_t nfull = c >> 5, rem = c & 31u;
     const uint64_t *gw = a.grp_word + (size_t)it * a.ngrp;
     const uint64_t *sw = a.span_word + (size_t)it * G + (size_t)nfull * 32;
-    while (E_it + 1 < it) {   // not taken in the round-robin schedule
+    while (E_it + 32 < it) {   // not taken in the round-robin schedule
         uint64_t v;
         do { v = ld_status(a.iter_word + E_it); } while ((uint32_t)(v >> 48) != G);
         E += (uint32_t)v;
         ++E_it;
     }
-    const bool need_iter = E_it < it;   // uniform
+    const uint32_t nit = it - E_it;   // <= 32 iteration words still to add
     uint64_t vi, vg, vs;
     unsigned ns = 8;
     for (;;) {
-        vi = (need_iter && lane == 0) ? ld_status(a.iter_word + E_it) : ((uint64_t)G << 48);
+        vi = (uint32_t)lane < nit ? ld_status(a.iter_word + E_it + lane) : ((uint64_t)G << 48);
         vg = (uint32_t)lane < nfull ? ld_status(gw + lane) : (32ull << 48);
         vs = (uint32_t)lane < rem ? ld_status(sw + lane) : (1ull << 32);
         const bool ok = (uint32_t)(vi >> 48) == G && (uint32_t)(vg >> 48) == 32u && (uint32_t)(vs >> 32) != 0u;
@@ -327,10 +331,8 @@ __device__ __forceinline__ uint32_t iter_lookback(const MergeArgs &a, uint32_t G
         __nanosleep(ns);
         if (ns < 128) ns += ns;
     }
-    if (need_iter) {
-        E += __shfl_sync(kFull, (uint32_t)vi, 0);
-        ++E_it;
-    }
+    E += warp_sum((uint32_t)vi);
+    E_it = it;
     return E + warp_sum((uint32_t)vg + (uint32_t)vs);
 }
 
@@ -340,6 +342,25 @@ __device__ __forceinline__ void write_index(const MergeArgs &a, uint32_t ts, uin
     if ((uint32_t)lane < mt) {
         a.Io[ts + lane] = excl + tincl - tc;
         if (ts + lane + 1 == a.T) a.Io[a.T] = excl + tincl;
+    }
+}
+
+// One warp writes a walked span's output region to Ao + off.  Packed (no cancellation): the region is
+// contiguous.  Otherwise the walkers left their runs (first word, survivors) in shared memory: lane l
+// moves the runs of threads 32q + l, q = 0..15, offsets from a running warp scan.
+__device__ __forceinline__ void warp_flush(uint32_t *__restrict__ Ao, const uint32_t *out, uint32_t off, uint32_t surv_total,
+                                           uint32_t cand_total, const uint16_t *run_at, const uint16_t *run_k, int lane) {
+    uint32_t *dst = Ao + off;
+    if (surv_total == cand_total) {
+        for (uint32_t i = lane; i < surv_total; i += 32) dst[i] = out[i];
+        return;
+    }
+    uint32_t base = 0;
+    for (int q = 0; q < kMergeWarps; ++q) {
+        const uint32_t k = run_k[32 * q + lane], at = run_at[32 * q + lane];
+        const uint32_t incl = warp_incl_scan(k, lane);
+        for (uint32_t i = 0; i < k; ++i) dst[base + incl - k + i] = out[at + i];
+        base += __shfl_sync(kFull, incl, 31);
     }
 }
 
@@ -384,7 +405,7 @@ __device__ __forceinline__ WalkOut tile_pass(const MergeArgs &a, uint32_t *stage
 }
 
 
-constexpr int kMergeLaunchThreads = kMergeThreads + 32;   // 16 walker warps + the staging / scan warp
+constexpr int kMergeLaunchThreads = kMergeThreads + 64;   // 16 walker warps + one service warp per stage
 
 __global__ void __launch_bounds__(kMergeLaunchThreads, kMergeMinBlocks)
 reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
@@ -415,7 +436,7 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     const uint32_t spans = (T + m - 1) / m;
     uint32_t *const out = pool + 2 * kStageWords;
     const uint32_t full0 = smem_u32(&sh.full[0]), free0 = smem_u32(&sh.stage_free[0]);
-    const uint32_t cnt0 = smem_u32(&sh.counts[0]), lbd0 = smem_u32(&sh.lb_done[0]);
+    const uint32_t cnt0 = smem_u32(&sh.counts[0]), lbd0 = smem_u32(&sh.lb_done[0]), fl0 = smem_u32(&sh.flushed[0]);
     const uint32_t slow_bar = smem_u32(&sh.slow_bar);
     if (tid == 0) {
 #pragma unroll
@@ -424,20 +445,26 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
             mbar_init(free0 + 8 * s, 1);
             mbar_init(cnt0 + 8 * s, 1);
             mbar_init(lbd0 + 8 * s, 1);
+            mbar_init(fl0 + 8 * s, 1);
         }
         mbar_init(slow_bar, 1);
     }
     __syncthreads();
-    // Spans are dealt round-robin: CTA c takes spans c, c + G, c + 2G, ...; j counts this CTA's spans.
-    // The launch is cooperative (all G CTAs are co-resident), so every span a look-back waits on
-    // belongs to a running CTA, and span j of a CTA only depends on spans <= j of the others.
+    // Spans are dealt round-robin: CTA c takes spans c, c + G, c + 2G, ...; j counts this CTA's spans,
+    // span j lives in stage / output region s = j & 1.  The launch is cooperative (all G CTAs are
+    // co-resident), so every span a look-back waits on belongs to a running CTA, and span j of a CTA
+    // only depends on spans <= j of the others.
     const uint32_t c = blockIdx.x;
 
-    if (warp == kMergeWarps) {
-        // =============================== staging / scan warp ===============================
-        // For this CTA's span j (stage s = j & 1): (A) once the walkers have left stage s, start the
-        // copies of span j + 2 into it; (B) once span j's count is published, take its prefix, write
-        // its index entries and hand the prefix to the walkers.  Whichever is ready first is served.
+    if (warp >= kMergeWarps) {
+        // ============================ service warp of stage s ============================
+        // For this CTA's spans j = s, s + 2, ...: start the copies of span j (stage s is free once the
+        // walkers have left span j - 2); once span j's count is published take its prefix, write its
+        // index entries, write its output region to Ao and release the region.  The walkers never wait
+        // for a look-back: they only need stage s filled and region s released two spans later.
+        const uint32_t s = (uint32_t)warp - kMergeWarps;
+        uint32_t *const stage = pool + s * kStageWords;
+        const uint32_t *const out_s = out + s * kOutWords;
         auto load_index = [&](uint32_t gg, uint32_t &ixl, uint32_t &iyl) {   // lanes 0..mt hold I[ts .. ts+mt]
             ixl = 0;
             iyl = 0;
@@ -447,13 +474,13 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
                 iyl = __ldg(a.Iy + ts + jj);
             }
         };
-        auto prepare = [&](uint32_t gg, uint32_t ixl, uint32_t iyl, uint32_t s) {
+        auto prepare = [&](uint32_t gg, uint32_t ixl, uint32_t iyl) {
             if (gg >= spans) return;
             const uint32_t ts = gg * m, mt = min(m, T - ts);
             const uint32_t xs = __shfl_sync(kFull, ixl, 0), xe = __shfl_sync(kFull, ixl, mt);
             const uint32_t ys = __shfl_sync(kFull, iyl, 0), ye = __shfl_sync(kFull, iyl, mt);
             const bool fits = span_fits(m, xe - xs, ye - ys, mt);
-            const SpanLayout L = span_stage(a, pool + s * kStageWords, full0 + 8 * s, ts, m, mt, xs, xe - xs, ys, ye - ys, false, lane);
+            const SpanLayout L = span_stage(a, stage, full0 + 8 * s, ts, m, mt, xs, xe - xs, ys, ye - ys, false, lane);
             if (lane == 0) {
                 sh.info[s].fits = fits ? 1u : 0u;
                 sh.info[s].Xb = L.Xb;
@@ -462,98 +489,82 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
                 sh.info[s].ys = ys;
             }
             __syncwarp();
-            if (fits) span_stage(a, pool + s * kStageWords, full0 + 8 * s, ts, m, mt, xs, xe - xs, ys, ye - ys, true, lane);
+            if (fits) span_stage(a, stage, full0 + 8 * s, ts, m, mt, xs, xe - xs, ys, ye - ys, true, lane);
             else if (lane == 0) mbar_arrive(full0 + 8 * s);   // nothing to copy: the walkers stage tile by tile
         };
-        uint32_t ixa, iya, ixb, iyb;
-        load_index(c, ixa, iya);
-        load_index(c + G, ixb, iyb);
-        prepare(c, ixa, iya, 0u);
-        prepare(c + G, ixb, iyb, 1u);
-        load_index(c + 2 * G, ixa, iya);   // entries of the next span to prepare, one span ahead
-        uint32_t E = 0, E_it = 0;          // survivors of the complete iterations [0, E_it)
-        for (uint32_t j = 0; c + j * G < spans; ++j) {
-            const uint32_t s = j & 1u, ph = (j >> 1) & 1u;
-            const uint32_t g = c + j * G, ts = g * m, mt = min(m, T - ts);
-            bool issued = false, looked = false;
-            while (!(issued && looked)) {
-                if (!issued && mbar_test(free0 + 8 * s, ph)) {
-                    prepare(g + 2 * G, ixa, iya, s);
-                    load_index(g + 3 * G, ixa, iya);
-                    issued = true;
-                }
-                if (!looked && mbar_test(cnt0 + 8 * s, ph)) {
-                    const uint32_t excl = iter_lookback(a, G, j, c, E, E_it, lane);
-                    write_index(a, ts, mt, (uint32_t)lane < mt ? sh.tcs[s][lane] : 0u, excl, lane);
-                    if (lane == 0) {
-                        sh.excl[s] = excl;
-                        mbar_arrive(lbd0 + 8 * s);
-                    }
-                    looked = true;
-                }
+        uint32_t ixa, iya;
+        load_index(c + s * G, ixa, iya);
+        prepare(c + s * G, ixa, iya);
+        load_index(c + (s + 2) * G, ixa, iya);   // entries of the next span to prepare, one ahead
+        uint32_t E = 0, E_it = 0;                // survivors of the complete iterations [0, E_it)
+        for (uint32_t j = s; c + j * G < spans; j += 2) {
+            const uint32_t ph = (j >> 1) & 1u;
+            const uint32_t ts = (c + j * G) * m, mt = min(m, T - ts);
+            mbar_wait(cnt0 + 8 * s, ph);
+            const uint32_t excl = iter_lookback(a, G, j, c, E, E_it, lane);
+            write_index(a, ts, mt, (uint32_t)lane < mt ? sh.tcs[s][lane] : 0u, excl, lane);
+            const uint32_t tot = sh.tot[s], cand = sh.cand[s];
+            if (lane == 0) {
+                sh.excl[s] = excl;
+                mbar_arrive(lbd0 + 8 * s);
             }
+            mbar_wait(free0 + 8 * s, ph);
+            prepare(c + (j + 2) * G, ixa, iya);
+            load_index(c + (j + 4) * G, ixa, iya);
+            if (cand != ~0u) warp_flush(a.Ao, out_s, excl, tot, cand, sh.run_at[s], sh.run_k[s], lane);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(fl0 + 8 * s);
         }
         return;
     }
 
     // ======================================= walker warps =======================================
-    // A walked span whose flush is deferred behind the next span's walk: its count is published at
-    // once, the staging warp takes its prefix meanwhile.
-    bool pending = false;
-    WalkOut pr = {0, 0, 0, 0};
-    uint32_t p_before = 0, p_total = 0, p_j = 0;
-    auto finish_pending = [&]() {
-        if (!pending) return;
-        const uint32_t ps = p_j & 1u;
-        mbar_wait(lbd0 + 8 * ps, (p_j >> 1) & 1u);
-        PICI_TR(p_j + 1u, 5);
-        span_flush(a.Ao, out + ps * kOutWords, pr, sh.excl[ps], p_total, p_before, tid);
-        pending = false;
-    };
     uint32_t slow_par = 0;
-
     for (uint32_t j = 0; c + j * G < spans; ++j) {
         const uint32_t s = j & 1u, ph = (j >> 1) & 1u;
         const uint32_t g = c + j * G, ts = g * m, mt = min(m, T - ts);
         uint32_t *const stage = pool + s * kStageWords;
         uint32_t *const out_s = out + s * kOutWords;
         PICI_TR(j, 0);
+        if (j >= 2) mbar_wait(fl0 + 8 * s, ph ^ 1u);   // span j - 2 has left output region s
         mbar_wait(full0 + 8 * s, ph);
         PICI_TR(j, 1);
         const SpanInfo info = sh.info[s];
 
         if (info.fits) {
-            // ---- walk now, publish the count, flush the PREVIOUS span, leave this one pending -----------
+            // ---- walk, publish the count; the service warp of stage s does the rest ---------------------
             uint32_t ao[4];
             const WalkOut r = walk_span<true>(stage, out_s, sh, m * kTileWords, info.Xb, info.Yb, m, mt, ao, tid, j);
             uint32_t before, surv_total;
             survivor_sums(sh, warp, before, surv_total);
+            const bool cancelled = surv_total != r.cand_total;   // uniform
+            if (cancelled) {   // the region is not contiguous: leave the runs for the flush
+                sh.run_at[s][tid] = (uint16_t)r.ko0;
+                sh.run_k[s][tid] = (uint16_t)r.k;
+                walkers_sync();
+            }
             if (warp == 0) {
-                if (lane == 0) {
-                    mbar_arrive(free0 + 8 * s);               // every walker is past barrier #2
-                    publish_span(a, g, j, c, surv_total);
-                }
                 const uint32_t wpt = (uint32_t)kMergeWarps / m;   // a tile is covered by 16/m consecutive warps
                 uint32_t tc = 0;
                 if ((uint32_t)lane < mt)
                     for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
                 if (lane < kMaxSpan) sh.tcs[s][lane] = tc;
+                if (lane == 0) {
+                    sh.tot[s] = surv_total;
+                    sh.cand[s] = r.cand_total;
+                    publish_span(a, g, j, c, surv_total);
+                    mbar_arrive(free0 + 8 * s);           // every walker is past barrier #2
+                }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(cnt0 + 8 * s);
             }
             store_piece(a, ts, m, mt, tid, ao);
-            finish_pending();
             PICI_TR(j, 6);
-            pending = true;
-            pr = r;
-            p_before = before + r.sk - r.k;
-            p_total = surv_total;
-            p_j = j;
         } else {
             // ---- the span does not fit: tile by tile (one tile always fits), two sweeps -----------------
             // Sweep 1 counts the survivors of every tile so that the span's count is published before
-            // anything waits (no other CTA ever waits on a half-processed span); sweep 2 emits.
-            finish_pending();
+            // anything waits (no other CTA ever waits on a half-processed span); sweep 2 emits and the
+            // walkers write Ao themselves (cand = ~0 tells the service warp not to).
             for (uint32_t i = 0; i < mt; ++i) {
                 const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
                 const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
@@ -568,6 +579,8 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
             if (tid == 0) {
                 uint32_t span_total = 0;
                 for (uint32_t i = 0; i < mt; ++i) span_total += sh.tcs[s][i];
+                sh.tot[s] = span_total;
+                sh.cand[s] = ~0u;
                 publish_span(a, g, j, c, span_total);
                 mbar_arrive(cnt0 + 8 * s);
             }
@@ -586,7 +599,6 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
             if (tid == 0) mbar_arrive(free0 + 8 * s);
         }
     }
-    finish_pending();
 }
 
 cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void *Ax, const uint64_t *By,
