@@ -61,12 +61,17 @@ def measured_peak() -> tuple[float, str]:
 
 
 def ncu_traffic() -> dict:
-    """Per-launch DRAM bytes of each kernel from the committed ncu --set full capture (text)."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of each op from the committed
+    ncu --set full capture: profiles/traffic.csv, lines `op,read_bytes,write_bytes` (see profiles/*.md)."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    out = {}
     if os.path.exists(p):
         with open(p) as f:
-            return json.load(f)
-    return {}
+            for line in f:
+                parts = line.strip().split(",")
+                if len(parts) == 3 and parts[1].replace(".", "").isdigit():
+                    out[parts[0]] = int(float(parts[1]) + float(parts[2]))
+    return out
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -204,7 +209,7 @@ class HotPath:
         self.dense = torch.empty(n, dtype=torch.float32, device=device)
         self.cnt = torch.zeros(1, dtype=torch.int32, device=device)
         self.flag = torch.zeros(1, dtype=torch.int32, device=device)
-        self.launches_per_step = 6
+        self.launches_per_step = 7      # compress x2, reduce_ss, nnz, expand (densify), scatter_add_sparse + expand (reduce_sd)
 
     OPS = ("compress", "compress", "reduce_ss", "nnz", "maybe_densify", "reduce_sd")
 
