@@ -255,13 +255,14 @@ def time_op(fn, iters: int, warm: int = 2):
     return ts[len(ts) // 2], ts[0]
 
 
-def run_sweep(pk, n: int, peak: float, iters: int, device) -> list[dict]:
+def run_sweep(pk, n: int, peak: float, iters: int, device, dtypes=("f32", "bf16"), sparsities=None,
+              ops=("compress", "decompress", "reduce_ss", "reduce_sd")) -> list[dict]:
     """Every kernel alone at every sparsity of configs[1] (seed 0; fp32: all ops, bf16: compress/decompress)."""
     rows = []
-    for dtype in ("f32", "bf16"):
+    for dtype in dtypes:
         s = 4 if dtype == "f32" else 2
         D = pk.F32 if dtype == "f32" else pk.BF16
-        for sp in wl.CONFIG2_SPARSITIES:
+        for sp in (sparsities or wl.CONFIG2_SPARSITIES):
             d = 1.0 - sp
             x = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 0), dtype=dtype, device=device)
             px = pk.alloc_pici(n, D, device)
@@ -273,23 +274,28 @@ def run_sweep(pk, n: int, peak: float, iters: int, device) -> list[dict]:
                              "dense_equiv_gbs": round(n * s / ms / 1e6, 1), "bytes_moved_gbs": round(nbytes / ms / 1e6, 1),
                              "frac": round(nbytes / ms / 1e6 / peak, 3)})
 
-            ms, mn = time_op(lambda: pk.compress(x, px, ws), iters)
+            pk.compress(x, px, ws)
             nx = px.nnz_host()
-            row("compress", ms, mn, bytes_compress(n, s, nx))
-            ms, mn = time_op(lambda: pk.decompress(px, out), iters)
-            row("decompress", ms, mn, bytes_decompress(n, s, nx))
-            if dtype == "f32":
+            if "compress" in ops:
+                ms, mn = time_op(lambda: pk.compress(x, px, ws), iters)
+                row("compress", ms, mn, bytes_compress(n, s, nx))
+            if "decompress" in ops:
+                ms, mn = time_op(lambda: pk.decompress(px, out), iters)
+                row("decompress", ms, mn, bytes_decompress(n, s, nx))
+            if dtype == "f32" and ("reduce_ss" in ops or "reduce_sd" in ops):
                 y = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 1), dtype=dtype, device=device)
                 py, po = pk.alloc_pici(n, D, device), pk.alloc_pici(n, D, device)
                 pk.compress(y, py, ws)
                 pk.reduce_ss(px, py, po, ws)
                 ny, no = py.nnz_host(), po.nnz_host()
-                ms, mn = time_op(lambda: pk.reduce_ss(px, py, po, ws), iters)
-                row("reduce_ss", ms, mn, bytes_reduce_ss(n, nx, ny, no))
-                sect = touched_sectors_f32(x)
-                ms, mn = time_op(lambda: pk.reduce_sd(px, y), iters)      # in place into a 2^28 dense buffer
-                row("reduce_sd", ms, mn, bytes_reduce_sd(n, nx, sect))
-                rows[-1]["touched_sector_frac"] = round(sect / (n / 8), 4)
+                if "reduce_ss" in ops:
+                    ms, mn = time_op(lambda: pk.reduce_ss(px, py, po, ws), iters)
+                    row("reduce_ss", ms, mn, bytes_reduce_ss(n, nx, ny, no))
+                if "reduce_sd" in ops:
+                    sect = touched_sectors_f32(x)
+                    ms, mn = time_op(lambda: pk.reduce_sd(px, y), iters)      # in place into a 2^28 dense buffer
+                    row("reduce_sd", ms, mn, bytes_reduce_sd(n, nx, sect))
+                    rows[-1]["touched_sector_frac"] = round(sect / (n / 8), 4)
                 del y, py, po
             del x, px, out, ws
             torch.cuda.empty_cache()
@@ -363,6 +369,11 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--sweep-iters", type=int, default=7)
+    ap.add_argument("--sweep-only", action="store_true",
+                    help="time single kernels only (one JSON line per row); filters: --ops --dtypes --sparsities")
+    ap.add_argument("--ops", default="compress,decompress,reduce_ss,reduce_sd")
+    ap.add_argument("--dtypes", default="f32,bf16")
+    ap.add_argument("--sparsities", default="")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -383,6 +394,11 @@ def main():
     n = 1 << args.log2n
     density = 1.0 - args.sparsity
     peak, peak_src = measured_peak()
+    if args.sweep_only:   # kernel-by-kernel timing (also the program the single-kernel ncu captures run)
+        sp = tuple(float(v) for v in args.sparsities.split(",")) if args.sparsities else None
+        for r in run_sweep(pk, n, peak, args.sweep_iters, device, tuple(args.dtypes.split(",")), sp, tuple(args.ops.split(","))):
+            print(json.dumps(r), flush=True)
+        return
     from paper_2607_04676_b200 import replicas
     seed_x, seed_y = replicas.rank_seeds(0, rank, 2)
     hp = HotPath(pk, n, density, seed_x, seed_y, device)
