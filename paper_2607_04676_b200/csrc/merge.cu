@@ -64,7 +64,7 @@ constexpr uint32_t kStageWords = 2 * kTileWords + 2 * kTile + 16;
 constexpr uint32_t kOutWords = kTile;                   // candidates (bits of x | y) of a span
 constexpr uint32_t kPoolWords = 2 * kStageWords + 2 * kOutWords;   // two stages, two output regions
 constexpr int kMergeMinBlocks = 2;
-constexpr uint32_t kMaxGrid = 1024;                     // groups of 32 spans per iteration fit one warp
+constexpr uint32_t kMaxGrid = kRoundRobinMaxUnits;       // units per iteration the round-robin scan supports
 
 // What the staging warp tells the walkers about the span in a stage.
 struct SpanInfo {
@@ -109,10 +109,8 @@ struct MergeArgs {
     const uint32_t *Ix, *Iy, *Ax, *Ay;
     uint64_t *Bo;
     uint32_t *Io, *Ao;
-    uint64_t *span_word;   // [spans]          (1 << 32) | survivors once published
-    uint64_t *grp_word;    // [iterations][ngrp] (adds << 48) + sum
-    uint64_t *iter_word;   // [iterations]       (adds << 48) + sum
-    uint32_t T, ngrp;
+    RoundRobinScan scan;   // per-span / per-group / per-iteration words (pici_common.cuh)
+    uint32_t T;
     uint64_t a_limit;      // bytes of Ax / Ay that may be read: (n * 4) & ~15 (capacity >= n elements)
 };
 
@@ -292,48 +290,13 @@ __device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *ou
     return r;
 }
 
-// ---- Phase 2: counts -> exclusive prefix ------------------------------------------------------------
-constexpr uint64_t kOneAdd = 1ull << 48;
-__device__ __forceinline__ void red_add_u64(uint64_t *p, uint64_t v) {
-    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-// One thread: make span (it, c)'s survivor count visible in its three words.  Every word is
-// self-contained (count and sum travel in one 64-bit access), so relaxed gpu-scope accesses suffice.
+// ---- Phase 2: counts -> exclusive prefix: the round-robin scan of pici_common.cuh ----------------------
 __device__ __forceinline__ void publish_span(const MergeArgs &a, uint32_t g, uint32_t it, uint32_t c, uint32_t total) {
-    st_status(a.span_word + g, 1u, total);
-    red_add_u64(a.grp_word + (size_t)it * a.ngrp + (c >> 5), kOneAdd + total);
-    red_add_u64(a.iter_word + it, kOneAdd + total);
+    rr_publish(a.scan, g, it, c, total);
 }
-// One warp: survivors before span (it, c).  E = running sum of the complete iterations [0, E_it),
-// carried by the calling warp from look-back to look-back (a service warp sees every other iteration
-// of its CTA, so two iteration words are read; up to 32 in one go).  All G spans of an iteration below
-// `it` exist, and so do all 32 spans of a group below c's.
 __device__ __forceinline__ uint32_t iter_lookback(const MergeArgs &a, uint32_t G, uint32_t it, uint32_t c, uint32_t &E,
                                                   uint32_t &E_it, int lane) {
-    const uint32_t nfull = c >> 5, rem = c & 31u;
-    const uint64_t *gw = a.grp_word + (size_t)it * a.ngrp;
-    const uint64_t *sw = a.span_word + (size_t)it * G + (size_t)nfull * 32;
-    while (E_it + 32 < it) {   // not taken in the round-robin schedule
-        uint64_t v;
-        do { v = ld_status(a.iter_word + E_it); } while ((uint32_t)(v >> 48) != G);
-        E += (uint32_t)v;
-        ++E_it;
-    }
-    const uint32_t nit = it - E_it;   // <= 32 iteration words still to add
-    uint64_t vi, vg, vs;
-    unsigned ns = 8;
-    for (;;) {
-        vi = (uint32_t)lane < nit ? ld_status(a.iter_word + E_it + lane) : ((uint64_t)G << 48);
-        vg = (uint32_t)lane < nfull ? ld_status(gw + lane) : (32ull << 48);
-        vs = (uint32_t)lane < rem ? ld_status(sw + lane) : (1ull << 32);
-        const bool ok = (uint32_t)(vi >> 48) == G && (uint32_t)(vg >> 48) == 32u && (uint32_t)(vs >> 32) != 0u;
-        if (__all_sync(kFull, ok)) break;
-        __nanosleep(ns);
-        if (ns < 128) ns += ns;
-    }
-    E += warp_sum((uint32_t)vi);
-    E_it = it;
-    return E + warp_sum((uint32_t)vg + (uint32_t)vs);
+    return rr_lookback(a.scan, G, it, c, E, E_it, lane);
 }
 
 // Io for the mt tiles of a span (one warp; lane i < mt holds tc = survivors of tile ts + i).
@@ -633,8 +596,9 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
     a.Bx = Bx; a.By = By; a.Ix = Ix; a.Iy = Iy;
     a.Ax = reinterpret_cast<const uint32_t *>(Ax); a.Ay = reinterpret_cast<const uint32_t *>(Ay);
     a.Bo = Bo; a.Io = Io; a.Ao = reinterpret_cast<uint32_t *>(Ao);
-    a.span_word = base; a.iter_word = base + T; a.grp_word = base + T + iters;
-    a.T = (uint32_t)T; a.ngrp = (uint32_t)ngrp;
+    a.scan.unit_word = base; a.scan.iter_word = base + T; a.scan.grp_word = base + T + iters;
+    a.scan.ngrp = (uint32_t)ngrp;
+    a.T = (uint32_t)T;
     a.a_limit = (n * 4) & ~15ull;
 #ifdef PICI_MERGE_TRACE
     {

@@ -145,6 +145,66 @@ __device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t t
     return excl;
 }
 
+// ---- round-robin scan: exclusive prefix of per-unit counts in ONE L2 round trip --------------------
+// For persistent grids launched cooperatively (every worker resident) whose W workers take units
+// round-robin: worker c handles units c, c + W, c + 2W, ...; "iteration" it covers units
+// [it*W, (it+1)*W).  A worker publishes its unit's count as (a) a per-unit word (1 << 32 | count),
+// (b) a 64-bit atomic add of (1 << 48) + count into the word of its group of 32 units and (c) into the
+// word of its iteration; each word carries (number of adds, sum) in one 64-bit access, so relaxed
+// gpu-scope accesses suffice.  prefix(it, c) = complete iterations below it + complete groups below
+// c's + the units of c's own group below c: independent loads, 32 + 64 + 32 words at most.  The workers
+// run nearly in lock-step, so a flat decoupled look-back would find no prefix among the W - 1 units
+// of its own iteration and walk W / 32 dependent hops (measured in reduce_ss: ~8 us per iteration).
+constexpr uint32_t kRoundRobinMaxUnits = 2048;   // W <= 2048: two group words per lane
+struct RoundRobinScan {
+    uint64_t *unit_word;   // [units]
+    uint64_t *grp_word;    // [iterations][ngrp], ngrp = ceil(W / 32)
+    uint64_t *iter_word;   // [iterations]
+    uint32_t ngrp;
+};
+constexpr uint64_t kOneAdd = 1ull << 48;
+__device__ __forceinline__ void red_add_u64(uint64_t *p, uint64_t v) {
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// One thread: publish the count of unit u = it * W + c.
+__device__ __forceinline__ void rr_publish(const RoundRobinScan &sc, uint64_t u, uint32_t it, uint32_t c, uint32_t count) {
+    st_status(sc.unit_word + u, 1u, count);
+    red_add_u64(sc.grp_word + (size_t)it * sc.ngrp + (c >> 5), kOneAdd + count);
+    red_add_u64(sc.iter_word + it, kOneAdd + count);
+}
+// One warp: sum of the counts of all units below (it, c).  E = running sum of the complete iterations
+// [0, E_it), carried by the caller from call to call (up to 32 iteration words are added per call).
+// All W units of an iteration below `it` exist, and so do all 32 units of a group below c's.
+__device__ __forceinline__ uint32_t rr_lookback(const RoundRobinScan &sc, uint32_t W, uint32_t it, uint32_t c, uint32_t &E,
+                                                uint32_t &E_it, int lane) {
+    const uint32_t nfull = c >> 5, rem = c & 31u;
+    const uint64_t *gw = sc.grp_word + (size_t)it * sc.ngrp;
+    const uint64_t *uw = sc.unit_word + (size_t)it * W + (size_t)nfull * 32;
+    while (E_it + 32 < it) {   // not taken when a worker sees consecutive iterations
+        uint64_t v;
+        do { v = ld_status(sc.iter_word + E_it); } while ((uint32_t)(v >> 48) != W);
+        E += (uint32_t)v;
+        ++E_it;
+    }
+    const uint32_t nit = it - E_it;
+    uint64_t vi, vg, vh, vs;
+    unsigned ns = 8;
+    for (;;) {
+        vi = (uint32_t)lane < nit ? ld_status(sc.iter_word + E_it + lane) : ((uint64_t)W << 48);
+        vg = (uint32_t)lane < nfull ? ld_status(gw + lane) : (32ull << 48);
+        vh = (uint32_t)lane + 32u < nfull ? ld_status(gw + 32 + lane) : (32ull << 48);
+        vs = (uint32_t)lane < rem ? ld_status(uw + lane) : (1ull << 32);
+        const bool ok = (uint32_t)(vi >> 48) == W && (uint32_t)(vg >> 48) == 32u && (uint32_t)(vh >> 48) == 32u &&
+                        (uint32_t)(vs >> 32) != 0u;
+        if (__all_sync(kFull, ok)) break;
+        __nanosleep(ns);
+        if (ns < 128) ns += ns;
+    }
+    E += warp_sum((uint32_t)vi);
+    E_it = it;
+    return E + warp_sum((uint32_t)vg + (uint32_t)vh + (uint32_t)vs);
+}
+
 // ---- TMA 1-D bulk copy global -> shared, completion on an mbarrier (UBLKCP in SASS) -------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
