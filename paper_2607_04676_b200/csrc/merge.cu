@@ -463,7 +463,17 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
         for (uint32_t j = s; c + j * G < spans; j += 2) {
             const uint32_t ph = (j >> 1) & 1u;
             const uint32_t ts = (c + j * G) * m, mt = min(m, T - ts);
-            mbar_wait(cnt0 + 8 * s, ph);
+            // Copies first when the stage is already free (they are what the walkers wait for two spans
+            // later); a span on the slow path frees its stage only after its look-back, so poll both.
+            bool prepared = false;
+            for (;;) {
+                if (!prepared && mbar_test(free0 + 8 * s, ph)) {
+                    prepare(c + (j + 2) * G, ixa, iya);
+                    load_index(c + (j + 4) * G, ixa, iya);
+                    prepared = true;
+                }
+                if (mbar_test(cnt0 + 8 * s, ph)) break;
+            }
             const uint32_t excl = iter_lookback(a, G, j, c, E, E_it, lane);
             write_index(a, ts, mt, (uint32_t)lane < mt ? sh.tcs[s][lane] : 0u, excl, lane);
             const uint32_t tot = sh.tot[s], cand = sh.cand[s];
@@ -471,9 +481,11 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
                 sh.excl[s] = excl;
                 mbar_arrive(lbd0 + 8 * s);
             }
-            mbar_wait(free0 + 8 * s, ph);
-            prepare(c + (j + 2) * G, ixa, iya);
-            load_index(c + (j + 4) * G, ixa, iya);
+            if (!prepared) {
+                mbar_wait(free0 + 8 * s, ph);
+                prepare(c + (j + 2) * G, ixa, iya);
+                load_index(c + (j + 4) * G, ixa, iya);
+            }
             if (cand != ~0u) warp_flush(a.Ao, out_s, excl, tot, cand, sh.run_at[s], sh.run_k[s], lane);
             __syncwarp();
             if (lane == 0) mbar_arrive(fl0 + 8 * s);
