@@ -1,0 +1,94 @@
+"""CPU-side checks of the C-ABI boundary (no GPU, no compute): libpici_b200.so builds for sm_100a and loads,
+exports every function include/pici.h declares, reports the sizes the format fixes, and
+rejects bad arguments with error codes before any CUDA call is made (include/pici.h "Errors").
+"""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2607_04676_b200 import pici
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared() -> list[str]:
+    """Function names declared between the extern "C" braces of include/pici.h."""
+    src = open(os.path.join(ROOT, "include", "pici.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(pici_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported_and_bound():
+    names = _declared()
+    assert {"pici_compress", "pici_decompress", "pici_reduce_ss", "pici_reduce_sd", "pici_nnz",
+            "pici_maybe_densify"} <= set(names)              # the six names north_star fixes
+    lib = pici.lib()
+    for n in names:
+        assert hasattr(lib, n), f"{n} is declared in include/pici.h but not exported"
+    assert set(names) == set(pici.EXPORTS), "the Python binding and the header disagree on the entry points"
+    assert lib.pici_version() == 100
+
+
+def test_oracle_and_product_share_no_code():
+    """Neither side imports, includes or links the other (the oracle is test infrastructure)."""
+    pkg = os.path.join(ROOT, "paper_2607_04676_b200")
+    for d, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(d, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+\S*oracle", text, flags=re.M), f"{f} imports the oracle"
+                assert not re.search(r"#\s*include\s*[<\"].*oracle", text), f"{f} includes the oracle"
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(from|import)\s+paper_2607_04676_b200", text, flags=re.M), f
+            assert not re.search(r"#\s*include\s*[<\"].*(csrc|pici\.h|pici_common)", text), f
+
+
+@pytest.mark.parametrize("n", [0, 1, 4095, 4096, 4097, 8192, 1 << 20, (1 << 28), (1 << 32) - 1])
+@pytest.mark.parametrize("dtype", [pici.F32, pici.BF16])
+def test_sizes_follow_the_format(n, dtype):
+    lib = pici.lib()
+    bw, ie, cap, ws = (ctypes.c_uint64() for _ in range(4))
+    assert lib.pici_sizes(n, dtype, ctypes.byref(bw), ctypes.byref(ie), ctypes.byref(cap), ctypes.byref(ws)) == 0
+    T = (n + 4095) // 4096
+    assert bw.value == 64 * T            # one 64-bit word per column of every 64x64 tile
+    assert ie.value == T + 1             # exclusive prefix per tile + total nnz
+    assert cap.value == n                # worst case: every element stored
+    assert ws.value >= 8 * T and ws.value % 16 == 0
+    if n and n % 4096 == 0:              # metadata / fp32 dense = (1/8 + 4/4096) / 4 + 4 bytes
+        assert 8 * bw.value + 4 * ie.value == n // 8 + n // 1024 + 4
+    assert lib.pici_sizes(n, dtype, None, None, None, None) == 0          # every output is optional
+
+
+def test_sizes_and_calls_reject_bad_arguments_without_touching_the_device():
+    lib = pici.lib()
+    INVALID, DTYPE, ALIGN, CAPACITY, WORKSPACE = -1, -2, -3, -4, -5
+    assert lib.pici_sizes(1 << 32, pici.F32, None, None, None, None) == INVALID      # n < 2^32 (32-bit I)
+    assert lib.pici_sizes(16, 7, None, None, None, None) == DTYPE
+    a = 0x1000                                                                      # a fake, 16-aligned "pointer"
+    n = 8192
+    ws = ctypes.c_uint64()
+    lib.pici_sizes(n, pici.F32, None, None, None, ctypes.byref(ws))
+    C = lib.pici_compress
+    assert C(a, n, 9, a, a, a, n, a, ws.value, None) == DTYPE
+    assert C(a, 1 << 32, pici.F32, a, a, a, 1 << 32, a, ws.value, None) == INVALID
+    assert C(None, n, pici.F32, a, a, a, n, a, ws.value, None) == INVALID
+    assert C(a, n, pici.F32, a, None, a, n, a, ws.value, None) == INVALID
+    assert C(a + 4, n, pici.F32, a, a, a, n, a, ws.value, None) == ALIGN
+    assert C(a, n, pici.F32, a + 8, a, a, n, a, ws.value, None) == ALIGN
+    assert C(a, n, pici.F32, a, a + 2, a, n, a, ws.value, None) == ALIGN
+    assert C(a, n, pici.F32, a, a, a, n - 1, a, ws.value, None) == CAPACITY
+    assert C(a, n, pici.F32, a, a, a, n, a, ws.value - 1, None) == WORKSPACE
+    assert C(a, n, pici.F32, a, a, a, n, None, ws.value, None) == WORKSPACE
+    S = lib.pici_reduce_ss
+    assert S(a, a, a, a, a, a, n, pici.BF16, a, a, a, n, a, ws.value, None) == DTYPE       # reductions are fp32 only
+    assert S(a, a, a, a, a, a, n, pici.F32, a, a, a, n - 1, a, ws.value, None) == CAPACITY
+    assert S(a, a, a, a, None, a, n, pici.F32, a, a, a, n, a, ws.value, None) == INVALID
+    assert lib.pici_reduce_sd(a, a, a, n, pici.BF16, a, None) == DTYPE
+    assert lib.pici_decompress(a, a, a, n, pici.F32, None, None) == INVALID
+    assert lib.pici_decompress(a, a, a, n, pici.F32, a + 4, None) == ALIGN
+    for code in (0, INVALID, DTYPE, ALIGN, CAPACITY, WORKSPACE, -6, -99):
+        assert lib.pici_strerror(code)                                               # always a string, never NULL
