@@ -131,7 +131,8 @@ def test_reduce_sd_mixed_tiles(pk, lo, hi, every):
     assert np.array_equal(_bits(got), want.view(np.uint32))
 
 
-@pytest.mark.parametrize("lo,hi,every", ((0.002, 1.0, 16), (0.0, 0.5, 5), (0.7, 0.0, 2), (0.01, 0.9, 9)))
+@pytest.mark.parametrize("lo,hi,every", ((0.002, 1.0, 16), (0.0, 0.5, 5), (0.7, 0.0, 2), (0.01, 0.9, 9),
+                                         (0.001, 1.0, 64), (0.02, 0.2, 40), (0.0, 0.07, 3)))
 def test_reduce_ss_mixed_tiles(pk, lo, hi, every):
     n = 133 * wl.TILE + 77
     x = _clustered(n, lo, hi, every, seed=81)
