@@ -147,7 +147,8 @@ struct SpanLayout {
     uint32_t tx;       // bytes the bulk copies signal on the mbarrier
 };
 __device__ __forceinline__ bool span_fits(uint32_t m, uint32_t nx, uint32_t ny, uint32_t mt) {
-    return 2u * m * kTileWords + nx + ny + 16u <= kStageWords && min(nx + ny, (uint32_t)kTile * mt) <= kOutWords;
+    (void)mt;   // the output region is checked on the exact candidate count, after the popc scan (walk_span)
+    return 2u * m * kTileWords + nx + ny + 16u <= kStageWords;
 }
 
 // Warp 0: start the copies of the span of mt tiles at tile ts (m tiles per span) into `stage`; returns
@@ -256,6 +257,10 @@ __device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *ou
             bu += u;
         }
         cand_total += u;
+    }
+    if (EMIT && cand_total > kOutWords) {   // uniform: more candidates than the output region holds
+        WalkOut none = {0u, 0u, 0u, cand_total};
+        return none;                        // the caller takes the tile-by-tile path (only one barrier passed)
     }
     uint32_t kx = Xb + (bxy & 0xFFFFu) + (sxy & 0xFFFFu) - cx;
     uint32_t ky = Yb + (bxy >> 16) + (sxy >> 16) - cy;
@@ -387,11 +392,15 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     // spans per CTA (ring chunks are a few thousand tiles).
     uint32_t m = 1;
     {
-        const uint64_t tot = (uint64_t)__ldg(a.Ix + T) + (uint64_t)__ldg(a.Iy + T);
-        const uint64_t avg = (tot + T - 1) / T;   // values per tile, X and Y together
+        const uint64_t nx = __ldg(a.Ix + T), ny = __ldg(a.Iy + T);
+        const uint64_t avg = (nx + ny + T - 1) / T;   // values per tile, X and Y together
+        // candidates per tile: the union of two INDEPENDENT supports of these densities (a span whose
+        // union is larger than the output region takes the slow path, so this is an estimate, not a bound)
+        const uint64_t both = (nx / T) * (ny / T) / kTile;
+        const uint64_t uni = min(avg - min(both, avg), (uint64_t)kTile);
 #pragma unroll
         for (uint32_t mm = kMaxSpan; mm >= 2; mm /= 2) {
-            const uint64_t vals = avg * mm + 16, cand = min(avg, (uint64_t)kTile) * mm;
+            const uint64_t vals = avg * mm + 16, cand = uni * mm;
             if (m == 1 && 2u * mm * kTileWords + vals + vals / 16 <= kStageWords && cand + cand / 16 <= kOutWords) m = mm;
         }
         while (m > 1 && (T + m - 1) / m < 2u * G) m /= 2;
@@ -506,36 +515,41 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
         PICI_TR(j, 1);
         const SpanInfo info = sh.info[s];
 
-        if (info.fits) {
+        bool slow = info.fits == 0u;
+        if (!slow) {
             // ---- walk, publish the count; the service warp of stage s does the rest ---------------------
             uint32_t ao[4];
             const WalkOut r = walk_span<true>(stage, out_s, sh, m * kTileWords, info.Xb, info.Yb, m, mt, ao, tid, j);
-            uint32_t before, surv_total;
-            survivor_sums(sh, warp, before, surv_total);
-            const bool cancelled = surv_total != r.cand_total;   // uniform
-            if (cancelled) {   // the region is not contiguous: leave the runs for the flush
-                sh.run_at[s][tid] = (uint16_t)r.ko0;
-                sh.run_k[s][tid] = (uint16_t)r.k;
-                walkers_sync();
-            }
-            if (warp == 0) {
-                const uint32_t wpt = (uint32_t)kMergeWarps / m;   // a tile is covered by 16/m consecutive warps
-                uint32_t tc = 0;
-                if ((uint32_t)lane < mt)
-                    for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
-                if (lane < kMaxSpan) sh.tcs[s][lane] = tc;
-                if (lane == 0) {
-                    sh.tot[s] = surv_total;
-                    sh.cand[s] = r.cand_total;
-                    publish_span(a, g, j, c, surv_total);
-                    mbar_arrive(free0 + 8 * s);           // every walker is past barrier #2
+            slow = r.cand_total > kOutWords;   // uniform; nothing was written
+            if (!slow) {
+                uint32_t before, surv_total;
+                survivor_sums(sh, warp, before, surv_total);
+                const bool cancelled = surv_total != r.cand_total;   // uniform
+                if (cancelled) {   // the region is not contiguous: leave the runs for the flush
+                    sh.run_at[s][tid] = (uint16_t)r.ko0;
+                    sh.run_k[s][tid] = (uint16_t)r.k;
+                    walkers_sync();
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(cnt0 + 8 * s);
+                if (warp == 0) {
+                    const uint32_t wpt = (uint32_t)kMergeWarps / m;   // a tile is covered by 16/m consecutive warps
+                    uint32_t tc = 0;
+                    if ((uint32_t)lane < mt)
+                        for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
+                    if (lane < kMaxSpan) sh.tcs[s][lane] = tc;
+                    if (lane == 0) {
+                        sh.tot[s] = surv_total;
+                        sh.cand[s] = r.cand_total;
+                        publish_span(a, g, j, c, surv_total);
+                        mbar_arrive(free0 + 8 * s);           // every walker is past barrier #2
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(cnt0 + 8 * s);
+                }
+                store_piece(a, ts, m, mt, tid, ao);
+                PICI_TR(j, 6);
             }
-            store_piece(a, ts, m, mt, tid, ao);
-            PICI_TR(j, 6);
-        } else {
+        }
+        if (slow) {
             // ---- the span does not fit: tile by tile (one tile always fits), two sweeps -----------------
             // Sweep 1 counts the survivors of every tile so that the span's count is published before
             // anything waits (no other CTA ever waits on a half-processed span); sweep 2 emits and the

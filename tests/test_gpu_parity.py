@@ -162,6 +162,26 @@ def test_reduce_ss_matches_oracle(pk, n, dx, dy):
     _assert_pici_equal(pk, out, want)
 
 
+@pytest.mark.parametrize("d", (0.26, 0.13, 0.06))
+def test_reduce_ss_disjoint_supports(pk, d):
+    """Disjoint supports: the union is larger than two independent supports of the same densities would
+    give, so a span length chosen from that estimate overflows the output region and the kernel has to fall
+    back to the tile-by-tile path on the exact candidate count."""
+    n = 300 * wl.TILE + 5
+    g = torch.Generator().manual_seed(91)
+    u = torch.rand(n, generator=g)
+    vx, vy = wl.values(n, 92), wl.values(n, 93)
+    x = wl.apply_mask(u < d, vx)
+    y = wl.apply_mask((u >= d) & (u < 2 * d), vy)
+    xo, yo = po.compress(_bits(x), "f32"), po.compress(_bits(y), "f32")
+    want = po.reduce_ss(xo, yo)
+    assert want.nnz == xo.nnz + yo.nnz
+    out = pk.alloc_pici(n, pk.F32)
+    out.B.fill_(-1); out.I.fill_(-1)
+    pk.reduce_ss(_upload(pk, xo), _upload(pk, yo), out, pk.alloc_workspace(n))
+    _assert_pici_equal(pk, out, want)
+
+
 def test_reduce_ss_special_values(pk):
     n = 4096 + 50
     sp = wl.special_values_f32()
