@@ -355,6 +355,52 @@ def run_cpu_baseline(n: int, density: float) -> dict:
             "host_cores_available": os.cpu_count()}
 
 
+def run_ring(pk, name: str, iters: int, device) -> None:
+    """Ring collectives of configs[2..4] on P logical ranks in one HBM: local-compute time of
+    the whole collective (CUDA events around the driver's enqueues, pointer hand-offs cost nothing) and the step
+    at which each chunk switched to dense.  One JSON line per (collective, strategy, threshold)."""
+    from paper_2607_04676_b200 import ring
+    cfg = {"config3": wl.config3, "config4": wl.config4, "config5": lambda: wl.config5(0)}[name]()
+    X = cfg.buffers(device=device)
+    P, n = cfg.ranks, cfg.chunk
+    dense_bytes = P * P * n * 4
+
+    def timed(fn):
+        fn()                                   # warm-up (also builds the pooled buffers)
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(iters):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); res = fn(); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        ts.sort()
+        return ts[len(ts) // 2], res
+
+    if name == "config3":
+        cases = [("reduce_scatter", st, pm) for st in ("fused", "paper") for pm in (400, 80, 40, 20)]
+    elif name == "config4":
+        cases = [("all_reduce", st, pm) for st in ("fused", "paper") for pm in (400, 200, 100)]
+    else:
+        cases = [("all_gather", "fused", 900), ("all_reduce", "fused", 400), ("all_reduce", "paper", 400)]
+    for coll, strategy, permille in cases:
+        drv = ring.RingDriver(P, n, device=device, strategy=strategy)
+        sw = wl.nnz_switch_from_permille(n, permille)
+        if coll == "reduce_scatter":
+            ms, res = timed(lambda: drv.reduce_scatter(X, sw))
+        elif coll == "all_reduce":
+            ms, res = timed(lambda: drv.all_reduce(X, sw, wl.nnz_switch_from_permille(n, 900)))
+        else:
+            ms, res = timed(lambda: drv.all_gather([X[r][r * n:(r + 1) * n] for r in range(P)]))
+        steps = res.switch_steps("rs") if coll != "all_gather" else {}
+        print(json.dumps({"config": name, "collective": coll, "strategy": strategy, "theta_permille": permille,
+                          "ranks": P, "chunk": n, "ms": round(ms, 3),
+                          "dense_equiv_gbs": round(dense_bytes / ms / 1e6, 1),   # P ranks x N elements x 4 bytes
+                          "switch_step_per_chunk": [steps.get(c) for c in range(P)] if steps else None}), flush=True)
+        del drv, res
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -374,6 +420,8 @@ def main():
     ap.add_argument("--ops", default="compress,decompress,reduce_ss,reduce_sd")
     ap.add_argument("--dtypes", default="f32,bf16")
     ap.add_argument("--sparsities", default="")
+    ap.add_argument("--ring", default="", choices=["", "config3", "config4", "config5"],
+                    help="time the ring collectives of that config on P logical ranks (one JSON line per case)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -394,6 +442,8 @@ def main():
     n = 1 << args.log2n
     density = 1.0 - args.sparsity
     peak, peak_src = measured_peak()
+    if args.ring:
+        return run_ring(pk, args.ring, max(3, args.sweep_iters), device)
     if args.sweep_only:   # kernel-by-kernel timing (also the program the single-kernel ncu captures run)
         sp = tuple(float(v) for v in args.sparsities.split(",")) if args.sparsities else None
         for r in run_sweep(pk, n, peak, args.sweep_iters, device, tuple(args.dtypes.split(",")), sp, tuple(args.ops.split(","))):
