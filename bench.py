@@ -366,16 +366,34 @@ def run_ring(pk, name: str, iters: int, device) -> None:
     dense_bytes = P * P * n * 4
 
     def timed(fn):
+        """(median ms of eager enqueues, median ms of CUDA-graph replays of the same enqueues, result)"""
         fn()                                   # warm-up (also builds the pooled buffers)
         torch.cuda.synchronize()
-        ts = []
-        for _ in range(iters):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); res = fn(); b.record()
+
+        def med(run):
+            ts = []
+            for _ in range(iters):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); run(); b.record()
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            ts.sort()
+            return ts[len(ts) // 2]
+
+        eager = med(fn)
+        graph_ms = None
+        try:                                   # the whole collective as ONE graph launch: no per-kernel host cost
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                res = fn()
+            g.replay()
             torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b))
-        ts.sort()
-        return ts[len(ts) // 2], res
+            graph_ms = med(g.replay)
+        except Exception as e:                 # report, do not hide
+            res = fn()
+            graph_ms = f"capture failed: {type(e).__name__}: {e}"[:160]
+        torch.cuda.synchronize()
+        return eager, graph_ms, res
 
     if name == "config3":
         cases = [("reduce_scatter", st, pm) for st in ("fused", "paper") for pm in (400, 80, 40, 20)]
@@ -387,15 +405,16 @@ def run_ring(pk, name: str, iters: int, device) -> None:
         drv = ring.RingDriver(P, n, device=device, strategy=strategy)
         sw = wl.nnz_switch_from_permille(n, permille)
         if coll == "reduce_scatter":
-            ms, res = timed(lambda: drv.reduce_scatter(X, sw))
+            ms, gms, res = timed(lambda: drv.reduce_scatter(X, sw))
         elif coll == "all_reduce":
-            ms, res = timed(lambda: drv.all_reduce(X, sw, wl.nnz_switch_from_permille(n, 900)))
+            ms, gms, res = timed(lambda: drv.all_reduce(X, sw, wl.nnz_switch_from_permille(n, 900)))
         else:
-            ms, res = timed(lambda: drv.all_gather([X[r][r * n:(r + 1) * n] for r in range(P)]))
+            ms, gms, res = timed(lambda: drv.all_gather([X[r][r * n:(r + 1) * n] for r in range(P)]))
         steps = res.switch_steps("rs") if coll != "all_gather" else {}
         print(json.dumps({"config": name, "collective": coll, "strategy": strategy, "theta_permille": permille,
-                          "ranks": P, "chunk": n, "ms": round(ms, 3),
-                          "dense_equiv_gbs": round(dense_bytes / ms / 1e6, 1),   # P ranks x N elements x 4 bytes
+                          "ranks": P, "chunk": n, "ms_eager": round(ms, 3),
+                          "ms_cuda_graph": round(gms, 3) if isinstance(gms, float) else gms,
+                          "dense_equiv_gbs": round(dense_bytes / (gms if isinstance(gms, float) else ms) / 1e6, 1),   # P ranks x N x 4 bytes
                           "switch_step_per_chunk": [steps.get(c) for c in range(P)] if steps else None}), flush=True)
         del drv, res
         torch.cuda.empty_cache()

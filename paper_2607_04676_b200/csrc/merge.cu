@@ -607,7 +607,9 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
         per_sm = v > 0 ? v : 1;
         configured = true;
     }
-    uint64_t blocks = T;   // the span length is chosen on the device; surplus CTAs find no span and exit
+    // the span length is chosen on the device.  A chunk of a few thousand tiles does not need the whole GPU:
+    // one CTA per 16 tiles leaves room for the other logical ranks' launches of the same ring step
+    uint64_t blocks = (T + 15) / 16;
     uint64_t cap = (uint64_t)num_sms() * per_sm;   // cooperative: exactly one co-resident wave
     if (cap > kMaxGrid) cap = kMaxGrid;
     if (blocks > cap) blocks = cap;

@@ -19,6 +19,11 @@ Two equivalent ways to take the step, both bit-identical to the oracle's message
                     touching a dense buffer while the chunk stays sparse (north_star).
 A chunk that reached nnz >= nnz_switch travels dense from then on (pici_maybe_densify, PAPER.md:227;
 once dense it stays dense within the reduce-scatter, C8).
+
+The P ranks' kernels of one ring step are independent of one another, and a chunk is a few thousand tiles -
+too little to fill 148 SMs from one launch - so with concurrent=True every logical rank enqueues on its own
+CUDA stream and the streams join after every step (SURVEY.md S7 hard part 5).  The whole collective can be
+captured into ONE CUDA graph (the cross-stream events become graph edges): bench.py --ring times both.
 """
 from __future__ import annotations
 
@@ -72,10 +77,14 @@ class RingResult:
 class RingDriver:
     """Buffers for P logical ranks with chunk length n (elements, multiple of 4096), fp32."""
 
-    def __init__(self, ranks: int, chunk: int, device="cuda", strategy: str = "fused", keep_messages: bool = False):
+    def __init__(self, ranks: int, chunk: int, device="cuda", strategy: str = "fused", keep_messages: bool = False,
+                 concurrent: bool = True):
         assert chunk % pk.TILE == 0 and ranks >= 2 and strategy in ("fused", "paper")
         self.P, self.n, self.device, self.strategy = ranks, chunk, device, strategy
         self.keep = keep_messages
+        self.streams = [torch.cuda.Stream(device=device) for _ in range(ranks)] if concurrent else None
+        self._ev_main = torch.cuda.Event()
+        self._ev_rank = [torch.cuda.Event() for _ in range(ranks)]
         P = ranks
         n_sets = (2 * P) if not keep_messages else None
         self._pool: list[_Msg] = []
@@ -103,6 +112,24 @@ class RingDriver:
         return m
 
     # ------------------------------------------------------------------------------------------
+    def _step(self, body) -> None:
+        """Run body(r) for every rank r: on rank r's own stream (all forked from the current stream, all joined
+        back into it afterwards) when concurrent, else in order on the current stream."""
+        if self.streams is None:
+            for r in range(self.P):
+                body(r)
+            return
+        main = torch.cuda.current_stream(self.device)
+        self._ev_main.record(main)
+        for r in range(self.P):
+            st = self.streams[r]
+            st.wait_event(self._ev_main)
+            with torch.cuda.stream(st):
+                body(r)
+            self._ev_rank[r].record(st)
+        for r in range(self.P):
+            main.wait_event(self._ev_rank[r])
+
     def _begin(self) -> RingResult:
         res = RingResult([], [], self.fmt, self.nnz)
         return res
@@ -141,20 +168,23 @@ class RingDriver:
         chunk = lambda r, c: X[r][c * n:(c + 1) * n]
 
         cur = [None] * P
-        for r in range(P):                                   # step 0: always compress
+
+        def step0(r):                                        # step 0: always compress
             c = (r - 1) % P
             cur[r] = self._encode(res, "rs", 0, r, c, chunk(r, c), nnz_switch, copy_dense=True)
+        self._step(step0)
 
         for s in range(1, P):
             nxt = [None] * P
-            for r in range(P):
+
+            def step(r, s=s, cur=cur, nxt=nxt):
                 (m_in, f_in) = cur[(r - 1) % P]
                 c = (r - 1 - s) % P
                 loc = chunk(r, c)
                 if s == P - 1:                                # last step: acc is rank r's dense output
                     pk.reduce_sd_out(m_in.pici, loc, outs[r], gate=f_in, gate_value=pk.FMT_PICI)
                     pk.dense_add(m_in.dense, loc, outs[r], None, gate=f_in, gate_value=pk.FMT_DENSE)
-                    continue
+                    return
                 m = self._msg()
                 rec = self._record(res, "rs", s, r, c, m)
                 f = self.fmt[rec.fmt_index:rec.fmt_index + 1]
@@ -169,6 +199,7 @@ class RingDriver:
                 pk.nnz(m.pici, self.nnz[rec.nnz_index:rec.nnz_index + 1])
                 pk.dense_add(m_in.dense, loc, m.dense, f, gate=f_in, gate_value=pk.FMT_DENSE)
                 nxt[r] = (m, f)
+            self._step(step)
             cur = nxt
         res.outputs = outs
         return res
@@ -184,16 +215,19 @@ class RingDriver:
         outs = outputs or [torch.empty(P * n, dtype=torch.float32, device=self.device) for _ in range(P)]
         switch = nnz_switch if nnz_switch is not None else n + 1
         msgs = [None] * P
-        for r in range(P):                                   # step 0: compress once
+
+        def step0(r):                                        # step 0: compress once
             msgs[r] = self._encode(res, phase, 0, r, r, shards[r], switch, copy_dense=False)
             pk.dense_copy(shards[r], outs[r][r * n:(r + 1) * n])          # own slot: plain copy (C9 #12)
+        self._step(step0)
         for s in range(1, P):
-            for r in range(P):
+            def step(r, s=s):
                 c = (r - s) % P                               # forwarded unchanged: still rank c's message
                 m, f = msgs[c]
                 slot = outs[r][c * n:(c + 1) * n]
                 pk.decompress(m.pici, slot, gate=f, gate_value=pk.FMT_PICI)
                 pk.dense_copy(m.dense, slot, gate=f, gate_value=pk.FMT_DENSE)
+            self._step(step)
         res.outputs = outs
         return res
 
