@@ -163,3 +163,28 @@ def test_pooled_buffers_give_the_same_outputs(mods):
         torch.cuda.synchronize()
         for r in range(cfg.ranks):
             assert np.array_equal(_u32(res.outputs[r]), want[r].view(np.uint32))
+
+
+def test_ring_is_cuda_graph_capturable(mods):
+    """The whole collective - per-rank streams, gated kernels, cooperative launches, workspace memsets - is
+    captured into ONE CUDA graph; replays give the oracle's outputs again (no host decision inside)."""
+    pk, ring = mods
+    cfg = _small(4, 6, 0.03, seed=21)
+    Xh = [b.numpy() for b in cfg.buffers()]
+    n = cfg.chunk
+    sw = wl.nnz_switch_from_permille(n, 70)
+    want_out, _ = ro.ring_reduce_scatter(Xh, sw, keep_messages=False)
+    X = [torch.from_numpy(v).cuda() for v in Xh]
+    drv = ring.RingDriver(cfg.ranks, n)
+    drv.reduce_scatter(X, sw)                       # warm-up outside the capture (lazy one-time setup)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        res = drv.reduce_scatter(X, sw)
+    for _ in range(3):
+        for o in res.outputs:
+            o.fill_(7.0)
+        g.replay()
+        torch.cuda.synchronize()
+        for r in range(cfg.ranks):
+            assert np.array_equal(_u32(res.outputs[r]), want_out[r].view(np.uint32))
