@@ -233,7 +233,7 @@ struct WalkOut {
 template <bool EMIT>
 __device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *out, MergeShared &sh, uint32_t By0, uint32_t Xb,
                                              uint32_t Yb, uint32_t m, uint32_t mt, uint32_t (&ao)[4], int tid,
-                                             uint32_t trace_it = 99u) {
+                                             uint16_t *run_at = nullptr, uint16_t *run_k = nullptr, uint32_t trace_it = 99u) {
     const int lane = tid & 31, warp = tid >> 5;
     uint32_t ax[4], ay[4];
     read_piece(stage, By0, m, mt, tid, ax, ay);
@@ -248,16 +248,21 @@ __device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *ou
     }
     walkers_sync();  // #1: warp totals are visible
     PICI_TR(trace_it, 2);
-    uint32_t bxy = 0, bu = 0, cand_total = 0;
+    // prefix over the 16 warp totals: lanes 0..15 of every warp scan them with shuffles (an unrolled loop over
+    // the 16 shared-memory words costs ~80 instructions per thread; the kernel is issue-bound on exactly this
+    // kind of per-span bookkeeping: 60 % issue activity with almost no values to add at 99.99 % sparsity)
+    uint32_t pw = lane < kMergeWarps ? sh.wxy[lane] : 0u, uw = lane < kMergeWarps ? sh.wu[lane] : 0u;
 #pragma unroll
-    for (int q = 0; q < kMergeWarps; ++q) {
-        const uint32_t p = sh.wxy[q], u = sh.wu[q];
-        if (q < warp) {
-            bxy += p;
-            bu += u;
+    for (int d = 1; d < kMergeWarps; d <<= 1) {
+        const uint32_t o1 = __shfl_up_sync(kFull, pw, d), o2 = __shfl_up_sync(kFull, uw, d);
+        if (lane >= d) {
+            pw += o1;
+            uw += o2;
         }
-        cand_total += u;
     }
+    const uint32_t cand_total = __shfl_sync(kFull, uw, kMergeWarps - 1);
+    const uint32_t bxy = warp > 0 ? __shfl_sync(kFull, pw, (warp + 31) & 31) : 0u;   // inclusive prefix of warp - 1
+    const uint32_t bu = warp > 0 ? __shfl_sync(kFull, uw, (warp + 31) & 31) : 0u;
     if (EMIT && cand_total > kOutWords) {   // uniform: more candidates than the output region holds
         WalkOut none = {0u, 0u, 0u, cand_total};
         return none;                        // the caller takes the tile-by-tile path (only one barrier passed)
@@ -290,6 +295,10 @@ __device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *ou
     r.sk = warp_incl_scan(r.k, lane);
     r.cand_total = cand_total;
     if (lane == 31) sh.ws[warp] = r.sk;
+    if (run_at != nullptr) {   // where this thread's survivors sit: only read if the span had a cancellation
+        run_at[tid] = (uint16_t)ko0;
+        run_k[tid] = (uint16_t)r.k;
+    }
     walkers_sync();  // #2: survivor totals and the output region are visible; the stage is no longer read
     PICI_TR(trace_it, 4);
     return r;
@@ -519,18 +528,12 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
         if (!slow) {
             // ---- walk, publish the count; the service warp of stage s does the rest ---------------------
             uint32_t ao[4];
-            const WalkOut r = walk_span<true>(stage, out_s, sh, m * kTileWords, info.Xb, info.Yb, m, mt, ao, tid, j);
+            const WalkOut r = walk_span<true>(stage, out_s, sh, m * kTileWords, info.Xb, info.Yb, m, mt, ao, tid,
+                                              sh.run_at[s], sh.run_k[s], j);
             slow = r.cand_total > kOutWords;   // uniform; nothing was written
             if (!slow) {
-                uint32_t before, surv_total;
-                survivor_sums(sh, warp, before, surv_total);
-                const bool cancelled = surv_total != r.cand_total;   // uniform
-                if (cancelled) {   // the region is not contiguous: leave the runs for the flush
-                    sh.run_at[s][tid] = (uint16_t)r.ko0;
-                    sh.run_k[s][tid] = (uint16_t)r.k;
-                    walkers_sync();
-                }
-                if (warp == 0) {
+                if (warp == 0) {   // the other 15 warps go straight on to their piece of Bo and the next span
+                    const uint32_t surv_total = warp_sum(lane < kMergeWarps ? sh.ws[lane] : 0u);
                     const uint32_t wpt = (uint32_t)kMergeWarps / m;   // a tile is covered by 16/m consecutive warps
                     uint32_t tc = 0;
                     if ((uint32_t)lane < mt)
