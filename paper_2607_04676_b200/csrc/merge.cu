@@ -519,7 +519,9 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
         uint32_t *const stage = pool + s * kStageWords;
         uint32_t *const out_s = out + s * kOutWords;
         PICI_TR(j, 0);
-        if (j >= 2) mbar_wait(fl0 + 8 * s, ph ^ 1u);   // span j - 2 has left output region s
+        // span j - 2 must have left output region s before anything is written to it; warp 0 waits for all (the
+        // first write comes behind the walkers' barrier #1, which warp 0 joins afterwards): 15 warps fewer polling
+        if (j >= 2 && warp == 0) mbar_wait(fl0 + 8 * s, ph ^ 1u);
         mbar_wait(full0 + 8 * s, ph);
         PICI_TR(j, 1);
         const SpanInfo info = sh.info[s];
