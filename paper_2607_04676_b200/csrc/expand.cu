@@ -205,6 +205,9 @@ expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, co
         uint32_t k1 = k0 + cnt0;                                  // cursor of column 2l+1
         const uint32_t w0lo = (uint32_t)w.x, w0hi = (uint32_t)(w.x >> 32);
         const uint32_t w1lo = (uint32_t)w.y, w1hi = (uint32_t)(w.y >> 32);
+        // rows of the tile that hold any value at all (at 99 % sparsity half of them do not: those rows are
+        // one store of zeros, no bit tests, no shared-memory reads)
+        const uint32_t rows_lo = __reduce_or_sync(kFull, w0lo | w1lo), rows_hi = __reduce_or_sync(kFull, w0hi | w1hi);
 
         if (full) {
             constexpr int kChunk = 16;
@@ -231,8 +234,12 @@ expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, co
                     const bool b1 = ((r < 32 ? w1lo : w1hi) & m) != 0u;
                     if constexpr (MODE == kModeDecompress) {
                         uint32_t v0 = 0, v1 = 0;
-                        if (b0) v0 = stage[k0++];
-                        if (b1) v1 = stage[k1++];
+                        if (DT != PICI_F32 || ((r < 32 ? rows_lo : rows_hi) & m)) {   // warp-uniform: some lane has a value in
+                                                                                      // this row (bf16: the test costs more
+                                                                                      // than it saves, measured)
+                            if (b0) v0 = stage[k0++];
+                            if (b1) v1 = stage[k1++];
+                        }
                         if constexpr (DT == PICI_F32) {
                             stg_stream_u2(reinterpret_cast<uint2 *>(Dout + base) + lane + 32 * r, make_uint2(v0, v1));
                         } else {
