@@ -16,9 +16,7 @@ Two equivalent ways to take the step, both bit-identical to the oracle's message
   strategy="paper": scatter-add the received Pici into a dense scratch (pici_reduce_sd), recompress
                     it (pici_compress), PAPER.md:219;
   strategy="fused": compress the local chunk and merge sparse+sparse (pici_reduce_ss), never
-                    touching a dense buffer while the chunk stays sparse (north_star).  The local chunks
-                    of all later steps are compressed at step 0 (they depend on no message), which takes
-                    the compress out of every step's dependent chain.
+                    touching a dense buffer while the chunk stays sparse (north_star).
 A chunk that reached nnz >= nnz_switch travels dense from then on (pici_maybe_densify, PAPER.md:227;
 once dense it stays dense within the reduce-scatter, C8).
 
@@ -92,10 +90,7 @@ class RingDriver:
         self._pool: list[_Msg] = []
         self._n_sets = n_sets
         self._cursor = 0
-        # fused strategy: rank r's local chunks of steps 1 .. P-2 are compressed up front, all ranks and steps at
-        # once (they do not depend on any incoming message), so a ring step is merge + switch only
-        self.local = [[pk.alloc_pici(chunk, pk.F32, device) for _ in range(max(P - 2, 0))] for _ in range(P)] \
-            if strategy == "fused" else None
+        self.local = [pk.alloc_pici(chunk, pk.F32, device) for _ in range(P)] if strategy == "fused" else None
         self.ws = [pk.alloc_workspace(chunk, device) for _ in range(P)]
         max_records = 4 * P * P + 4 * P
         self.fmt = torch.zeros(max_records, dtype=torch.int32, device=device)
@@ -177,9 +172,6 @@ class RingDriver:
         def step0(r):                                        # step 0: always compress
             c = (r - 1) % P
             cur[r] = self._encode(res, "rs", 0, r, c, chunk(r, c), nnz_switch, copy_dense=True)
-            if self.strategy == "fused":                     # ... and the local operands of the later merges
-                for s in range(1, P - 1):
-                    pk.compress(chunk(r, (r - 1 - s) % P), self.local[r][s - 1], self.ws[r])
         self._step(step0)
 
         for s in range(1, P):
@@ -197,7 +189,8 @@ class RingDriver:
                 rec = self._record(res, "rs", s, r, c, m)
                 f = self.fmt[rec.fmt_index:rec.fmt_index + 1]
                 if self.strategy == "fused":
-                    pk.reduce_ss(m_in.pici, self.local[r][s - 1], m.pici, self.ws[r], gate=f_in, gate_value=pk.FMT_PICI)
+                    pk.compress(loc, self.local[r], self.ws[r], gate=f_in, gate_value=pk.FMT_PICI)
+                    pk.reduce_ss(m_in.pici, self.local[r], m.pici, self.ws[r], gate=f_in, gate_value=pk.FMT_PICI)
                     pk.maybe_densify(m.pici, nnz_switch, m.dense, f, gate=f_in, gate_value=pk.FMT_PICI)
                 else:
                     pk.reduce_sd_out(m_in.pici, loc, m.dense, gate=f_in, gate_value=pk.FMT_PICI)
