@@ -12,29 +12,29 @@
 // position: it is a 1-D merge of two (bit string, value stream) pairs, and I[t] is the number of
 // survivors before bit 4096*t.  The kernel works on SPANS of that string:
 //   * a span is m = 16, 8, 4, 2 or 1 consecutive tiles, the same m for the whole launch: the largest
-//     whose AVERAGE contents fit one shared-memory stage (read on the device from Ix[T] + Iy[T]),
-//     halved while the launch has fewer than two spans per CTA;
-//   * the launch is COOPERATIVE with G CTAs of 512 threads (two per SM); CTA c takes spans c, c + G,
-//     c + 2G, ... and runs a two-stage software pipeline: while span i is walked, the whole of span
-//     i+1 - its Bx / By words (contiguous) and its X / Y value runs (contiguous in Ax / Ay) - is in
-//     flight into the other stage as four 1-D TMA bulk copies on one mbarrier; index entries are
-//     loaded two spans ahead so the copies never wait on them;
-//   * thread j owns the 8m-bit piece j of the span; x's and y's cursors come from the block-wide popc
-//     prefix of their own pieces, the candidate cursor from the popc prefix of the OR; every thread
-//     walks the set bits of its piece, adds, tests the predicate and packs its surviving sums into its
-//     own run of an output region (runs start at the OR-prefix, so they never overlap);
-//   * Phase 2 (exclusive scan of the counts) uses the round-robin structure: iteration
-//     `it` of the grid covers spans [it*G, (it+1)*G).  A CTA publishes its span's survivor count as
-//     (a) a per-span word, (b) an atomic add into the word of its group of 32 spans, (c) an atomic add
-//     into the word of its iteration; each word carries (how many have added, sum).  The prefix of
-//     span (it, c) = running sum of complete iterations + complete groups below c + the spans of its
-//     own group below c: three independent loads, ONE L2 round trip, 64 words per look-back (a flat
-//     decoupled look-back walks up to G/32 dependent hops here because the CTAs run in lock-step and
-//     nobody below has a prefix yet; a block-wide flat read hot-spots a few L2 lines - both measured);
-//   * a span's look-back and flush are DEFERRED behind the next span's walk (second output region),
-//     so one iteration of skew between CTAs is absorbed;
-//   * a span denser than the stage (the average said it would fit) is processed tile by tile in two
-//     sweeps (count, then emit) - one tile always fits.
+//     whose AVERAGE contents fit one shared-memory stage and whose expected union of the two supports fits
+//     the output region (read on the device from Ix[T], Iy[T]), halved while the launch has fewer than
+//     two spans per CTA;
+//   * the launch is COOPERATIVE with G CTAs (two per SM, all co-resident); CTA c takes spans c, c + G,
+//     c + 2G, ...  A CTA is 16 WALKER warps plus one SERVICE warp per stage (576 threads).  The service
+//     warp of stage s starts the four 1-D TMA bulk copies of a span - its Bx / By words (contiguous) and
+//     its X / Y value runs (contiguous in Ax / Ay), one mbarrier - two spans ahead, index entries loaded
+//     one span before that, so the walkers find the stage filled when they get to it;
+//   * walkers: thread j owns the 8m-bit piece j of the span; x's and y's cursors come from the
+//     block-wide popc prefix of their own pieces, the candidate cursor from the popc prefix of the OR;
+//     every thread walks the set bits of its piece, adds, tests the predicate and packs its surviving
+//     sums into its own run of the stage's output region (runs start at the OR-prefix, so they never
+//     overlap); they publish the span's count and go on - they never wait for a look-back;
+//   * Phase 2 (exclusive scan of the counts) is the round-robin scan of pici_common.cuh:
+//     per-span / per-32-spans / per-iteration words, prefix = three independent loads (a flat decoupled
+//     look-back walks up to G/32 dependent hops here because the CTAs run in lock-step; a block-wide flat
+//     read hot-spots a few L2 lines - both measured).  The service warp takes the prefix once the count
+//     is out, writes the span's index entries and copies the output region to Ao (packed; if a
+//     cancellation left gaps, run by run from what the walkers recorded), then releases the region;
+//   * a span whose values do not fit the stage, or whose exact candidate count exceeds the output region
+//     (the span length is chosen from an estimate), is processed tile by tile in two sweeps (count, then
+//     emit) by the walkers themselves - one tile always fits.
+// The kernel is bound by the issue of its per-span bookkeeping, not by HBM (S5).
 #include "launch.h"
 #include "pici_common.cuh"
 #include "../../include/pici.h"
