@@ -149,6 +149,14 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
             reinterpret_cast<ulonglong2 *>(B + (size_t)t * kSide)[lane] = w;
         }
 
+        // ---- the next tile (its ticket has arrived during Phase 1) starts moving HBM -> L2 now, as ONE bulk
+        // prefetch of its 16 KB / 8 KB: the 64 row loads issued at the end of this iteration then hit L2 ----
+        const uint32_t tn = __shfl_sync(kFull, t_next, 0);
+        if (tn < Tfull && lane == 0) {
+            const unsigned char *src = reinterpret_cast<const unsigned char *>(dense) + (size_t)tn * kTile * sizeof(Elem);
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(kTile * sizeof(Elem))) : "memory");
+        }
+
         // ---- Phase 3b of the PREVIOUS tile: its prefix has had a whole iteration to arrive --------
         flush_pending();
 
@@ -177,7 +185,6 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
         pt = t;
         pnnz = tile_nnz;
 
-        const uint32_t tn = __shfl_sync(kFull, t_next, 0);
         if (tn < Tfull) {
             load_full(tn, v);
         } else if (tn < T) {  // the ragged tile is padded through the stage: flush first
