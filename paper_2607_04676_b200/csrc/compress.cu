@@ -113,9 +113,16 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
         }
     };
 
+    uint32_t t_next = 0;  // next ticket (lane 0): requested right behind a tile's loads, it arrives while they do
+    if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
     while (t < T) {
-        uint32_t t_next = 0;  // next ticket: its latency hides behind this tile
-        if (lane == 0) t_next = atomicAdd(ticket, 1u);
+        // ---- the next tile starts moving HBM -> L2 now, as ONE bulk prefetch of its 16 KB / 8 KB: the 64 row
+        // loads issued at the end of this iteration then hit L2 ----
+        const uint32_t tn = __shfl_sync(kFull, t_next, 0);
+        if (tn < Tfull && lane == 0) {
+            const unsigned char *src = reinterpret_cast<const unsigned char *>(dense) + (size_t)tn * kTile * sizeof(Elem);
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(kTile * sizeof(Elem))) : "memory");
+        }
 
         // ---- Phase 1: column words (bit r <-> row r) and counts --------------------------------
         uint32_t w0lo = 0, w0hi = 0, w1lo = 0, w1hi = 0;
@@ -147,14 +154,6 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
             w.x = ((uint64_t)w0hi << 32) | w0lo;
             w.y = ((uint64_t)w1hi << 32) | w1lo;
             reinterpret_cast<ulonglong2 *>(B + (size_t)t * kSide)[lane] = w;
-        }
-
-        // ---- the next tile (its ticket has arrived during Phase 1) starts moving HBM -> L2 now, as ONE bulk
-        // prefetch of its 16 KB / 8 KB: the 64 row loads issued at the end of this iteration then hit L2 ----
-        const uint32_t tn = __shfl_sync(kFull, t_next, 0);
-        if (tn < Tfull && lane == 0) {
-            const unsigned char *src = reinterpret_cast<const unsigned char *>(dense) + (size_t)tn * kTile * sizeof(Elem);
-            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(kTile * sizeof(Elem))) : "memory");
         }
 
         // ---- Phase 3b of the PREVIOUS tile: its prefix has had a whole iteration to arrive --------
@@ -192,6 +191,7 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
             load_ragged(tn, v);
         }
         t = tn;
+        if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
     }
     flush_pending();
 }
