@@ -222,7 +222,8 @@ static cudaError_t launch_compress_t(const void *dense, uint64_t n, uint64_t *B,
     using Cfg = CompressCfg<DT>;
     const uint64_t T = (n + kTile - 1) / kTile;
     const size_t smem = (size_t)kCompressWarps * kTile * sizeof(typename Cfg::Elem);
-    static bool configured = false;
+    static bool configured_on[64] = {false};
+    bool &configured = configured_on[current_device_slot()];
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(compress_kernel<DT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;

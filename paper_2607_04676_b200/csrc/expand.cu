@@ -378,7 +378,8 @@ static cudaError_t launch_expand_t(const uint64_t *B, const uint32_t *I, const v
                                    const void *local, void *out, DensifyCtl ctl, Gate g, cudaStream_t s) {
     const uint64_t T = (n + kTile - 1) / kTile;
     const size_t smem = (size_t)kExpandWarps * ExpandCfg<DT>::kStageBytes;
-    static bool configured = false;
+    static bool configured_on[64] = {false};
+    bool &configured = configured_on[current_device_slot()];
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(expand_kernel<DT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;

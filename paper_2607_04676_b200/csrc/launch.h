@@ -14,6 +14,14 @@ struct Gate {
 
 int num_sms();  // cached cudaDevAttrMultiProcessorCount of the current device
 
+// Index (0..63) of the current device: one-time per-kernel setup (cudaFuncSetAttribute, occupancy) is kept
+// per device, so a process that drives several GPUs configures each of them.
+inline int current_device_slot() {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return (dev < 0 || dev >= 64) ? 0 : dev;
+}
+
 uint64_t scan_workspace_bytes(uint64_t n);
 
 cudaError_t launch_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,

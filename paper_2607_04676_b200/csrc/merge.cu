@@ -601,8 +601,10 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
     if (n == 0) return launch_set_u32(Io, 0u, g, s);
     const uint64_t T = (n + kTile - 1) / kTile;
     const size_t smem = (size_t)kPoolWords * sizeof(uint32_t);
-    static bool configured = false;
-    static int per_sm = 0;
+    static bool configured_on[64] = {false};
+    static int per_sm_on[64] = {0};
+    bool &configured = configured_on[current_device_slot()];
+    int &per_sm = per_sm_on[current_device_slot()];
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(reduce_ss_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
