@@ -35,6 +35,8 @@
 //     (the span length is chosen from an estimate), is processed tile by tile in two sweeps (count, then
 //     emit) by the walkers themselves - one tile always fits.
 // The kernel is bound by the issue of its per-span bookkeeping, not by HBM (S5).
+#include <type_traits>
+
 #include "launch.h"
 #include "pici_common.cuh"
 #include "../../include/pici.h"
@@ -165,6 +167,11 @@ __device__ __forceinline__ SpanLayout span_stage(const MergeArgs &a, uint32_t *s
     const uint32_t bbytes = mt * kTileWords * 4u;
     L.tx = 2u * bbytes + wx.bulk + wy.bulk;
     if (issue) {
+        // tail elements first (plain stores, < 4 per operand), so that lane 0's arrive on the mbarrier - the
+        // release the walkers' wait acquires - is ordered behind every lane's stores
+        if (wx.tail_beg + lane < nx) stage[L.Xb + wx.tail_beg + lane] = a.Ax[xs + wx.tail_beg + lane];
+        if (wy.tail_beg + lane < ny) stage[L.Yb + wy.tail_beg + lane] = a.Ay[ys + wy.tail_beg + lane];
+        __syncwarp();
         if (lane == 0) {
             fence_proxy_async_smem();
             mbar_expect_tx(bar, L.tx);
@@ -174,8 +181,6 @@ __device__ __forceinline__ SpanLayout span_stage(const MergeArgs &a, uint32_t *s
             if (wy.bulk)
                 bulk_g2s(smem_u32(stage + V + wx.words), reinterpret_cast<const unsigned char *>(a.Ay) + wy.g_beg, wy.bulk, bar);
         }
-        if (wx.tail_beg + lane < nx) stage[L.Xb + wx.tail_beg + lane] = a.Ax[xs + wx.tail_beg + lane];   // < 4 elements
-        if (wy.tail_beg + lane < ny) stage[L.Yb + wy.tail_beg + lane] = a.Ay[ys + wy.tail_beg + lane];
     }
     return L;
 }
@@ -512,86 +517,98 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     }
 
     // ======================================= walker warps =======================================
+    // The loop is instantiated once per span length, so the piece width, the tile / warp ratio and the empty
+    // words of narrow pieces are compile-time facts (the kernel is bound by exactly these instructions).
     uint32_t slow_par = 0;
-    for (uint32_t j = 0; c + j * G < spans; ++j) {
-        const uint32_t s = j & 1u, ph = (j >> 1) & 1u;
-        const uint32_t g = c + j * G, ts = g * m, mt = min(m, T - ts);
-        uint32_t *const stage = pool + s * kStageWords;
-        uint32_t *const out_s = out + s * kOutWords;
-        PICI_TR(j, 0);
-        // span j - 2 must have left output region s before anything is written to it; warp 0 waits for all (the
-        // first write comes behind the walkers' barrier #1, which warp 0 joins afterwards): 15 warps fewer polling
-        if (j >= 2 && warp == 0) mbar_wait(fl0 + 8 * s, ph ^ 1u);
-        mbar_wait(full0 + 8 * s, ph);
-        PICI_TR(j, 1);
-        const SpanInfo info = sh.info[s];
+    auto walkers = [&](auto span_len) {
+        constexpr uint32_t M = decltype(span_len)::value;
+        for (uint32_t j = 0; c + j * G < spans; ++j) {
+            const uint32_t s = j & 1u, ph = (j >> 1) & 1u;
+            const uint32_t g = c + j * G, ts = g * M, mt = min(M, T - ts);
+            uint32_t *const stage = pool + s * kStageWords;
+            uint32_t *const out_s = out + s * kOutWords;
+            PICI_TR(j, 0);
+            // span j - 2 must have left output region s before anything is written to it; warp 0 waits for all (the
+            // first write comes behind the walkers' barrier #1, which warp 0 joins afterwards): 15 warps fewer polling
+            if (j >= 2 && warp == 0) mbar_wait(fl0 + 8 * s, ph ^ 1u);
+            mbar_wait(full0 + 8 * s, ph);
+            PICI_TR(j, 1);
+            const SpanInfo info = sh.info[s];
 
-        bool slow = info.fits == 0u;
-        if (!slow) {
-            // ---- walk, publish the count; the service warp of stage s does the rest ---------------------
-            uint32_t ao[4];
-            const WalkOut r = walk_span<true>(stage, out_s, sh, m * kTileWords, info.Xb, info.Yb, m, mt, ao, tid,
-                                              sh.run_at[s], sh.run_k[s], j);
-            slow = r.cand_total > kOutWords;   // uniform; nothing was written
+            bool slow = info.fits == 0u;
             if (!slow) {
-                if (warp == 0) {   // the other 15 warps go straight on to their piece of Bo and the next span
-                    const uint32_t surv_total = warp_sum(lane < kMergeWarps ? sh.ws[lane] : 0u);
-                    const uint32_t wpt = (uint32_t)kMergeWarps / m;   // a tile is covered by 16/m consecutive warps
-                    uint32_t tc = 0;
-                    if ((uint32_t)lane < mt)
-                        for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
-                    if (lane < kMaxSpan) sh.tcs[s][lane] = tc;
-                    if (lane == 0) {
-                        sh.tot[s] = surv_total;
-                        sh.cand[s] = r.cand_total;
-                        publish_span(a, g, j, c, surv_total);
-                        mbar_arrive(free0 + 8 * s);           // every walker is past barrier #2
+                // ---- walk, publish the count; the service warp of stage s does the rest ---------------------
+                uint32_t ao[4];
+                const WalkOut r = walk_span<true>(stage, out_s, sh, M * kTileWords, info.Xb, info.Yb, M, mt, ao, tid,
+                                                  sh.run_at[s], sh.run_k[s], j);
+                slow = r.cand_total > kOutWords;   // uniform; nothing was written
+                if (!slow) {
+                    if (warp == 0) {   // the other 15 warps go straight on to their piece of Bo and the next span
+                        const uint32_t surv_total = warp_sum(lane < kMergeWarps ? sh.ws[lane] : 0u);
+                        const uint32_t wpt = (uint32_t)kMergeWarps / M;   // a tile is covered by 16/m consecutive warps
+                        uint32_t tc = 0;
+                        if ((uint32_t)lane < mt)
+                            for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
+                        if (lane < kMaxSpan) sh.tcs[s][lane] = tc;
+                        if (lane == 0) {
+                            sh.tot[s] = surv_total;
+                            sh.cand[s] = r.cand_total;
+                            publish_span(a, g, j, c, surv_total);
+                            mbar_arrive(free0 + 8 * s);           // every walker is past barrier #2
+                        }
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(cnt0 + 8 * s);
                     }
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(cnt0 + 8 * s);
+                    store_piece(a, ts, M, mt, tid, ao);
+                    PICI_TR(j, 6);
                 }
-                store_piece(a, ts, m, mt, tid, ao);
-                PICI_TR(j, 6);
             }
-        }
-        if (slow) {
-            // ---- the span does not fit: tile by tile (one tile always fits), two sweeps -----------------
-            // Sweep 1 counts the survivors of every tile so that the span's count is published before
-            // anything waits (no other CTA ever waits on a half-processed span); sweep 2 emits and the
-            // walkers write Ao themselves (cand = ~0 tells the service warp not to).
-            for (uint32_t i = 0; i < mt; ++i) {
-                const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
-                const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
-                tile_pass<false>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, slow_bar, slow_par, tid);
+            if (slow) {
+                // ---- the span does not fit: tile by tile (one tile always fits), two sweeps -----------------
+                // Sweep 1 counts the survivors of every tile so that the span's count is published before
+                // anything waits (no other CTA ever waits on a half-processed span); sweep 2 emits and the
+                // walkers write Ao themselves (cand = ~0 tells the service warp not to).
+                for (uint32_t i = 0; i < mt; ++i) {
+                    const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
+                    const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
+                    tile_pass<false>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, slow_bar, slow_par, tid);
+                    if (tid == 0) {
+                        uint32_t cnt = 0;
+                        for (int q = 0; q < kMergeWarps; ++q) cnt += sh.ws[q];
+                        sh.tcs[s][i] = cnt;
+                    }
+                }
+                walkers_sync();
                 if (tid == 0) {
-                    uint32_t cnt = 0;
-                    for (int q = 0; q < kMergeWarps; ++q) cnt += sh.ws[q];
-                    sh.tcs[s][i] = cnt;
+                    uint32_t span_total = 0;
+                    for (uint32_t i = 0; i < mt; ++i) span_total += sh.tcs[s][i];
+                    sh.tot[s] = span_total;
+                    sh.cand[s] = ~0u;
+                    publish_span(a, g, j, c, span_total);
+                    mbar_arrive(cnt0 + 8 * s);
                 }
+                mbar_wait(lbd0 + 8 * s, ph);
+                uint32_t off = sh.excl[s];
+                for (uint32_t i = 0; i < mt; ++i) {
+                    const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
+                    const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
+                    const WalkOut r = tile_pass<true>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, slow_bar, slow_par, tid);
+                    uint32_t before, surv_total;
+                    survivor_sums(sh, warp, before, surv_total);
+                    span_flush(a.Ao, out_s, r, off, surv_total, before + r.sk - r.k, tid);
+                    off += surv_total;
+                }
+                walkers_sync();
+                if (tid == 0) mbar_arrive(free0 + 8 * s);
             }
-            walkers_sync();
-            if (tid == 0) {
-                uint32_t span_total = 0;
-                for (uint32_t i = 0; i < mt; ++i) span_total += sh.tcs[s][i];
-                sh.tot[s] = span_total;
-                sh.cand[s] = ~0u;
-                publish_span(a, g, j, c, span_total);
-                mbar_arrive(cnt0 + 8 * s);
-            }
-            mbar_wait(lbd0 + 8 * s, ph);
-            uint32_t off = sh.excl[s];
-            for (uint32_t i = 0; i < mt; ++i) {
-                const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
-                const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
-                const WalkOut r = tile_pass<true>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, slow_bar, slow_par, tid);
-                uint32_t before, surv_total;
-                survivor_sums(sh, warp, before, surv_total);
-                span_flush(a.Ao, out_s, r, off, surv_total, before + r.sk - r.k, tid);
-                off += surv_total;
-            }
-            walkers_sync();
-            if (tid == 0) mbar_arrive(free0 + 8 * s);
         }
+    };
+    switch (m) {
+        case 16: walkers(std::integral_constant<uint32_t, 16>{}); break;
+        case 8: walkers(std::integral_constant<uint32_t, 8>{}); break;
+        case 4: walkers(std::integral_constant<uint32_t, 4>{}); break;
+        case 2: walkers(std::integral_constant<uint32_t, 2>{}); break;
+        default: walkers(std::integral_constant<uint32_t, 1>{}); break;
     }
 }
 
