@@ -182,6 +182,26 @@ def test_reduce_ss_disjoint_supports(pk, d):
     _assert_pici_equal(pk, out, want)
 
 
+@pytest.mark.parametrize("n,dx,dy", ((1, 1.0, 1.0), (3, 0.7, 0.7), (4096 + 3, 0.5, 0.5), (9 * 4096 + 1, 0.02, 0.9),
+                                     (40 * 4096, 0.3, 0.3), (700 * 4096 + 5, 0.01, 0.01)))
+def test_reduce_ss_is_repeatable(pk, n, dx, dy):
+    """The merge kernel hands data between warp roles through mbarriers (staging / walking / scanning): the same
+    launch repeated many times, on buffers whose previous contents differ, must give the oracle's result every
+    time (a stale shared-memory word shows up as an occasional wrong value, not as a steady one)."""
+    x = wl.sparse_buffer(n, dx, seed=31 + n)
+    y = wl.sparse_buffer(n, dy, seed=32 + n)
+    y = torch.where((x != 0) & (y != 0) & (torch.arange(n) % 2 == 0), -x, y)     # many exact cancellations
+    xo, yo = po.compress(_bits(x), "f32"), po.compress(_bits(y), "f32")
+    want = po.reduce_ss(xo, yo)
+    xd, yd = _upload(pk, xo), _upload(pk, yo)
+    ws = pk.alloc_workspace(n)
+    out = pk.alloc_pici(n, pk.F32)
+    for it in range(40):
+        out.B.fill_(it - 3); out.I.fill_(it - 3); out.A.fill_(float(it))
+        pk.reduce_ss(xd, yd, out, ws)
+        _assert_pici_equal(pk, out, want)
+
+
 def test_reduce_ss_special_values(pk):
     n = 4096 + 50
     sp = wl.special_values_f32()
