@@ -190,6 +190,30 @@ def test_index_invariants(density):
     assert not tail_rows[idx >= n].any()
 
 
+def test_nnz_dense_bf16_counts_ieee_nonzeros():
+    """Pin for oracle_nnz_dense_b16 (predicate C1): the count of a bf16 buffer equals
+    (a) the FPU's `x != 0` over the same bits widened exactly to fp32, (b) a brute-force Python loop on
+    the hand-listed special patterns, (c) len(A) of the bf16 compressor - on ragged sizes."""
+    special = np.array([0x0000, 0x8000, 0x0001, 0x8001, 0x007F, 0x0080, 0x7F80, 0xFF80, 0x7FC0, 0xFFC1, 0x7F81,
+                        0x3F80, 0xBF80, 0x7FFF, 0xFFFF], np.uint16)
+    # by hand: only +0 (0x0000) and -0 (0x8000) are zeros; subnormals, Inf and every NaN count
+    assert po.nnz_dense(special, "bf16") == special.size - 2
+    assert po.nnz_dense(special, "bf16") == sum(1 for b in special.tolist() if (b & 0x7FFF) != 0)
+    for k in range(special.size + 1):                 # every prefix: a dropped / doubled element shows
+        assert po.nnz_dense(special[:k].copy(), "bf16") == int(nz_np(special[:k]).sum())
+    for n, dens, seed in ((0, 0.5, 1), (1, 1.0, 2), (63, 0.3, 3), (4097, 0.01, 4), (3 * 4096 + 17, 0.5, 5),
+                          (40 * 4096 + 123, 0.1, 6)):
+        d = b16bits(wl.sparse_buffer(n, dens, seed=seed, dtype="bf16")).copy()
+        if n > 20:
+            d[3], d[7], d[n - 1] = 0x8000, 0x0001, 0x7FC0        # -0.0, smallest subnormal, NaN
+        want = int(nz_np(d).sum())
+        assert po.nnz_dense(d, "bf16") == want
+        assert po.compress(d, "bf16").A.size == want == po.nnz_pici(po.compress(d, "bf16"))
+    # an fp32 buffer viewed as twice as many 16-bit words is NOT the same count: the two variants differ
+    f = f32bits(wl.sparse_buffer(4096, 0.5, seed=9))
+    assert po.nnz_dense(f, "f32") != po.nnz_dense(f.view(np.uint16).copy(), "bf16")
+
+
 def test_index_is_a_random_access_offset_table():
     n = 9 * 4096 + 5
     d = f32bits(wl.sparse_buffer(n, 0.3, seed=2))
