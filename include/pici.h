@@ -24,7 +24,10 @@
  *     including nnz and switch flags, live in device memory.
  *   - The caller owns every buffer.  The library never allocates, frees or retains pointers and has
  *     no global state; it is re-entrant.  `ws` is scratch that must not be shared by calls that may
- *     run concurrently (one workspace per stream).
+ *     run concurrently (one workspace per stream).  A workspace must be cleared ONCE after it is
+ *     allocated (pici_workspace_init, or any memset to 0); after that any sequence of calls on one
+ *     stream may reuse it without clearing: its first 64 bytes hold a launch epoch that the kernels
+ *     advance themselves, and every scan word is tagged with it, so no call starts with a memset.
  *   - Alignment: dense, B, A, ws pointers 16-byte aligned; I 4-byte aligned.  Violations return
  *     PICI_ERR_ALIGN.
  *   - Sizes: B holds 64*T words and I holds T+1 entries even when n % 4096 != 0; A (and Ao) must
@@ -75,6 +78,10 @@ const char *pici_strerror(int code);
  * may be NULL.  Host-only, no CUDA call. */
 int pici_sizes(uint64_t n, int dtype, uint64_t *bitvec_words, uint64_t *index_entries,
                uint64_t *values_capacity, uint64_t *workspace_bytes);
+
+/* Clears a workspace of ws_bytes bytes (one cudaMemsetAsync on `stream`).  Required once per
+ * allocation before the first pici_compress / pici_reduce_ss that uses it (see "ws" above). */
+int pici_workspace_init(void *ws, uint64_t ws_bytes, void *stream);
 
 /* a1-a3. Compress (Algorithm 1): dense[n] -> (B, I, A) in ONE pass over `dense`:
  * mask words + tile counts (Phase 1), device-wide exclusive scan of tile counts by decoupled

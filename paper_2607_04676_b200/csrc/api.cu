@@ -93,6 +93,13 @@ int pici_sizes(uint64_t n, int dtype, uint64_t *bitvec_words, uint64_t *index_en
     return PICI_OK;
 }
 
+int pici_workspace_init(void *ws, uint64_t ws_bytes, void *stream) {
+    if (ws == nullptr) return ws_bytes == 0 ? PICI_OK : PICI_ERR_INVALID_ARG;
+    if (!aligned(ws, 16)) return PICI_ERR_ALIGN;
+    if (ws_bytes == 0) return PICI_OK;
+    return cuda_rc(cudaMemsetAsync(ws, 0, ws_bytes, static_cast<cudaStream_t>(stream)));
+}
+
 int pici_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A, uint64_t A_capacity,
                   void *ws, uint64_t ws_bytes, void *stream) {
     return do_compress(dense, n, dtype, B, I, A, A_capacity, ws, ws_bytes, kOpen, stream);

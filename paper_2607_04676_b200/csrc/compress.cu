@@ -209,11 +209,10 @@ int num_sms() {
     return cached[dev];
 }
 
-// Scratch for the scans: compress uses one status word per tile; reduce_ss uses one word per span plus
-// its per-iteration and per-group accumulators (merge.cu), bounded by T + 4096 more words.
+// Scratch for the scans (layout: pici_common.cuh): header, reduce_ss's accumulators, one word per tile.
 uint64_t scan_workspace_bytes(uint64_t n) {
     const uint64_t T = (n + kTile - 1) / kTile;
-    return (uint64_t)kWsHeaderBytes + (2 * T + 4096) * 8;
+    return (uint64_t)kWsHeaderBytes + ((uint64_t)kWsAccWords + ((T + 65) & ~1ull)) * 8;   // multiple of 16
 }
 
 template <int DT>
@@ -229,13 +228,17 @@ static cudaError_t launch_compress_t(const void *dense, uint64_t n, uint64_t *B,
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    cudaError_t e = cudaMemsetAsync(ws, 0, (size_t)kWsHeaderBytes + T * 8, s);
+    // bytes [0, 64) of the workspace hold reduce_ss's persistent header (epoch, merge.cu): never cleared here
+    unsigned char *wsb = reinterpret_cast<unsigned char *>(ws);
+    uint64_t *status = reinterpret_cast<uint64_t *>(wsb + kWsHeaderBytes) + kWsAccWords;
+    cudaError_t e = cudaMemsetAsync(wsb + kWsCompressTicket, 0, kWsHeaderBytes - kWsCompressTicket, s);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(status, 0, T * 8, s);
     if (e != cudaSuccess) return e;
     uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
     const uint64_t cap = (uint64_t)num_sms() * Cfg::kMinBlocks;           // persistent: one resident wave
     if (blocks > cap) blocks = cap;
-    uint32_t *ticket = reinterpret_cast<uint32_t *>(ws);
-    uint64_t *status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);
+    uint32_t *ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + kWsCompressTicket);
     compress_kernel<DT><<<(unsigned)blocks, kCompressWarps * 32, smem, s>>>(dense, n, B, I, A, ticket, status,
                                                                           g.ptr, g.value);
     return cudaGetLastError();

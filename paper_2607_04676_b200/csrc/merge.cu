@@ -10,89 +10,117 @@
 // Because A is ordered tile -> column -> row and B[64t+c] is column c with bit r = row r, the words of
 // B read as ONE little-endian bit string ARE the order of A.  The merge therefore never needs a dense
 // position: it is a 1-D merge of two (bit string, value stream) pairs, and I[t] is the number of
-// survivors before bit 4096*t.  The kernel works on SPANS of that string:
-//   * a span is m = 16, 8, 4, 2 or 1 consecutive tiles, the same m for the whole launch: the largest
-//     whose AVERAGE contents fit one shared-memory stage and whose expected union of the two supports fits
-//     the output region (read on the device from Ix[T], Iy[T]), halved while the launch has fewer than
-//     two spans per CTA;
-//   * the launch is COOPERATIVE with G CTAs (two per SM, all co-resident); CTA c takes spans c, c + G,
-//     c + 2G, ...  A CTA is 16 WALKER warps plus one SERVICE warp per stage (576 threads).  The service
-//     warp of stage s starts the four 1-D TMA bulk copies of a span - its Bx / By words (contiguous) and
-//     its X / Y value runs (contiguous in Ax / Ay), one mbarrier - two spans ahead, index entries loaded
-//     one span before that, so the walkers find the stage filled when they get to it;
-//   * walkers: thread j owns the 8m-bit piece j of the span; x's and y's cursors come from the
-//     block-wide popc prefix of their own pieces, the candidate cursor from the popc prefix of the OR;
-//     every thread walks the set bits of its piece, adds, tests the predicate and packs its surviving
-//     sums into its own run of the stage's output region (runs start at the OR-prefix, so they never
-//     overlap); they publish the span's count and go on - they never wait for a look-back;
-//   * Phase 2 (exclusive scan of the counts) is the round-robin scan of pici_common.cuh:
-//     per-span / per-32-spans / per-iteration words, prefix = three independent loads (a flat decoupled
-//     look-back walks up to G/32 dependent hops here because the CTAs run in lock-step; a block-wide flat
-//     read hot-spots a few L2 lines - both measured).  The service warp takes the prefix once the count
-//     is out, writes the span's index entries and copies the output region to Ao (packed; if a
-//     cancellation left gaps, run by run from what the walkers recorded), then releases the region;
-//   * a span whose values do not fit the stage, or whose exact candidate count exceeds the output region
-//     (the span length is chosen from an estimate), is processed tile by tile in two sweeps (count, then
-//     emit) by the walkers themselves - one tile always fits.
-// The kernel is bound by the issue of its per-span bookkeeping, not by HBM (S5).
-#include <type_traits>
-
+// survivors before bit 4096*t.
+//
+// Structure (one persistent CTA per SM, NOT cooperative, no per-launch memset):
+//   * work is handed out in BLOCKS of m consecutive tiles (m = 32 ... 1, the same for the whole launch,
+//     chosen on the device from Ix[T] + Iy[T]) by a dynamic ticket; a block whose data does not fit the
+//     CTA's shared-memory rings is cut into sub-spans of whole tiles (one tile always fits), so there is
+//     no separate slow path: every sub-span is an ordinary item of the pipeline;
+//   * the PRODUCER warp takes tickets two blocks ahead, loads the blocks' index entries one block ahead,
+//     allocates an item's input bytes (its Bx / By words - contiguous - and its X / Y value runs -
+//     contiguous in Ax / Ay) in the INPUT ring and its worst-case output words in the OUTPUT ring, and
+//     starts the four 1-D TMA bulk copies on the item's `full` mbarrier;
+//   * 16 WORKER warps, each on its own: an item is cut into pieces of 32 * LB bits (LB = bits per lane,
+//     128 ... 8 with the density), piece p of the item goes to worker (base + p) mod 16.  A worker finds
+//     its x / y cursors by itself - I[t] of its tile plus the popcount of the tile's words before its
+//     piece (two REDUX) plus a warp scan of its own lanes - walks the set bits of x | y (add, re-test,
+//     pack into the tile's region of the output ring at the candidate prefix), writes its piece of Bo and
+//     leaves (start, survivors) of the piece in the item's descriptor.  No block-wide barrier or scan
+//     exists; a worker never waits for a look-back;
+//   * 4 FLUSHER warps (blocks are dealt to them round-robin): once an item's 16 workers have arrived on
+//     `done`, the flusher publishes the item's per-tile survivor counts, takes the exclusive prefix of
+//     the item's first tile (Phase 2, below), writes the item's index entries and copies
+//     the pieces' survivors from the output ring to Ao, then releases the output words (`flushed`).
+//     The input bytes are released as soon as the workers are done;
+//   * Phase 2, the device-wide exclusive scan of the tile counts, is a three-level STORE-ONLY hierarchy
+//     over tiles: one word per tile, one per group of 32 tiles, one per 1024 tiles, each (tag | value)
+//     in one 64-bit word where tag = launch epoch.  prefix(t0) = [1024-blocks below] + [groups below in
+//     the own block] + [tiles below in the own group]: independent loads, no chain of look-backs.  The
+//     flusher whose item ends a group has just read the group's other tiles for its own prefix, so it
+//     stores the group word for free (likewise the 1024-block word).  A prefix only ever waits for
+//     COUNTS of earlier tiles, which are published before their owners wait for anything, and earlier
+//     tiles belong to tickets taken earlier, i.e. to running CTAs: forward progress needs no
+//     co-residency;
+//   * the epoch lives in the workspace header and is advanced by the last flusher warp of the launch to
+//     finish, which also resets the ticket: stale words of earlier launches never match the tag, so
+//     nothing has to be cleared between launches (the workspace must have been zeroed ONCE,
+//     pici_workspace_init).
 #include "launch.h"
 #include "pici_common.cuh"
 #include "../../include/pici.h"
 
 namespace pici {
 
-#ifdef PICI_MERGE_TRACE   // debug only: per-CTA, per-iteration %globaltimer stamps
-__device__ uint64_t *g_merge_trace;
-#define PICI_TR(it, k)                                                                      \
-    do {                                                                                    \
-        if (threadIdx.x == 0 && (it) < 16u) {                                               \
-            uint64_t t_;                                                                    \
-            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                          \
-            g_merge_trace[((size_t)blockIdx.x * 16 + (it)) * 8 + (k)] = t_;                 \
-        }                                                                                   \
-    } while (0)
-#else
-#define PICI_TR(it, k) do { } while (0)
+#ifndef PICI_MERGE_CTAS
+#define PICI_MERGE_CTAS 1
 #endif
+constexpr int kCtasPerSm = PICI_MERGE_CTAS;
+constexpr int kWorkers = 16 / kCtasPerSm;                    // worker warps per CTA
+constexpr int kFlushers = 4 / kCtasPerSm;                    // flusher warps per CTA
+constexpr int kMergeThreads = 32 * (kWorkers + 2 + kFlushers);   // + the producer and the publisher warp
+constexpr int kDesc = 8;                                     // items in flight per CTA
+constexpr uint32_t kTileWords = 2 * kSide;                   // u32 words of B per tile
+constexpr uint32_t kMaxBlockTiles = 32;                      // m <= 32: one producer / flusher lane per tile
+constexpr uint32_t kEnd = 0xFFFFFFFFu;
+// One tile with every bit set in both operands: 2 x 128 words of B, 2 x 4096 values (+ window slack).
+constexpr uint32_t kMaxTileIn = 2 * kTileWords + 2 * kTile + 16;
+constexpr uint32_t kMaxTileOut = 2 * kTile + 4;        // candidates are bounded by |x| + |y| (cheap to prefix)
+constexpr uint32_t kPoolWords = kCtasPerSm == 2 ? 26624 : 55296;   // 104 KB (two CTAs per SM) or 216 KB of dynamic shared memory
+constexpr uint32_t kMinIn = kMaxTileIn, kMinOut = kMaxTileOut;   // one worst-case tile fits each ring
+constexpr uint32_t kDepth = 4;                               // an average block takes <= 1/kDepth of a ring
+static_assert(kMinIn + kMinOut <= kPoolWords, "pool too small for two full tiles in flight");
 
-constexpr int kMergeWarps = 16;
-constexpr int kMergeThreads = kMergeWarps * 32;
-constexpr int kMaxSpan = 16;                            // tiles per span: 16, 8, 4, 2 or 1
-constexpr uint32_t kTileWords = 2 * kSide;              // u32 words of B per tile
-// stage = [Bx words of the span][By words][X window][Y window]; one full tile always fits
-constexpr uint32_t kStageWords = 2 * kTileWords + 2 * kTile + 16;
-constexpr uint32_t kOutWords = kTile;                   // candidates (bits of x | y) of a span
-constexpr uint32_t kPoolWords = 2 * kStageWords + 2 * kOutWords;   // two stages, two output regions
-constexpr int kMergeMinBlocks = 2;
-constexpr uint32_t kMaxGrid = kRoundRobinMaxUnits;       // units per iteration the round-robin scan supports
-
-// What the staging warp tells the walkers about the span in a stage.
-struct SpanInfo {
-    uint32_t fits;      // 0: the span takes the slow path (nothing was copied)
-    uint32_t Xb, Yb;    // stage word of the first x / y value
-    uint32_t xs, ys;    // Ix[ts], Iy[ts]
+struct MergeHeader {          // first 64 bytes of the workspace; persistent across launches
+    uint32_t epoch;           // tag of the last finished launch
+    uint32_t ticket;          // next block
+    uint32_t finished;        // flusher warps that have left
 };
+
+struct ItemDesc {
+    uint32_t t0;                       // first tile, kEnd = no more items
+    uint32_t k;                        // tiles
+    uint32_t npieces;                  // k * (128 / LB)
+    uint32_t bx, by;                   // pool word of the item's Bx / By words
+    uint32_t flusher;                  // which flusher warp owns the item
+    uint32_t piece_base;               // pieces handed out before this item, mod kWorkers
+    uint32_t tile_x[kMaxBlockTiles];   // pool word of tile i's first x value
+    uint32_t tile_y[kMaxBlockTiles];
+    uint32_t tile_out[kMaxBlockTiles]; // pool word of tile i's output region
+    uint32_t piece_at[kMaxBlockTiles]; // workers: pool word of the piece's survivors, and how many
+    uint32_t piece_cnt[kMaxBlockTiles];
+};
+
+struct alignas(16) IndexSlot {  // index entries of one block, copied ahead by the producer (cp.async)
+    uint32_t ix[36], iy[36];                   // Ix[ts + i], Iy[ts + i], i = 0 .. tiles of the block (inclusive)
+    uint32_t g;                                // the block
+};
+
 struct MergeShared {
-    uint64_t full[2];         // mbarrier: the copies of the span in stage s have landed
-    uint64_t stage_free[2];   // mbarrier: the walkers are done with stage s
-    uint64_t counts[2];       // mbarrier: out region s, tcs[s], tot[s] are written, the count is published
-    uint64_t lb_done[2];      // mbarrier: excl[s] is written
-    uint64_t flushed[2];      // mbarrier: out region s has been written to Ao
-    uint64_t slow_bar;        // mbarrier: copies of the slow path
-    SpanInfo info[2];
-    uint32_t excl[2];                 // survivors before the span (from the look-back)
-    uint32_t tot[2], cand[2];         // survivors / candidates of the span; cand == ~0u: the walkers flush it
-    uint32_t tcs[2][kMaxSpan];        // per-tile survivors of the span
-    uint32_t wxy[kMergeWarps];        // per-warp totals: popc(x piece) | popc(y piece) << 16
-    uint32_t wu[kMergeWarps];         // per-warp totals: popc(x | y)
-    uint32_t ws[kMergeWarps];         // per-warp totals: survivors
-    uint16_t run_at[2][kMergeThreads];   // per-thread runs of a span that had cancellations: first word,
-    uint16_t run_k[2][kMergeThreads];    // survivors
+    uint64_t full[kDesc];      // mbarrier: the item's copies have landed, its descriptor is valid
+    uint64_t done[kDesc];      // mbarrier: all workers are through with the item
+    uint64_t flushed[kDesc];   // mbarrier: all flushers are through with the item
+    ItemDesc desc[kDesc];
+    uint32_t in_end[kDesc], out_end[kDesc];   // producer only: ring heads after the item's allocations
+    IndexSlot idx[4];
 };
-// Barrier of the 16 walker warps (the staging warp never joins it).
-__device__ __forceinline__ void walkers_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kMergeThreads) : "memory"); }
+
+struct MergeArgs {
+    const uint64_t *Bx, *By;
+    const uint32_t *Ix, *Iy, *Ax, *Ay;
+    uint64_t *Bo;
+    uint32_t *Io, *Ao;
+    MergeHeader *hdr;
+    uint64_t *blk_acc;     // [kWsBlkWords]  (tiles << 48) + survivors per 1024 tiles; zero between launches
+    uint64_t *grp_acc;     // [kWsGrpWords]  (tiles << 48) + survivors per 32 tiles;   zero between launches
+    uint64_t *tile_word;   // [T]            (tag << 32) | survivors of the tile
+    uint64_t tile_words;   // tagged words behind the accumulators (cleared when the epoch wraps)
+    uint32_t T;
+    uint32_t zero;         // 0, but only the host knows: keeps the ticket's address non-uniform for ptxas, which
+                           // otherwise makes the atomic warp-aggregated - with a shuffle that waits for its result
+    uint64_t a_limit;      // bytes of Ax / Ay that may be read: (n * 4) & ~15 (capacity >= n elements)
+};
+
 __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
     uint32_t ok;
     asm volatile(
@@ -102,29 +130,52 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0u;
 }
+// Wait with back-off: for the producer and the flushers, whose waits are long and must not take issue slots from
+// the workers (a bare try_wait loop re-issues every few cycles).
+__device__ __forceinline__ bool mbar_peek(uint32_t bar, uint32_t parity) {   // non-blocking
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0u;
+}
+__device__ __forceinline__ void mbar_wait_idle(uint32_t bar, uint32_t parity) {
+    unsigned ns = 32;
+    while (!mbar_peek(bar, parity)) {
+        __nanosleep(ns);
+        if (ns < 256) ns += ns;
+    }
+}
+__device__ __forceinline__ void ticket_if(bool take, uint32_t *ticket, uint32_t &t) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.u32 p, %1, 0;\n\t"
+        "@p atom.global.add.u32 %0, [%2], 1;\n\t}"
+        : "+r"(t) : "r"((uint32_t)take), "l"(ticket) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+__device__ __forceinline__ void cp_async_4(uint32_t dst, const void *src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
+// 16-byte copy of which only the first src_bytes are read (the rest is zero-filled)
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void *src, uint32_t src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ uint32_t popc4(uint4 v) { return __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w); }
 
-struct MergeArgs {
-    const uint64_t *Bx, *By;
-    const uint32_t *Ix, *Iy, *Ax, *Ay;
-    uint64_t *Bo;
-    uint32_t *Io, *Ao;
-    RoundRobinScan scan;   // per-span / per-group / per-iteration words (pici_common.cuh)
-    uint32_t T;
-    uint64_t a_limit;      // bytes of Ax / Ay that may be read: (n * 4) & ~15 (capacity >= n elements)
-};
-
-// ---- staging ------------------------------------------------------------------------------------
+// ---- value windows ------------------------------------------------------------------------------
 // The values A[beg .. beg+cnt) are copied as ONE bulk copy of the 16-byte aligned window around them
-// (up to 12 bytes before and after belong to neighbouring spans of the same buffer; the window never
+// (up to 12 bytes before and after belong to neighbouring items of the same buffer; the window never
 // passes a_limit, so nothing outside the caller's capacity is read).  Only a run that ends in the last
 // < 16 bytes of a completely full buffer keeps a tail, moved by plain loads.
 struct Window {
     uint64_t g_beg;    // byte offset in A of the window start
     uint32_t bulk;     // bytes of the bulk copy (multiple of 16, may be 0)
-    uint32_t words;    // window length in words, multiple of 4 (what the stage reserves)
+    uint32_t words;    // window length in words, multiple of 4 (what the ring reserves)
     uint32_t first;    // word index inside the window of element 0
     uint32_t tail_beg; // element index (relative to beg) where the plain-load tail starts; == cnt if none
 };
@@ -142,473 +193,731 @@ __device__ __forceinline__ Window window_of(uint32_t beg, uint32_t cnt, uint64_t
     return w;
 }
 
-// Layout of a span inside a stage (m tiles per span).
-struct SpanLayout {
-    uint32_t By0;      // word of the span's By words (Bx words start at 0)
-    uint32_t Xb, Yb;   // word of the first x / y value
-    uint32_t tx;       // bytes the bulk copies signal on the mbarrier
+// ---- rings (producer only; every lane computes the same) -------------------------------------------
+struct Ring {
+    uint32_t cap, head, tail, live;
 };
-__device__ __forceinline__ bool span_fits(uint32_t m, uint32_t nx, uint32_t ny, uint32_t mt) {
-    (void)mt;   // the output region is checked on the exact candidate count, after the popc scan (walk_span)
-    return 2u * m * kTileWords + nx + ny + 16u <= kStageWords;
-}
-
-// Warp 0: start the copies of the span of mt tiles at tile ts (m tiles per span) into `stage`; returns
-// its layout.  Other callers pass issue = false to get the layout only.
-__device__ __forceinline__ SpanLayout span_stage(const MergeArgs &a, uint32_t *stage, uint32_t bar, uint32_t ts, uint32_t m,
-                                                 uint32_t mt, uint32_t xs, uint32_t nx, uint32_t ys, uint32_t ny,
-                                                 bool issue, int lane) {
-    const Window wx = window_of(xs, nx, a.a_limit), wy = window_of(ys, ny, a.a_limit);
-    SpanLayout L;
-    L.By0 = m * kTileWords;
-    const uint32_t V = 2u * m * kTileWords;
-    L.Xb = V + wx.first;
-    L.Yb = V + wx.words + wy.first;
-    const uint32_t bbytes = mt * kTileWords * 4u;
-    L.tx = 2u * bbytes + wx.bulk + wy.bulk;
-    if (issue) {
-        // tail elements first (plain stores, < 4 per operand), so that lane 0's arrive on the mbarrier - the
-        // release the walkers' wait acquires - is ordered behind every lane's stores
-        if (wx.tail_beg + lane < nx) stage[L.Xb + wx.tail_beg + lane] = a.Ax[xs + wx.tail_beg + lane];
-        if (wy.tail_beg + lane < ny) stage[L.Yb + wy.tail_beg + lane] = a.Ay[ys + wy.tail_beg + lane];
-        __syncwarp();
-        if (lane == 0) {
-            fence_proxy_async_smem();
-            mbar_expect_tx(bar, L.tx);
-            bulk_g2s(smem_u32(stage), a.Bx + (size_t)ts * kSide, bbytes, bar);
-            bulk_g2s(smem_u32(stage + L.By0), a.By + (size_t)ts * kSide, bbytes, bar);
-            if (wx.bulk) bulk_g2s(smem_u32(stage + V), reinterpret_cast<const unsigned char *>(a.Ax) + wx.g_beg, wx.bulk, bar);
-            if (wy.bulk)
-                bulk_g2s(smem_u32(stage + V + wx.words), reinterpret_cast<const unsigned char *>(a.Ay) + wy.g_beg, wy.bulk, bar);
+__device__ __forceinline__ bool ring_alloc(Ring &r, uint32_t n, uint32_t &at) {
+    if (r.live == 0) r.head = r.tail = 0;
+    if (r.live != 0 && r.head == r.tail) return false;   // full
+    if (r.head >= r.tail) {                              // free: [head, cap) and [0, tail)
+        if (r.cap - r.head >= n) {
+            at = r.head;
+            r.head += n;
+            if (r.head == r.cap) r.head = 0;
+        } else if (r.tail >= n) {                        // skip the rest of the buffer
+            at = 0;
+            r.head = n;
+        } else {
+            return false;
         }
+    } else {                                             // free: [head, tail)
+        if (r.tail - r.head < n) return false;
+        at = r.head;
+        r.head += n;
     }
-    return L;
+    ++r.live;
+    return true;
 }
 
-// This thread's 8*m-bit piece of the staged Bx / By words.  Pieces past the span's last tile are 0.
-__device__ __forceinline__ void read_piece(const uint32_t *stage, uint32_t By0, uint32_t m, uint32_t mt, int tid,
-                                           uint32_t (&ax)[4], uint32_t (&ay)[4]) {
-    ax[0] = ax[1] = ax[2] = ax[3] = 0u;
-    ay[0] = ay[1] = ay[2] = ay[3] = 0u;
-    if ((uint32_t)tid * m >= (uint32_t)kMergeThreads * mt) return;
-    const uint32_t *bx = stage, *by = stage + By0;
-    if (m == 16) {
-        const uint4 p = reinterpret_cast<const uint4 *>(bx)[tid], q = reinterpret_cast<const uint4 *>(by)[tid];
-        ax[0] = p.x; ax[1] = p.y; ax[2] = p.z; ax[3] = p.w;
-        ay[0] = q.x; ay[1] = q.y; ay[2] = q.z; ay[3] = q.w;
-    } else if (m == 8) {
-        const uint2 p = reinterpret_cast<const uint2 *>(bx)[tid], q = reinterpret_cast<const uint2 *>(by)[tid];
-        ax[0] = p.x; ax[1] = p.y;
-        ay[0] = q.x; ay[1] = q.y;
-    } else if (m == 4) {
-        ax[0] = bx[tid];
-        ay[0] = by[tid];
-    } else if (m == 2) {
-        ax[0] = reinterpret_cast<const uint16_t *>(bx)[tid];
-        ay[0] = reinterpret_cast<const uint16_t *>(by)[tid];
-    } else {
-        ax[0] = reinterpret_cast<const uint8_t *>(bx)[tid];
-        ay[0] = reinterpret_cast<const uint8_t *>(by)[tid];
-    }
-}
-__device__ __forceinline__ void store_piece(const MergeArgs &a, uint32_t ts, uint32_t m, uint32_t mt, int tid,
-                                            const uint32_t (&ao)[4]) {
-    if ((uint32_t)tid * m >= (uint32_t)kMergeThreads * mt) return;
-    const size_t wbase = (size_t)ts * kSide;
-    if (m == 16) reinterpret_cast<uint4 *>(a.Bo + wbase)[tid] = make_uint4(ao[0], ao[1], ao[2], ao[3]);
-    else if (m == 8) reinterpret_cast<uint2 *>(a.Bo + wbase)[tid] = make_uint2(ao[0], ao[1]);
-    else if (m == 4) reinterpret_cast<uint32_t *>(a.Bo + wbase)[tid] = ao[0];
-    else if (m == 2) reinterpret_cast<uint16_t *>(a.Bo + wbase)[tid] = (uint16_t)ao[0];
-    else reinterpret_cast<uint8_t *>(a.Bo + wbase)[tid] = (uint8_t)ao[0];
-}
-
-// What a thread keeps from one walk of a span.
-struct WalkOut {
-    uint32_t k;            // this thread's survivors
-    uint32_t ko0;          // word of this thread's run in the output region
-    uint32_t sk;           // inclusive warp scan of k
-    uint32_t cand_total;   // candidates (bits of x | y) in the span
+// ---- launch-wide geometry, computed identically by every thread ---------------------------------------
+struct Geometry {
+    uint32_t m;          // tiles per block
+    uint32_t lb;         // bits per lane of a piece: 128, 64, 32, 16 or 8
+    uint32_t in_cap, out_cap;
+    uint32_t blocks;
 };
+__device__ __forceinline__ Geometry geometry(const MergeArgs &a, uint32_t G) {
+    Geometry g;
+    const uint32_t T = a.T;
+    const uint64_t nx = __ldg(a.Ix + T), ny = __ldg(a.Iy + T);
+    const uint64_t avg = (nx + ny + T - 1) / T;                     // values per tile, X and Y together
+    const uint64_t in_tile = 2 * kTileWords + avg + 8;
+    const uint64_t out_tile = avg + 4;
+    // output words live two to three times as long as input words (publish + prefix + flush against load + merge)
+    uint64_t oc = (uint64_t)kPoolWords * 2 * out_tile / (in_tile + 2 * out_tile);
+    oc = max(oc, (uint64_t)kMinOut);
+    oc = min(oc, (uint64_t)(kPoolWords - kMinIn));
+    g.out_cap = (uint32_t)oc & ~3u;
+    g.in_cap = kPoolWords - g.out_cap;
+    uint32_t m = 1;
+#pragma unroll
+    for (uint32_t mm = kMaxBlockTiles; mm >= 2; mm /= 2)
+        if (m == 1 && mm * in_tile <= g.in_cap / kDepth && mm * out_tile <= g.out_cap / kDepth) m = mm;
+    while (m > 1 && (T + m - 1) / m < 2u * G) m /= 2;               // small inputs: keep every CTA busy
+    g.m = m;
+    g.lb = min(16u * m, 128u);
+    g.blocks = (T + m - 1) / m;
+    return g;
+}
 
-// Read this thread's piece of the staged span, block-wide popc prefixes, then the walk of the piece's
-// set bits: add, re-test, pack.  The caller has waited for the span's copies.  With EMIT the surviving
-// sums go to `out` and ao[] receives the piece of Bo; without it the survivors are only counted.
-// Contains two walkers_sync(); on return sh.ws[] holds the per-warp survivor totals and nobody reads
-// the stage any more.
-template <bool EMIT>
-__device__ __forceinline__ WalkOut walk_span(const uint32_t *stage, uint32_t *out, MergeShared &sh, uint32_t By0, uint32_t Xb,
-                                             uint32_t Yb, uint32_t m, uint32_t mt, uint32_t (&ao)[4], int tid,
-                                             uint16_t *run_at = nullptr, uint16_t *run_k = nullptr, uint32_t trace_it = 99u) {
-    const int lane = tid & 31, warp = tid >> 5;
-    uint32_t ax[4], ay[4];
-    read_piece(stage, By0, m, mt, tid, ax, ay);
-    const uint32_t cx = __popc(ax[0]) + __popc(ax[1]) + __popc(ax[2]) + __popc(ax[3]);
-    const uint32_t cy = __popc(ay[0]) + __popc(ay[1]) + __popc(ay[2]) + __popc(ay[3]);
-    const uint32_t cu = __popc(ax[0] | ay[0]) + __popc(ax[1] | ay[1]) + __popc(ax[2] | ay[2]) + __popc(ax[3] | ay[3]);
-    const uint32_t sxy = warp_incl_scan(cx | (cy << 16), lane);
-    const uint32_t su = warp_incl_scan(cu, lane);
-    if (lane == 31) {
-        sh.wxy[warp] = sxy;
-        sh.wu[warp] = su;
-    }
-    walkers_sync();  // #1: warp totals are visible
-    PICI_TR(trace_it, 2);
-    // prefix over the 16 warp totals: lanes 0..15 of every warp scan them with shuffles (an unrolled loop over
-    // the 16 shared-memory words costs ~80 instructions per thread; the kernel is issue-bound on exactly this
-    // kind of per-span bookkeeping: 60 % issue activity with almost no values to add at 99.99 % sparsity)
-    uint32_t pw = lane < kMergeWarps ? sh.wxy[lane] : 0u, uw = lane < kMergeWarps ? sh.wu[lane] : 0u;
-#pragma unroll
-    for (int d = 1; d < kMergeWarps; d <<= 1) {
-        const uint32_t o1 = __shfl_up_sync(kFull, pw, d), o2 = __shfl_up_sync(kFull, uw, d);
-        if (lane >= d) {
-            pw += o1;
-            uw += o2;
-        }
-    }
-    const uint32_t cand_total = __shfl_sync(kFull, uw, kMergeWarps - 1);
-    const uint32_t bxy = warp > 0 ? __shfl_sync(kFull, pw, (warp + 31) & 31) : 0u;   // inclusive prefix of warp - 1
-    const uint32_t bu = warp > 0 ? __shfl_sync(kFull, uw, (warp + 31) & 31) : 0u;
-    if (EMIT && cand_total > kOutWords) {   // uniform: more candidates than the output region holds
-        WalkOut none = {0u, 0u, 0u, cand_total};
-        return none;                        // the caller takes the tile-by-tile path (only one barrier passed)
-    }
-    uint32_t kx = Xb + (bxy & 0xFFFFu) + (sxy & 0xFFFFu) - cx;
-    uint32_t ky = Yb + (bxy >> 16) + (sxy >> 16) - cy;
-    const uint32_t ko0 = bu + su - cu;
-    uint32_t ko = ko0;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        uint32_t u = ax[q] | ay[q], o = 0;
-        while (u) {
-            const uint32_t bit = u & (0u - u);
-            u ^= bit;
-            float x = 0.0f, y = 0.0f;
-            if (ax[q] & bit) x = __uint_as_float(stage[kx++]);
-            if (ay[q] & bit) y = __uint_as_float(stage[ky++]);
-            const uint32_t sum = __float_as_uint(__fadd_rn(x, y));   // received + local (C9 #7)
-            if (nz32(sum)) {
-                o |= bit;
-                if (EMIT) out[ko] = sum;
-                ++ko;
+// =========================================== producer ===========================================
+__device__ __forceinline__ void producer(const MergeArgs &a, MergeShared &sh, uint32_t *pool, const Geometry &geo,
+                                         uint32_t tk0, int lane) {
+    const uint32_t T = a.T, m = geo.m, ppt = 128u / geo.lb;
+    const uint32_t full0 = smem_u32(&sh.full[0]), done0 = smem_u32(&sh.done[0]), fl0 = smem_u32(&sh.flushed[0]);
+    Ring rin = {geo.in_cap, 0, 0, 0}, rout = {geo.out_cap, 0, 0, 0};
+    const uint32_t in_limit = max(geo.in_cap / 2, kMaxTileIn), out_limit = max(geo.out_cap / 2, kMaxTileOut);
+    uint32_t j = 0;                 // items emitted
+    uint32_t in_tail = 0, out_tail = 0;   // oldest item whose input / output words are still allocated
+    uint32_t blk_seq = 0, piece_base = 0;
+
+    auto free_in = [&]() {          // wait for the oldest item's workers, release its input words
+        const uint32_t d = in_tail % kDesc;
+        mbar_wait_idle(done0 + 8 * d, (in_tail / kDesc) & 1u);
+        rin.tail = sh.in_end[d];
+        --rin.live;
+        ++in_tail;
+    };
+    auto free_out = [&]() {
+        const uint32_t d = out_tail % kDesc;
+        mbar_wait_idle(fl0 + 8 * d, (out_tail / kDesc) & 1u);
+        rout.tail = sh.out_end[d];
+        --rout.live;
+        ++out_tail;
+    };
+    // ---- block pipeline --------------------------------------------------------------------------------------
+    // A ticket costs an L2 round trip and so does a block's index entries, each about as long as the CTA has for a
+    // whole block in the sparse regime, so both run well ahead of the block in hand (n): tickets are requested
+    // five blocks ahead (two atomics in flight, all by lane 0, hence increasing), index entries are copied to
+    // shared memory by cp.async three blocks ahead (slot n & 3).
+    const bool wide = m >= 4u && ((reinterpret_cast<uintptr_t>(a.Ix) | reinterpret_cast<uintptr_t>(a.Iy)) & 15u) == 0u;
+    auto issue_index = [&](uint32_t slot, uint32_t g) {
+        IndexSlot &S = sh.idx[slot];
+        if (g < geo.blocks) {
+            const uint32_t ts = g * m;
+            if (wide) {          // ts * 4 bytes is 16-byte aligned: entries ts + 4c .. ts + 4c + 3 as one 16-byte copy
+                const uint32_t e0 = ts + 4u * (uint32_t)lane;          // lanes 0 .. m/4 (the last one: the end entry)
+                if (4u * (uint32_t)lane <= m && e0 <= T) {
+                    const uint32_t bytes = min(4u, T + 1u - e0) * 4u;  // never read past I[T]
+                    cp_async_16(smem_u32(&S.ix[4 * lane]), a.Ix + e0, bytes);
+                    cp_async_16(smem_u32(&S.iy[4 * lane]), a.Iy + e0, bytes);
+                }
+            } else if ((uint32_t)lane <= m && ts + (uint32_t)lane <= T) {
+                cp_async_4(smem_u32(&S.ix[lane]), a.Ix + ts + lane);
+                cp_async_4(smem_u32(&S.iy[lane]), a.Iy + ts + lane);
             }
         }
-        ao[q] = o;
-    }
-    WalkOut r;
-    r.k = ko - ko0;
-    r.ko0 = ko0;
-    r.sk = warp_incl_scan(r.k, lane);
-    r.cand_total = cand_total;
-    if (lane == 31) sh.ws[warp] = r.sk;
-    if (run_at != nullptr) {   // where this thread's survivors sit: only read if the span had a cancellation
-        run_at[tid] = (uint16_t)ko0;
-        run_k[tid] = (uint16_t)r.k;
-    }
-    walkers_sync();  // #2: survivor totals and the output region are visible; the stage is no longer read
-    PICI_TR(trace_it, 4);
-    return r;
-}
-
-// ---- Phase 2: counts -> exclusive prefix: the round-robin scan of pici_common.cuh ----------------------
-__device__ __forceinline__ void publish_span(const MergeArgs &a, uint32_t g, uint32_t it, uint32_t c, uint32_t total) {
-    rr_publish(a.scan, g, it, c, total);
-}
-__device__ __forceinline__ uint32_t iter_lookback(const MergeArgs &a, uint32_t G, uint32_t it, uint32_t c, uint32_t &E,
-                                                  uint32_t &E_it, int lane) {
-    return rr_lookback(a.scan, G, it, c, E, E_it, lane);
-}
-
-// Io for the mt tiles of a span (one warp; lane i < mt holds tc = survivors of tile ts + i).
-__device__ __forceinline__ void write_index(const MergeArgs &a, uint32_t ts, uint32_t mt, uint32_t tc, uint32_t excl, int lane) {
-    const uint32_t tincl = warp_incl_scan((uint32_t)lane < mt ? tc : 0u, lane);
-    if ((uint32_t)lane < mt) {
-        a.Io[ts + lane] = excl + tincl - tc;
-        if (ts + lane + 1 == a.T) a.Io[a.T] = excl + tincl;
-    }
-}
-
-// One warp writes a walked span's output region to Ao + off.  Packed (no cancellation): the region is
-// contiguous.  Otherwise the walkers left their runs (first word, survivors) in shared memory: lane l
-// moves the runs of threads 32q + l, q = 0..15, offsets from a running warp scan.
-__device__ __forceinline__ void warp_flush(uint32_t *__restrict__ Ao, const uint32_t *out, uint32_t off, uint32_t surv_total,
-                                           uint32_t cand_total, const uint16_t *run_at, const uint16_t *run_k, int lane) {
-    uint32_t *dst = Ao + off;
-    if (surv_total == cand_total) {
-        for (uint32_t i = lane; i < surv_total; i += 32) dst[i] = out[i];
-        return;
-    }
-    uint32_t base = 0;
-    for (int q = 0; q < kMergeWarps; ++q) {
-        const uint32_t k = run_k[32 * q + lane], at = run_at[32 * q + lane];
-        const uint32_t incl = warp_incl_scan(k, lane);
-        for (uint32_t i = 0; i < k; ++i) dst[base + incl - k + i] = out[at + i];
-        base += __shfl_sync(kFull, incl, 31);
-    }
-}
-
-// Write a walked span's output region to Ao + off.  Packed (no cancellation happened): the region is
-// contiguous; otherwise every thread moves its own run (before = survivors of earlier threads).
-__device__ __forceinline__ void span_flush(uint32_t *__restrict__ Ao, const uint32_t *out, const WalkOut &r, uint32_t off,
-                                           uint32_t surv_total, uint32_t before, int tid) {
-    uint32_t *dst = Ao + off;
-    if (surv_total == r.cand_total) {
-        for (uint32_t i = tid; i < surv_total; i += kMergeThreads) dst[i] = out[i];
+        if (lane == 0) S.g = g;
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    uint32_t n = 0;                 // block in hand (counted per CTA)
+    bool dry = false;               // a ticket beyond the last block has been seen: request no more
+    // Start-up: every ticket is requested only after the one before it has returned, so the CTAs' first tickets
+    // interleave (CTA c holds blocks ~c, ~G + c, ~2G + c, ...) instead of forming runs of consecutive blocks - a
+    // CTA that holds a run and cannot allocate its last block yet would hold up everyone behind it.
+    // How far ahead: blocks of a few dense tiles last long enough for one block of lead; in the sparse regime a
+    // block lasts about one memory round trip and the lead is three.  (More lead than needed means tickets held
+    // long before their tiles are merged, i.e. more skew between CTAs and longer waits for prefixes.)
+    const uint32_t lead = m <= 4u ? 1u : 3u;
+    uint32_t tkA = kEnd, tkB = kEnd;  // in flight: tickets of blocks n + lead (A on even n, B on odd n) and n + lead + 1
+    if (lead == 3u) {
+        auto next = [&](uint32_t prev) -> uint32_t {
+            uint32_t t = kEnd;
+            if (prev < geo.blocks && lane == 0) t = atomicAdd(&a.hdr->ticket, 1u);
+            return __shfl_sync(kFull, t, 0);
+        };
+        const uint32_t g0 = __shfl_sync(kFull, tk0, 0);
+        issue_index(0, g0);
+        const uint32_t g1 = next(g0);
+        issue_index(1, g1);
+        const uint32_t g2 = next(g1);
+        issue_index(2, g2);
+        tkA = next(g2);
+        dry = tkA >= geo.blocks;
+        if (!dry && lane == 0) tkB = atomicAdd(&a.hdr->ticket, 1u);
     } else {
-        for (uint32_t i = 0; i < r.k; ++i) dst[before + i] = out[r.ko0 + i];
+        const uint32_t g0 = __shfl_sync(kFull, tk0, 0);
+        issue_index(0, g0);
+        dry = g0 >= geo.blocks;
+        ticket_if(!dry && lane == 0, &a.hdr->ticket + (uint32_t)lane * a.zero, tkA);
+    }
+    // one block; tk is the register (tkA on even n, tkB on odd n: the loop is unrolled by two so that reading one
+    // in-flight ticket never waits for the other)
+    auto step = [&](uint32_t &tk) -> bool {
+        // the ticket of block n + 3 has had two blocks' time to return; its index entries start moving now
+        const uint32_t g3 = __shfl_sync(kFull, tk, 0);
+        if (g3 >= geo.blocks) dry = true;
+        // block n + 5's ticket; a predicated atomic, so that nothing reads the register before it is needed two
+        // blocks from now (a select between the atomic's result and kEnd would wait for the round trip here)
+        tk = kEnd;
+        ticket_if(!dry && lane == 0, &a.hdr->ticket + (uint32_t)lane * a.zero, tk);
+        issue_index((n + lead) & 3u, g3);
+        if (lead == 3u) asm volatile("cp.async.wait_group 3;" ::: "memory");   // block n's entries have landed
+        else asm volatile("cp.async.wait_group 1;" ::: "memory");
+        const IndexSlot &S = sh.idx[n & 3u];
+        __syncwarp();
+        const uint32_t g_cur = S.g;
+        if (g_cur >= geo.blocks) return false;
+        const uint32_t ts = g_cur * m, mt = min(m, T - ts);
+        const uint32_t l0 = min((uint32_t)lane, mt), l1 = min((uint32_t)lane + 1u, mt);
+        const uint32_t cx0 = S.ix[l0], cx1 = S.ix[l1], cy0 = S.iy[l0], cy1 = S.iy[l1];
+        ++n;
+        {
+        uint32_t i0 = 0;
+        while (i0 < mt) {
+            // ---- the longest run of tiles [i0, i1) whose data fits half of each ring; a tile's output region
+            // holds |x| + |y| words (its candidates cannot be more) ------------------------------------------------
+            const uint32_t xs = S.ix[i0], ys = S.iy[i0];
+            const uint32_t vals = (cx1 - xs) + (cy1 - ys);          // values of tiles i0 .. lane
+            const uint32_t need_in = 2u * kTileWords * ((uint32_t)lane - i0 + 1u) + vals + 16u;
+            const bool in_range = (uint32_t)lane >= i0 && (uint32_t)lane < mt;
+            const bool fits = need_in <= in_limit && vals + 4u <= out_limit;
+            const unsigned bad = __ballot_sync(kFull, in_range && !fits);
+            uint32_t i1 = bad ? (uint32_t)__ffs(bad) - 1u : mt;
+            if (i1 <= i0) i1 = i0 + 1;                      // one tile always fits (kMinIn, kMinOut)
+            const uint32_t k = i1 - i0;
+            const uint32_t xe = S.ix[i1], ye = S.iy[i1];
+            const uint32_t nx = xe - xs, ny = ye - ys;
+            const Window wx = window_of(xs, nx, a.a_limit), wy = window_of(ys, ny, a.a_limit);
+            const uint32_t in_words = 2u * kTileWords * k + wx.words + wy.words;
+            const uint32_t out_words = max((nx + ny + 3u) & ~3u, 4u);
+
+            // ---- descriptor slot and ring space -----------------------------------------------------------
+            const uint32_t d = j % kDesc;
+            while (out_tail + kDesc <= j) free_out();       // item j - kDesc has left slot d
+            while (in_tail + kDesc <= j) free_in();
+            uint32_t ib = 0, ob = 0;
+            while (!ring_alloc(rin, in_words, ib)) free_in();
+            while (!ring_alloc(rout, out_words, ob)) free_out();
+            ob += geo.in_cap;
+            ItemDesc &D = sh.desc[d];
+            const uint32_t V = ib + 2u * kTileWords * k;
+            const uint32_t Xb = V + wx.first, Yb = V + wx.words + wy.first;
+            if ((uint32_t)lane >= i0 && (uint32_t)lane < i1) {
+                const uint32_t i = (uint32_t)lane - i0;
+                D.tile_x[i] = Xb + (cx0 - xs);
+                D.tile_y[i] = Yb + (cy0 - ys);
+                D.tile_out[i] = ob + (cx0 - xs) + (cy0 - ys);
+            }
+            if (lane == 0) {
+                D.t0 = ts + i0;
+                D.k = k;
+                D.npieces = k * ppt;
+                D.bx = ib;
+                D.by = ib + kTileWords * k;
+                D.flusher = blk_seq % kFlushers;
+                D.piece_base = piece_base;
+                sh.in_end[d] = rin.head;
+                sh.out_end[d] = rout.head;
+            }
+            // tail elements (plain stores, < 4 per operand) before lane 0's arrive, which releases them
+            if (wx.tail_beg + lane < nx) pool[Xb + wx.tail_beg + lane] = a.Ax[xs + wx.tail_beg + lane];
+            if (wy.tail_beg + lane < ny) pool[Yb + wy.tail_beg + lane] = a.Ay[ys + wy.tail_beg + lane];
+            __syncwarp();
+            if (lane == 0) {
+                const uint32_t bar = full0 + 8 * d;
+                const uint32_t bbytes = k * kTileWords * 4u;
+                mbar_expect_tx(bar, 2u * bbytes + wx.bulk + wy.bulk);
+                bulk_g2s(smem_u32(pool + ib), a.Bx + (size_t)(ts + i0) * kSide, bbytes, bar);
+                bulk_g2s(smem_u32(pool + ib + kTileWords * k), a.By + (size_t)(ts + i0) * kSide, bbytes, bar);
+                if (wx.bulk) bulk_g2s(smem_u32(pool + V), reinterpret_cast<const unsigned char *>(a.Ax) + wx.g_beg, wx.bulk, bar);
+                if (wy.bulk)
+                    bulk_g2s(smem_u32(pool + V + wx.words), reinterpret_cast<const unsigned char *>(a.Ay) + wy.g_beg, wy.bulk, bar);
+            }
+            piece_base = (piece_base + k * ppt) % kWorkers;
+            ++j;
+            i0 = i1;
+        }
+        }
+        ++blk_seq;
+        return true;
+    };
+    if (lead == 3u) {
+        while (step(tkA) && step(tkB)) {
+        }
+    } else {
+        while (step(tkA)) {
+        }
+    }
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    // every ticket this warp requested must have returned before the item that ends the CTA is emitted (the
+    // launch's last flusher resets the ticket): both registers are read here
+    if (lane == 0 && (tkA & tkB) == 0x12345678u) sh.in_end[0] = 0;   // never true: tickets are < 2^31 or kEnd
+    const uint32_t d = j % kDesc;
+    while (out_tail + kDesc <= j) free_out();
+    while (in_tail + kDesc <= j) free_in();
+    if (lane == 0) {
+        sh.desc[d].t0 = kEnd;
+        mbar_arrive(full0 + 8 * d);
     }
 }
 
-// Survivors of earlier warps / of the whole block, from sh.ws[] (after walk_span's last barrier).
-__device__ __forceinline__ void survivor_sums(const MergeShared &sh, int warp, uint32_t &before, uint32_t &total) {
-    before = 0;
-    total = 0;
+// Two independent chains of the walk over the set bits of (wxA | wyA) and of (wxB | wyB): per candidate add
+// (received + local, C9 #7), re-test, store.  Cursors are shared-memory BYTE addresses.  Chain B's output cursor
+// starts at the CANDIDATE count of chain A, so the lane's survivors are contiguous only if nothing cancelled; the
+// caller checks survivors == candidates and redoes the piece with walk_packed otherwise.  A chain whose bits run
+// out idles (bit = 0: nothing loaded, sum = +0, nothing stored).  Hand-scheduled: 17 instructions per chain step.
+__device__ __forceinline__ void walk2(uint32_t wxA, uint32_t wyA, uint32_t wxB, uint32_t wyB, uint32_t &xaA, uint32_t &yaA,
+                                      uint32_t &oaA, uint32_t &xaB, uint32_t &yaB, uint32_t &oaB, uint32_t &oA,
+                                      uint32_t &oB) {
+    uint32_t uA = wxA | wyA, uB = wxB | wyB;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred pxA, pyA, psA, pxB, pyB, psB, pl;\n\t"
+        ".reg .b32 bA, bB, t, vxA, vyA, vxB, vyB, sA, sB;\n\t"
+        "or.b32 t, %0, %1;\n\t"
+        "setp.eq.u32 pl, t, 0;\n\t"
+        "@pl bra DONE_%=;\n\t"
+        "LOOP_%=:\n\t"
+        "neg.s32 bA, %0;\n\t"
+        "neg.s32 bB, %1;\n\t"
+        "and.b32 bA, bA, %0;\n\t"
+        "and.b32 bB, bB, %1;\n\t"
+        "xor.b32 %0, %0, bA;\n\t"
+        "xor.b32 %1, %1, bB;\n\t"
+        "and.b32 t, %10, bA;\n\t"
+        "setp.ne.u32 pxA, t, 0;\n\t"
+        "and.b32 t, %11, bA;\n\t"
+        "setp.ne.u32 pyA, t, 0;\n\t"
+        "and.b32 t, %12, bB;\n\t"
+        "setp.ne.u32 pxB, t, 0;\n\t"
+        "and.b32 t, %13, bB;\n\t"
+        "setp.ne.u32 pyB, t, 0;\n\t"
+        "mov.b32 vxA, 0;\n\t"
+        "mov.b32 vyA, 0;\n\t"
+        "mov.b32 vxB, 0;\n\t"
+        "mov.b32 vyB, 0;\n\t"
+        "@pxA ld.shared.b32 vxA, [%2];\n\t"
+        "@pyA ld.shared.b32 vyA, [%3];\n\t"
+        "@pxB ld.shared.b32 vxB, [%5];\n\t"
+        "@pyB ld.shared.b32 vyB, [%6];\n\t"
+        "@pxA add.u32 %2, %2, 4;\n\t"
+        "@pyA add.u32 %3, %3, 4;\n\t"
+        "@pxB add.u32 %5, %5, 4;\n\t"
+        "@pyB add.u32 %6, %6, 4;\n\t"
+        "add.rn.f32 sA, vxA, vyA;\n\t"
+        "add.rn.f32 sB, vxB, vyB;\n\t"
+        "and.b32 t, sA, 0x7fffffff;\n\t"
+        "setp.ne.u32 psA, t, 0;\n\t"
+        "and.b32 t, sB, 0x7fffffff;\n\t"
+        "setp.ne.u32 psB, t, 0;\n\t"
+        "@psA st.shared.b32 [%4], sA;\n\t"
+        "@psB st.shared.b32 [%7], sB;\n\t"
+        "@psA add.u32 %4, %4, 4;\n\t"
+        "@psB add.u32 %7, %7, 4;\n\t"
+        "@psA or.b32 %8, %8, bA;\n\t"
+        "@psB or.b32 %9, %9, bB;\n\t"
+        "or.b32 t, %0, %1;\n\t"
+        "setp.ne.u32 pl, t, 0;\n\t"
+        "@pl bra LOOP_%=;\n\t"
+        "DONE_%=:\n\t"
+        "}"
+        : "+r"(uA), "+r"(uB), "+r"(xaA), "+r"(yaA), "+r"(oaA), "+r"(xaB), "+r"(yaB), "+r"(oaB), "+r"(oA), "+r"(oB)
+        : "r"(wxA), "r"(wyA), "r"(wxB), "r"(wyB)
+        : "memory");
+}
+
+// ============================================ workers ============================================
+// One piece (32 * LB bits) of tile i of the item: cursors, walk, Bo, (start, survivors) of the piece.
+template <int LB>
+__device__ __forceinline__ void do_piece(const MergeArgs &a, uint32_t *pool, ItemDesc &D, uint32_t p, int lane) {
+    constexpr uint32_t PPT = 128 / LB;                       // pieces per tile
+    constexpr int NW = LB >= 32 ? LB / 32 : 1;               // 32-bit words per lane
+    const uint32_t i = p / PPT, sub = p % PPT;
+    const uint32_t *bx = pool + D.bx + i * kTileWords, *by = pool + D.by + i * kTileWords;
+    uint32_t kx = D.tile_x[i], ky = D.tile_y[i], ko = D.tile_out[i];
+    uint32_t ax[NW], ay[NW];
+    const uint32_t s0 = sub * LB;                            // first word of the piece inside the tile
+    if constexpr (LB == 128) {
+        const uint4 X = reinterpret_cast<const uint4 *>(bx)[lane], Y = reinterpret_cast<const uint4 *>(by)[lane];
+        ax[0] = X.x; ax[1] = X.y; ax[2] = X.z; ax[3] = X.w;
+        ay[0] = Y.x; ay[1] = Y.y; ay[2] = Y.z; ay[3] = Y.w;
+    } else {
+        if (sub != 0) {   // values / candidates of the tile before this piece
+            const uint4 X = reinterpret_cast<const uint4 *>(bx)[lane], Y = reinterpret_cast<const uint4 *>(by)[lane];
+            uint32_t pxy = 0, pu = 0;
+            if (4u * (uint32_t)lane < s0) {
+                pxy = popc4(X) | (popc4(Y) << 16);
+                pu = popc4(make_uint4(X.x | Y.x, X.y | Y.y, X.z | Y.z, X.w | Y.w));
+            }
+            pxy = __reduce_add_sync(kFull, pxy);
+            pu = __reduce_add_sync(kFull, pu);
+            kx += pxy & 0xFFFFu;
+            ky += pxy >> 16;
+            ko += pu;
+        }
+        if constexpr (LB == 64) {
+            const uint2 X = reinterpret_cast<const uint2 *>(bx + s0)[lane], Y = reinterpret_cast<const uint2 *>(by + s0)[lane];
+            ax[0] = X.x; ax[1] = X.y;
+            ay[0] = Y.x; ay[1] = Y.y;
+        } else if constexpr (LB == 32) {
+            ax[0] = bx[s0 + lane];
+            ay[0] = by[s0 + lane];
+        } else if constexpr (LB == 16) {
+            ax[0] = reinterpret_cast<const uint16_t *>(bx + s0)[lane];
+            ay[0] = reinterpret_cast<const uint16_t *>(by + s0)[lane];
+        } else {
+            ax[0] = reinterpret_cast<const uint8_t *>(bx + s0)[lane];
+            ay[0] = reinterpret_cast<const uint8_t *>(by + s0)[lane];
+        }
+    }
+    uint32_t cx = 0, cy = 0, cu = 0;
 #pragma unroll
-    for (int q = 0; q < kMergeWarps; ++q) {
-        const uint32_t v = sh.ws[q];
-        if (q < warp) before += v;
-        total += v;
+    for (int q = 0; q < NW; ++q) {
+        cx += __popc(ax[q]);
+        cy += __popc(ay[q]);
+        cu += __popc(ax[q] | ay[q]);
+    }
+    uint32_t ao[NW];
+    uint32_t ktot = 0;
+    const uint32_t piece_at = ko;
+    if (__any_sync(kFull, cu != 0u)) {
+        uint32_t ex, ey, eu;                                 // exclusive prefixes over the lanes
+        if constexpr (LB <= 16) {                            // totals <= 512: one packed scan
+            const uint32_t v = cx | (cy << 10) | (cu << 20);
+            const uint32_t s = warp_incl_scan(v, lane) - v;
+            ex = s & 1023u; ey = (s >> 10) & 1023u; eu = s >> 20;
+        } else {
+            const uint32_t v = cx | (cy << 16);
+            const uint32_t s = warp_incl_scan(v, lane) - v;
+            ex = s & 0xFFFFu; ey = s >> 16;
+            eu = warp_incl_scan(cu, lane) - cu;
+        }
+        kx += ex;
+        ky += ey;
+        const uint32_t ko0 = ko + eu;
+        // ---- fast walk: two chains per lane (the halves of a word, or two words) -----------------------------
+        const uint32_t sbase = smem_u32(pool);
+        uint32_t xa = sbase + 4u * kx, ya = sbase + 4u * ky, oa = sbase + 4u * ko0;
+        uint32_t surv = 0;
+        if constexpr (NW == 1) {
+            constexpr uint32_t kLo = (1u << (LB >= 32 ? 16 : LB / 2)) - 1u;
+            const uint32_t xlo = ax[0] & kLo, ylo = ay[0] & kLo, xhi = ax[0] & ~kLo, yhi = ay[0] & ~kLo;
+            uint32_t xb = xa + 4u * __popc(xlo), yb = ya + 4u * __popc(ylo), ob = oa + 4u * __popc(xlo | ylo);
+            const uint32_t oa0 = oa, ob0 = ob;
+            uint32_t oA = 0, oB = 0;
+            walk2(xlo, ylo, xhi, yhi, xa, ya, oa, xb, yb, ob, oA, oB);
+            ao[0] = oA | oB;
+            surv = ((oa - oa0) + (ob - ob0)) >> 2;
+        } else {
+#pragma unroll
+            for (int q = 0; q < NW; q += 2) {
+                uint32_t xb = xa + 4u * __popc(ax[q]), yb = ya + 4u * __popc(ay[q]), ob = oa + 4u * __popc(ax[q] | ay[q]);
+                const uint32_t oa0 = oa, ob0 = ob;
+                uint32_t oA = 0, oB = 0;
+                walk2(ax[q], ay[q], ax[q + 1], ay[q + 1], xa, ya, oa, xb, yb, ob, oA, oB);
+                ao[q] = oA;
+                ao[q + 1] = oB;
+                surv += ((oa - oa0) + (ob - ob0)) >> 2;
+                xa = xb; ya = yb; oa = ob;
+            }
+        }
+        ktot = __reduce_add_sync(kFull, surv);
+        if (__any_sync(kFull, surv != cu)) {
+            // ---- an exact cancellation: redo the piece with one packed run per lane, then close the gaps
+            // between the lanes' runs, lane by lane (dst <= src) ------------------------------------------------
+            __syncwarp();
+            const uint32_t *__restrict__ xp = pool + kx;
+            const uint32_t *__restrict__ yp = pool + ky;
+            uint32_t *__restrict__ op = pool + ko0;
+#pragma unroll
+            for (int q = 0; q < NW; ++q) {
+                uint32_t u = ax[q] | ay[q], o = 0;
+                const uint32_t wx = ax[q], wy = ay[q];
+                while (u) {
+                    const uint32_t bit = u & (0u - u);
+                    u ^= bit;
+                    const bool hx = (wx & bit) != 0u, hy = (wy & bit) != 0u;
+                    const float x = hx ? __uint_as_float(*xp) : 0.0f;
+                    const float y = hy ? __uint_as_float(*yp) : 0.0f;
+                    xp += hx ? 1 : 0;
+                    yp += hy ? 1 : 0;
+                    const uint32_t sum = __float_as_uint(__fadd_rn(x, y));
+                    if (nz32(sum)) {
+                        o |= bit;
+                        *op++ = sum;
+                    }
+                }
+                ao[q] = o;
+            }
+            const uint32_t kmine = (uint32_t)(op - pool) - ko0;
+            const uint32_t ek = warp_incl_scan(kmine, lane) - kmine;
+            __syncwarp();
+            for (int l = 0; l < 32; ++l) {
+                const uint32_t src = __shfl_sync(kFull, ko0, l), cnt = __shfl_sync(kFull, kmine, l);
+                const uint32_t dst = ko + __shfl_sync(kFull, ek, l);
+                if (src == dst) continue;
+                for (uint32_t b = 0; b < cnt; b += 32) {
+                    uint32_t v = 0;
+                    if (b + lane < cnt) v = pool[src + b + lane];
+                    __syncwarp();
+                    if (b + lane < cnt) pool[dst + b + lane] = v;
+                    __syncwarp();
+                }
+            }
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < NW; ++q) ao[q] = 0u;
+    }
+    // ---- this piece of Bo ------------------------------------------------------------------------------
+    uint32_t *bo = reinterpret_cast<uint32_t *>(a.Bo) + (size_t)(D.t0 + i) * kTileWords + s0;
+    if constexpr (LB == 128) reinterpret_cast<uint4 *>(bo)[lane] = make_uint4(ao[0], ao[1], ao[2], ao[3]);
+    else if constexpr (LB == 64) reinterpret_cast<uint2 *>(bo)[lane] = make_uint2(ao[0], ao[1]);
+    else if constexpr (LB == 32) bo[lane] = ao[0];
+    else if constexpr (LB == 16) reinterpret_cast<uint16_t *>(bo)[lane] = (uint16_t)ao[0];
+    else reinterpret_cast<uint8_t *>(bo)[lane] = (uint8_t)ao[0];
+    if (lane == 0) {
+        D.piece_at[p] = piece_at;
+        D.piece_cnt[p] = ktot;
     }
 }
 
-// One tile (a span of m = 1) end to end, copies included (walker warp 0 issues them on slow_bar): the
-// slow path of a span that does not fit.  Starts with a walkers_sync() (the stage may still be read).
-template <bool EMIT>
-__device__ __forceinline__ WalkOut tile_pass(const MergeArgs &a, uint32_t *stage, uint32_t *out, MergeShared &sh,
-                                             uint32_t t, uint32_t x0, uint32_t x1, uint32_t y0, uint32_t y1, uint32_t bar,
-                                             uint32_t &parity, int tid) {
-    walkers_sync();
-    const SpanLayout L = span_stage(a, stage, bar, t, 1u, 1u, x0, x1 - x0, y0, y1 - y0, tid < 32, tid & 31);
-    mbar_wait(bar, parity);
-    parity ^= 1u;
-    uint32_t ao[4];
-    const WalkOut r = walk_span<EMIT>(stage, out, sh, L.By0, L.Xb, L.Yb, 1u, 1u, ao, tid);
-    if (EMIT) store_piece(a, t, 1u, 1u, tid, ao);
-    return r;
+template <int LB>
+__device__ __forceinline__ void worker(const MergeArgs &a, MergeShared &sh, uint32_t *pool, int w, int lane) {
+    const uint32_t full0 = smem_u32(&sh.full[0]), done0 = smem_u32(&sh.done[0]);
+    for (uint32_t j = 0;; ++j) {
+        const uint32_t d = j % kDesc, ph = (j / kDesc) & 1u;
+        mbar_wait(full0 + 8 * d, ph);
+        ItemDesc &D = sh.desc[d];
+        if (D.t0 == kEnd) break;
+        const uint32_t np = D.npieces;
+        for (uint32_t p = ((uint32_t)w + kWorkers - D.piece_base) % kWorkers; p < np; p += kWorkers)
+            do_piece<LB>(a, pool, D, p, lane);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(done0 + 8 * d);
+    }
 }
 
+__device__ __forceinline__ bool tagged(uint64_t v, uint32_t tag) { return (uint32_t)(v >> 32) == tag; }
 
-constexpr int kMergeLaunchThreads = kMergeThreads + 64;   // 16 walker warps + one service warp per stage
+// ============================================ publisher ===========================================
+// Phase 2 input.  One warp that does nothing but make counts visible: as soon as an item's workers are done it
+// stores the item's per-tile survivor counts (tagged words) and adds (tiles, survivors) to the accumulators of
+// the item's group of 32 tiles and of its block of 1024 tiles.  It waits for nothing else - in particular never
+// for a prefix - so every count of the launch becomes visible a fixed latency after its tile was merged, and a
+// prefix, which only reads counts, can never be part of a chain of waits.
+__device__ __forceinline__ void publisher(const MergeArgs &a, MergeShared &sh, const Geometry &geo, uint32_t tag, int lane) {
+    const uint32_t full0 = smem_u32(&sh.full[0]), done0 = smem_u32(&sh.done[0]), fl0 = smem_u32(&sh.flushed[0]);
+    const uint32_t ppt = 128u / geo.lb;
+    for (uint32_t j = 0;; ++j) {
+        const uint32_t d = j % kDesc, ph = (j / kDesc) & 1u;
+        mbar_wait_idle(full0 + 8 * d, ph);
+        const ItemDesc &D = sh.desc[d];
+        const uint32_t t0 = D.t0;
+        if (t0 == kEnd) break;
+        const uint32_t k = D.k, np = D.npieces;
+        mbar_wait_idle(done0 + 8 * d, ph);
+        const uint32_t cnt = (uint32_t)lane < np ? D.piece_cnt[lane] : 0u;
+        const uint32_t incl = warp_incl_scan(cnt, lane);
+        const uint32_t total = __shfl_sync(kFull, incl, 31);
+        const uint32_t lo = __shfl_sync(kFull, incl - cnt, ((uint32_t)lane * ppt) & 31u);
+        const uint32_t hi = __shfl_sync(kFull, incl, ((uint32_t)lane * ppt + ppt - 1u) & 31u);
+        if ((uint32_t)lane < k) st_status(a.tile_word + t0 + lane, tag, hi - lo);
+        if (lane == 0) {
+            const uint64_t v = ((uint64_t)k << 48) + total;
+            red_add_u64(a.grp_acc + (t0 >> 5), v);
+            red_add_u64(a.blk_acc + (t0 >> 10), v);
+            mbar_arrive(fl0 + 8 * d);
+        }
+    }
+}
 
-__global__ void __launch_bounds__(kMergeLaunchThreads, kMergeMinBlocks)
+// ============================================ flushers ============================================
+// Exclusive prefix of tile t0 = survivors of all tiles below it (one warp): complete 1024-tile blocks below
+// (carried in E / E_blk from call to call) + complete groups of 32 below inside the own block + tiles below inside
+// the own group.  Three independent sets of loads; each word says by itself whether it is complete.
+__device__ __forceinline__ uint32_t tile_prefix(const MergeArgs &a, uint32_t tag, uint32_t t0, uint32_t &E,
+                                                uint32_t &E_blk, int lane) {
+    const uint32_t u = t0 & 31u, grp = (t0 >> 5) & 31u, blk = t0 >> 10, gbase = t0 & ~31u;
+    uint64_t va, vg, vb = 0;
+    unsigned ns = 8;
+    for (;;) {
+        va = (uint32_t)lane < u ? ld_status(a.tile_word + gbase + lane) : ((uint64_t)tag << 32);
+        vg = (uint32_t)lane < grp ? ld_status(a.grp_acc + blk * 32u + lane) : (32ull << 48);
+        const bool more = E_blk + (uint32_t)lane < blk;
+        vb = more ? ld_status(a.blk_acc + E_blk + lane) : (1024ull << 48);
+        if (__all_sync(kFull, tagged(va, tag) && (vg >> 48) == 32u && (vb >> 48) == 1024u)) break;
+        __nanosleep(ns);
+        if (ns < 128) ns += ns;
+    }
+    const uint32_t nb = min(32u, blk - E_blk);
+    E += __reduce_add_sync(kFull, (uint32_t)lane < nb ? (uint32_t)vb : 0u);
+    E_blk += nb;
+    while (E_blk < blk) {   // more than 32 new blocks since this warp's last prefix (first call on a huge input)
+        const uint32_t c = min(32u, blk - E_blk);
+        uint64_t v;
+        for (;;) {
+            v = (uint32_t)lane < c ? ld_status(a.blk_acc + E_blk + lane) : (1024ull << 48);
+            if (__all_sync(kFull, (v >> 48) == 1024u)) break;
+            __nanosleep(64);
+        }
+        E += __reduce_add_sync(kFull, (uint32_t)lane < c ? (uint32_t)v : 0u);
+        E_blk += c;
+    }
+    return E + __reduce_add_sync(kFull, (uint32_t)va + (uint32_t)vg);
+}
+
+// One warp copies cnt words from shared memory (word index src in pool) to global memory dst (4-byte aligned, any
+// 16-byte phase): a few single words up to the first 16-byte boundary of dst, then aligned 16-byte stores whose
+// four words come from two aligned 16-byte shared-memory reads (the phase difference is a whole number of words,
+// so realigning is a choice of registers, not a shift), then the last < 4 words.
+template <int K>
+__device__ __forceinline__ uint4 pick4(uint4 lo, uint4 hi) {   // words K .. K+3 of (lo.x lo.y lo.z lo.w hi.x hi.y hi.z hi.w)
+    if constexpr (K == 0) return lo;
+    else if constexpr (K == 1) return make_uint4(lo.y, lo.z, lo.w, hi.x);
+    else if constexpr (K == 2) return make_uint4(lo.z, lo.w, hi.x, hi.y);
+    else return make_uint4(lo.w, hi.x, hi.y, hi.z);
+}
+template <int K>
+__device__ __forceinline__ void copy_body(const uint32_t *pool, uint32_t src, uint4 *dst4, uint32_t nvec, int lane) {
+    const uint4 *s4 = reinterpret_cast<const uint4 *>(pool + (src - K));   // 16-byte aligned by construction
+    uint32_t i = lane;
+    for (; i + 32u < nvec; i += 64u) {     // two stores in flight per lane
+        const uint4 a0 = s4[i], a1 = K ? s4[i + 1] : a0, b0 = s4[i + 32], b1 = K ? s4[i + 33] : b0;
+        dst4[i] = pick4<K>(a0, a1);
+        dst4[i + 32] = pick4<K>(b0, b1);
+    }
+    if (i < nvec) {
+        const uint4 a0 = s4[i], a1 = K ? s4[i + 1] : a0;
+        dst4[i] = pick4<K>(a0, a1);
+    }
+}
+__device__ __forceinline__ void copy_run(const uint32_t *pool, uint32_t src, uint32_t *dst, uint32_t cnt, int lane) {
+    const uint32_t head = min((uint32_t)((16u - ((uint32_t)reinterpret_cast<uintptr_t>(dst) & 15u)) & 15u) >> 2, cnt);
+    if ((uint32_t)lane < head) dst[lane] = pool[src + lane];
+    const uint32_t nvec = (cnt - head) >> 2, body = nvec << 2;
+    const uint32_t s = src + head;
+    uint4 *d4 = reinterpret_cast<uint4 *>(dst + head);
+    switch (s & 3u) {
+        case 0: copy_body<0>(pool, s, d4, nvec, lane); break;
+        case 1: copy_body<1>(pool, s, d4, nvec, lane); break;
+        case 2: copy_body<2>(pool, s, d4, nvec, lane); break;
+        default: copy_body<3>(pool, s, d4, nvec, lane); break;
+    }
+    const uint32_t tail = cnt - head - body;
+    if ((uint32_t)lane < tail) dst[head + body + lane] = pool[s + body + lane];
+}
+
+__device__ __forceinline__ void flusher(const MergeArgs &a, MergeShared &sh, const uint32_t *pool, const Geometry &geo,
+                                        uint32_t tag, int f, int lane) {
+    const uint32_t full0 = smem_u32(&sh.full[0]), done0 = smem_u32(&sh.done[0]), fl0 = smem_u32(&sh.flushed[0]);
+    const uint32_t ppt = 128u / geo.lb;
+    uint32_t E = 0, E_blk = 0;
+    for (uint32_t j = 0;; ++j) {
+        const uint32_t d = j % kDesc, ph = (j / kDesc) & 1u;
+        mbar_wait_idle(full0 + 8 * d, ph);
+        const ItemDesc &D = sh.desc[d];
+        const uint32_t t0 = D.t0;
+        if (t0 == kEnd) break;
+        if (D.flusher == (uint32_t)f) {
+            const uint32_t k = D.k, np = D.npieces;
+            mbar_wait_idle(done0 + 8 * d, ph);
+            const uint32_t at = (uint32_t)lane < np ? D.piece_at[lane] : 0u;
+            const uint32_t cnt = (uint32_t)lane < np ? D.piece_cnt[lane] : 0u;
+            const uint32_t incl = warp_incl_scan(cnt, lane);
+            const uint32_t total = __shfl_sync(kFull, incl, 31);
+            const uint32_t lo = __shfl_sync(kFull, incl - cnt, ((uint32_t)lane * ppt) & 31u);   // lane i: before tile i
+            const uint32_t base = tile_prefix(a, tag, t0, E, E_blk, lane);
+            if ((uint32_t)lane < k) {
+                a.Io[t0 + lane] = base + lo;
+                if (t0 + lane + 1u == a.T) a.Io[a.T] = base + total;
+            }
+            // ---- the pieces' survivors -> Ao ----------------------------------------------------------------
+            const uint32_t dst = base + incl - cnt;
+            const uint32_t maxc = __reduce_max_sync(kFull, cnt);
+            if (maxc <= 8u) {               // a few values per piece: lane p moves piece p
+                for (uint32_t e = 0; e < cnt; ++e) a.Ao[dst + e] = pool[at + e];
+            } else if (total >= 256u * k) {
+                // long runs.  The pieces of a tile are contiguous in the output ring unless a cancellation left a gap:
+                // then a tile is ONE run (lane i < k: tile i), else every piece is its own run.
+                const uint32_t at_prev = __shfl_up_sync(kFull, at, 1), cnt_prev = __shfl_up_sync(kFull, cnt, 1);
+                const bool joint = (uint32_t)lane >= np || ((uint32_t)lane & (ppt - 1u)) == 0u || at == at_prev + cnt_prev;
+                const bool by_tile = __all_sync(kFull, joint);
+                const uint32_t nruns = by_tile ? k : np;
+                const uint32_t hi = __shfl_sync(kFull, incl, ((uint32_t)lane * ppt + ppt - 1u) & 31u);
+                const uint32_t r_at = by_tile ? __shfl_sync(kFull, at, ((uint32_t)lane * ppt) & 31u) : at;
+                const uint32_t r_cnt = by_tile ? hi - lo : cnt;
+                const uint32_t r_dst = by_tile ? base + lo : dst;
+                for (uint32_t r = 0; r < nruns; ++r)
+                    copy_run(pool, __shfl_sync(kFull, r_at, r), a.Ao + __shfl_sync(kFull, r_dst, r),
+                             __shfl_sync(kFull, r_cnt, r), lane);
+            } else {
+                // four pieces at a time: four independent shared -> global chains per lane
+                for (uint32_t p = 0; p < np; p += 4) {
+                    uint32_t s4[4], c4[4], o4[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        s4[q] = __shfl_sync(kFull, at, (p + q) & 31u);
+                        c4[q] = p + q < np ? __shfl_sync(kFull, cnt, (p + q) & 31u) : 0u;
+                        o4[q] = __shfl_sync(kFull, dst, (p + q) & 31u);
+                    }
+                    const uint32_t cmax = max(max(c4[0], c4[1]), max(c4[2], c4[3]));
+                    for (uint32_t e = lane; e < cmax; e += 32u) {
+                        uint32_t v[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) v[q] = e < c4[q] ? pool[s4[q] + e] : 0u;
+#pragma unroll
+                        for (int q = 0; q < 4; ++q)
+                            if (e < c4[q]) a.Ao[o4[q] + e] = v[q];
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(fl0 + 8 * d);
+    }
+    // ---- the last flusher warp of the launch clears the accumulators, resets the ticket, advances the epoch ----
+    uint32_t last = 0;
+    if (lane == 0) {
+        __threadfence();
+        last = atomicAdd(&a.hdr->finished, 1u) + 1u == gridDim.x * (uint32_t)kFlushers;
+    }
+    if (__shfl_sync(kFull, last, 0)) {
+        uint32_t e = tag & 0x7FFFFFFFu;
+        const uint32_t ngrp = (a.T + 31u) / 32u, nblk = (a.T + 1023u) / 1024u;
+        for (uint32_t q = lane; q < ngrp; q += 32) a.grp_acc[q] = 0;
+        for (uint32_t q = lane; q < nblk; q += 32) a.blk_acc[q] = 0;
+        if (e == 0x7FFFFFFFu) {   // the 31-bit epoch wraps: forget every tagged word (once per 2^31 launches)
+            for (uint64_t q = lane; q < a.tile_words; q += 32) a.tile_word[q] = 0;
+            e = 0;
+        }
+        __syncwarp();
+        if (lane == 0) {
+            a.hdr->ticket = 0;
+            a.hdr->finished = 0;
+            __threadfence();
+            a.hdr->epoch = e;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kMergeThreads, kCtasPerSm)
 reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     extern __shared__ __align__(128) uint32_t pool[];
     __shared__ MergeShared sh;
     if (gate_closed(gate, gate_value)) return;
 
-    const int tid = threadIdx.x;
-    const int lane = tid & 31;
-    const int warp = tid >> 5;
-    const uint32_t T = a.T;
-    const uint32_t G = gridDim.x;
-
-    // ---- span length of this launch: the largest m whose AVERAGE span (plus 1/16 margin) fits a stage
-    // and the output region, from the totals Ix[T], Iy[T]; halved while the launch has fewer than two
-    // spans per CTA (ring chunks are a few thousand tiles).
-    uint32_t m = 1;
-    {
-        const uint64_t nx = __ldg(a.Ix + T), ny = __ldg(a.Iy + T);
-        const uint64_t avg = (nx + ny + T - 1) / T;   // values per tile, X and Y together
-        // candidates per tile: the union of two INDEPENDENT supports of these densities (a span whose
-        // union is larger than the output region takes the slow path, so this is an estimate, not a bound)
-        const uint64_t both = (nx / T) * (ny / T) / kTile;
-        const uint64_t uni = min(avg - min(both, avg), (uint64_t)kTile);
-#pragma unroll
-        for (uint32_t mm = kMaxSpan; mm >= 2; mm /= 2) {
-            const uint64_t vals = avg * mm + 16, cand = uni * mm;
-            if (m == 1 && 2u * mm * kTileWords + vals + vals / 16 <= kStageWords && cand + cand / 16 <= kOutWords) m = mm;
-        }
-        while (m > 1 && (T + m - 1) / m < 2u * G) m /= 2;
-    }
-    const uint32_t spans = (T + m - 1) / m;
-    uint32_t *const out = pool + 2 * kStageWords;
-    const uint32_t full0 = smem_u32(&sh.full[0]), free0 = smem_u32(&sh.stage_free[0]);
-    const uint32_t cnt0 = smem_u32(&sh.counts[0]), lbd0 = smem_u32(&sh.lb_done[0]), fl0 = smem_u32(&sh.flushed[0]);
-    const uint32_t slow_bar = smem_u32(&sh.slow_bar);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // tag of this launch: epoch + 1 with the top bit set (compress's status flags 1 / 2 never have it)
+    const uint32_t tag = ((*reinterpret_cast<const volatile uint32_t *>(&a.hdr->epoch) + 1u) & 0x7FFFFFFFu) | 0x80000000u;
+    // the producer's first ticket is requested before anything else: it returns while the geometry loads do
+    uint32_t tk0 = 0;
+    if (warp == kWorkers && lane == 0) tk0 = atomicAdd(&a.hdr->ticket, 1u);
+    const Geometry geo = geometry(a, gridDim.x);
     if (tid == 0) {
-#pragma unroll
-        for (uint32_t s = 0; s < 2; ++s) {
-            mbar_init(full0 + 8 * s, 1);
-            mbar_init(free0 + 8 * s, 1);
-            mbar_init(cnt0 + 8 * s, 1);
-            mbar_init(lbd0 + 8 * s, 1);
-            mbar_init(fl0 + 8 * s, 1);
+        for (int d = 0; d < kDesc; ++d) {
+            mbar_init(smem_u32(&sh.full[d]), 1);
+            mbar_init(smem_u32(&sh.done[d]), kWorkers);
+            mbar_init(smem_u32(&sh.flushed[d]), kFlushers + 1);
         }
-        mbar_init(slow_bar, 1);
     }
     __syncthreads();
-    // Spans are dealt round-robin: CTA c takes spans c, c + G, c + 2G, ...; j counts this CTA's spans,
-    // span j lives in stage / output region s = j & 1.  The launch is cooperative (all G CTAs are
-    // co-resident), so every span a look-back waits on belongs to a running CTA, and span j of a CTA
-    // only depends on spans <= j of the others.
-    const uint32_t c = blockIdx.x;
 
-    if (warp >= kMergeWarps) {
-        // ============================ service warp of stage s ============================
-        // For this CTA's spans j = s, s + 2, ...: start the copies of span j (stage s is free once the
-        // walkers have left span j - 2); once span j's count is published take its prefix, write its
-        // index entries, write its output region to Ao and release the region.  The walkers never wait
-        // for a look-back: they only need stage s filled and region s released two spans later.
-        const uint32_t s = (uint32_t)warp - kMergeWarps;
-        uint32_t *const stage = pool + s * kStageWords;
-        const uint32_t *const out_s = out + s * kOutWords;
-        auto load_index = [&](uint32_t gg, uint32_t &ixl, uint32_t &iyl) {   // lanes 0..mt hold I[ts .. ts+mt]
-            ixl = 0;
-            iyl = 0;
-            if (gg < spans) {
-                const uint32_t ts = gg * m, jj = min((uint32_t)lane, min(m, T - ts));
-                ixl = __ldg(a.Ix + ts + jj);
-                iyl = __ldg(a.Iy + ts + jj);
-            }
-        };
-        auto prepare = [&](uint32_t gg, uint32_t ixl, uint32_t iyl) {
-            if (gg >= spans) return;
-            const uint32_t ts = gg * m, mt = min(m, T - ts);
-            const uint32_t xs = __shfl_sync(kFull, ixl, 0), xe = __shfl_sync(kFull, ixl, mt);
-            const uint32_t ys = __shfl_sync(kFull, iyl, 0), ye = __shfl_sync(kFull, iyl, mt);
-            const bool fits = span_fits(m, xe - xs, ye - ys, mt);
-            const SpanLayout L = span_stage(a, stage, full0 + 8 * s, ts, m, mt, xs, xe - xs, ys, ye - ys, false, lane);
-            if (lane == 0) {
-                sh.info[s].fits = fits ? 1u : 0u;
-                sh.info[s].Xb = L.Xb;
-                sh.info[s].Yb = L.Yb;
-                sh.info[s].xs = xs;
-                sh.info[s].ys = ys;
-            }
-            __syncwarp();
-            if (fits) span_stage(a, stage, full0 + 8 * s, ts, m, mt, xs, xe - xs, ys, ye - ys, true, lane);
-            else if (lane == 0) mbar_arrive(full0 + 8 * s);   // nothing to copy: the walkers stage tile by tile
-        };
-        uint32_t ixa, iya;
-        load_index(c + s * G, ixa, iya);
-        prepare(c + s * G, ixa, iya);
-        load_index(c + (s + 2) * G, ixa, iya);   // entries of the next span to prepare, one ahead
-        uint32_t E = 0, E_it = 0;                // survivors of the complete iterations [0, E_it)
-        for (uint32_t j = s; c + j * G < spans; j += 2) {
-            const uint32_t ph = (j >> 1) & 1u;
-            const uint32_t ts = (c + j * G) * m, mt = min(m, T - ts);
-            // Copies first when the stage is already free (they are what the walkers wait for two spans
-            // later); a span on the slow path frees its stage only after its look-back, so poll both.
-            bool prepared = false;
-            for (;;) {
-                if (!prepared && mbar_test(free0 + 8 * s, ph)) {
-                    prepare(c + (j + 2) * G, ixa, iya);
-                    load_index(c + (j + 4) * G, ixa, iya);
-                    prepared = true;
-                }
-                if (mbar_test(cnt0 + 8 * s, ph)) break;
-            }
-            const uint32_t excl = iter_lookback(a, G, j, c, E, E_it, lane);
-            write_index(a, ts, mt, (uint32_t)lane < mt ? sh.tcs[s][lane] : 0u, excl, lane);
-            const uint32_t tot = sh.tot[s], cand = sh.cand[s];
-            if (lane == 0) {
-                sh.excl[s] = excl;
-                mbar_arrive(lbd0 + 8 * s);
-            }
-            if (!prepared) {
-                mbar_wait(free0 + 8 * s, ph);
-                prepare(c + (j + 2) * G, ixa, iya);
-                load_index(c + (j + 4) * G, ixa, iya);
-            }
-            if (cand != ~0u) warp_flush(a.Ao, out_s, excl, tot, cand, sh.run_at[s], sh.run_k[s], lane);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(fl0 + 8 * s);
+    if (warp < kWorkers) {
+        switch (geo.lb) {
+            case 128: worker<128>(a, sh, pool, warp, lane); break;
+            case 64: worker<64>(a, sh, pool, warp, lane); break;
+            case 32: worker<32>(a, sh, pool, warp, lane); break;
+            default: worker<16>(a, sh, pool, warp, lane); break;
         }
-        return;
-    }
-
-    // ======================================= walker warps =======================================
-    // The loop is instantiated once per span length, so the piece width, the tile / warp ratio and the empty
-    // words of narrow pieces are compile-time facts (the kernel is bound by exactly these instructions).
-    uint32_t slow_par = 0;
-    auto walkers = [&](auto span_len) {
-        constexpr uint32_t M = decltype(span_len)::value;
-        for (uint32_t j = 0; c + j * G < spans; ++j) {
-            const uint32_t s = j & 1u, ph = (j >> 1) & 1u;
-            const uint32_t g = c + j * G, ts = g * M, mt = min(M, T - ts);
-            uint32_t *const stage = pool + s * kStageWords;
-            uint32_t *const out_s = out + s * kOutWords;
-            PICI_TR(j, 0);
-            // span j - 2 must have left output region s before anything is written to it; warp 0 waits for all (the
-            // first write comes behind the walkers' barrier #1, which warp 0 joins afterwards): 15 warps fewer polling
-            if (j >= 2 && warp == 0) mbar_wait(fl0 + 8 * s, ph ^ 1u);
-            mbar_wait(full0 + 8 * s, ph);
-            PICI_TR(j, 1);
-            const SpanInfo info = sh.info[s];
-
-            bool slow = info.fits == 0u;
-            if (!slow) {
-                // ---- walk, publish the count; the service warp of stage s does the rest ---------------------
-                uint32_t ao[4];
-                const WalkOut r = walk_span<true>(stage, out_s, sh, M * kTileWords, info.Xb, info.Yb, M, mt, ao, tid,
-                                                  sh.run_at[s], sh.run_k[s], j);
-                slow = r.cand_total > kOutWords;   // uniform; nothing was written
-                if (!slow) {
-                    if (warp == 0) {   // the other 15 warps go straight on to their piece of Bo and the next span
-                        const uint32_t surv_total = warp_sum(lane < kMergeWarps ? sh.ws[lane] : 0u);
-                        const uint32_t wpt = (uint32_t)kMergeWarps / M;   // a tile is covered by 16/m consecutive warps
-                        uint32_t tc = 0;
-                        if ((uint32_t)lane < mt)
-                            for (uint32_t q = 0; q < wpt; ++q) tc += sh.ws[lane * wpt + q];
-                        if (lane < kMaxSpan) sh.tcs[s][lane] = tc;
-                        if (lane == 0) {
-                            sh.tot[s] = surv_total;
-                            sh.cand[s] = r.cand_total;
-                            publish_span(a, g, j, c, surv_total);
-                            mbar_arrive(free0 + 8 * s);           // every walker is past barrier #2
-                        }
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(cnt0 + 8 * s);
-                    }
-                    store_piece(a, ts, M, mt, tid, ao);
-                    PICI_TR(j, 6);
-                }
-            }
-            if (slow) {
-                // ---- the span does not fit: tile by tile (one tile always fits), two sweeps -----------------
-                // Sweep 1 counts the survivors of every tile so that the span's count is published before
-                // anything waits (no other CTA ever waits on a half-processed span); sweep 2 emits and the
-                // walkers write Ao themselves (cand = ~0 tells the service warp not to).
-                for (uint32_t i = 0; i < mt; ++i) {
-                    const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
-                    const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
-                    tile_pass<false>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, slow_bar, slow_par, tid);
-                    if (tid == 0) {
-                        uint32_t cnt = 0;
-                        for (int q = 0; q < kMergeWarps; ++q) cnt += sh.ws[q];
-                        sh.tcs[s][i] = cnt;
-                    }
-                }
-                walkers_sync();
-                if (tid == 0) {
-                    uint32_t span_total = 0;
-                    for (uint32_t i = 0; i < mt; ++i) span_total += sh.tcs[s][i];
-                    sh.tot[s] = span_total;
-                    sh.cand[s] = ~0u;
-                    publish_span(a, g, j, c, span_total);
-                    mbar_arrive(cnt0 + 8 * s);
-                }
-                mbar_wait(lbd0 + 8 * s, ph);
-                uint32_t off = sh.excl[s];
-                for (uint32_t i = 0; i < mt; ++i) {
-                    const uint32_t x0 = __ldg(a.Ix + ts + i), x1 = __ldg(a.Ix + ts + i + 1);
-                    const uint32_t y0 = __ldg(a.Iy + ts + i), y1 = __ldg(a.Iy + ts + i + 1);
-                    const WalkOut r = tile_pass<true>(a, stage, out_s, sh, ts + i, x0, x1, y0, y1, slow_bar, slow_par, tid);
-                    uint32_t before, surv_total;
-                    survivor_sums(sh, warp, before, surv_total);
-                    span_flush(a.Ao, out_s, r, off, surv_total, before + r.sk - r.k, tid);
-                    off += surv_total;
-                }
-                walkers_sync();
-                if (tid == 0) mbar_arrive(free0 + 8 * s);
-            }
-        }
-    };
-    switch (m) {
-        case 16: walkers(std::integral_constant<uint32_t, 16>{}); break;
-        case 8: walkers(std::integral_constant<uint32_t, 8>{}); break;
-        case 4: walkers(std::integral_constant<uint32_t, 4>{}); break;
-        case 2: walkers(std::integral_constant<uint32_t, 2>{}); break;
-        default: walkers(std::integral_constant<uint32_t, 1>{}); break;
+    } else if (warp == kWorkers) {
+        producer(a, sh, pool, geo, tk0, lane);
+    } else if (warp == kWorkers + 1) {
+        publisher(a, sh, geo, tag, lane);
+    } else {
+        flusher(a, sh, pool, geo, tag, warp - kWorkers - 2, lane);
     }
 }
 
@@ -619,50 +928,31 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
     const uint64_t T = (n + kTile - 1) / kTile;
     const size_t smem = (size_t)kPoolWords * sizeof(uint32_t);
     static bool configured_on[64] = {false};
-    static int per_sm_on[64] = {0};
     bool &configured = configured_on[current_device_slot()];
-    int &per_sm = per_sm_on[current_device_slot()];
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(reduce_ss_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        int v = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, reduce_ss_kernel, kMergeLaunchThreads, smem);
-        if (e != cudaSuccess) return e;
-        per_sm = v > 0 ? v : 1;
         configured = true;
     }
-    // the span length is chosen on the device.  A chunk of a few thousand tiles does not need the whole GPU:
-    // one CTA per 16 tiles leaves room for the other logical ranks' launches of the same ring step
-    uint64_t blocks = (T + 15) / 16;
-    uint64_t cap = (uint64_t)num_sms() * per_sm;   // cooperative: exactly one co-resident wave
-    if (cap > kMaxGrid) cap = kMaxGrid;
+    // the block length is chosen on the device.  A chunk of a few thousand tiles does not need the whole GPU:
+    // one CTA per 16 tiles leaves SMs to the other logical ranks' launches of the same ring step
+    uint64_t blocks = (T + kWorkers - 1) / kWorkers;
+    const uint64_t cap = (uint64_t)kCtasPerSm * (uint64_t)num_sms();
     if (blocks > cap) blocks = cap;
-    // workspace: [header][span words: T][iteration words: iters][group words: iters * ngrp], all zero
-    const uint64_t iters = (T + blocks - 1) / blocks, ngrp = (blocks + 31) / 32;
-    const uint64_t words = T + iters * (1 + ngrp);
-    if ((uint64_t)kWsHeaderBytes + words * 8 > scan_workspace_bytes(n)) return cudaErrorInvalidValue;   // cannot happen
-    cudaError_t e = cudaMemsetAsync(ws, 0, (size_t)kWsHeaderBytes + words * 8, s);
-    if (e != cudaSuccess) return e;
+    if ((uint64_t)kWsHeaderBytes + ((uint64_t)kWsAccWords + T) * 8 > scan_workspace_bytes(n)) return cudaErrorInvalidValue;   // cannot happen
     uint64_t *base = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);
     MergeArgs a;
     a.Bx = Bx; a.By = By; a.Ix = Ix; a.Iy = Iy;
     a.Ax = reinterpret_cast<const uint32_t *>(Ax); a.Ay = reinterpret_cast<const uint32_t *>(Ay);
     a.Bo = Bo; a.Io = Io; a.Ao = reinterpret_cast<uint32_t *>(Ao);
-    a.scan.unit_word = base; a.scan.iter_word = base + T; a.scan.grp_word = base + T + iters;
-    a.scan.ngrp = (uint32_t)ngrp;
+    a.hdr = reinterpret_cast<MergeHeader *>(ws);
+    a.blk_acc = base; a.grp_acc = base + kWsBlkWords; a.tile_word = base + kWsAccWords;
+    a.tile_words = (scan_workspace_bytes(n) - kWsHeaderBytes) / 8 - kWsAccWords;
     a.T = (uint32_t)T;
+    a.zero = 0;
     a.a_limit = (n * 4) & ~15ull;
-#ifdef PICI_MERGE_TRACE
-    {
-        uint64_t *tr = base + words;   // needs a workspace with 296 * 16 * 8 spare words
-        cudaMemcpyToSymbolAsync(g_merge_trace, &tr, sizeof(tr), 0, cudaMemcpyHostToDevice, s);
-    }
-#endif
-    const int32_t *gate_ptr = g.ptr;
-    int32_t gate_value = g.value;
-    void *params[] = {&a, &gate_ptr, &gate_value};
-    return cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(reduce_ss_kernel), dim3((unsigned)blocks),
-                                       dim3(kMergeLaunchThreads), params, smem, s);
+    reduce_ss_kernel<<<(unsigned)blocks, kMergeThreads, smem, s>>>(a, g.ptr, g.value);
+    return cudaGetLastError();
 }
 
 }  // namespace pici

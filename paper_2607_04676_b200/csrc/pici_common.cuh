@@ -90,7 +90,12 @@ __device__ __forceinline__ bool gate_closed(const int32_t *gate, int32_t gate_va
 // progress without any residency assumption).  All sums are integers: the result does not depend on
 // scheduling.
 constexpr uint64_t kStEmpty = 0, kStAggregate = 1, kStPrefix = 2;
-constexpr int kWsHeaderBytes = 128;
+constexpr int kWsHeaderBytes = 128;       // [0, 64): reduce_ss's persistent header; [64, 128): compress's ticket
+constexpr int kWsCompressTicket = 64;
+// Behind the header, at FIXED offsets (so that calls with different n can share a workspace): reduce_ss's
+// accumulators - one word per 1024 tiles and one per 32 tiles, sized for the largest n (2^20 tiles), zero between
+// launches - then one word per tile: compress's status words / reduce_ss's tagged tile counts.
+constexpr uint32_t kWsBlkWords = 1024, kWsGrpWords = 32768, kWsAccWords = kWsBlkWords + kWsGrpWords;
 
 __device__ __forceinline__ uint64_t ld_status(const uint64_t *p) {
     uint64_t v;

@@ -22,7 +22,7 @@ TILE = 4096
 _DT = {torch.float32: F32, torch.bfloat16: BF16}
 
 EXPORTS = (
-    "pici_version", "pici_strerror", "pici_sizes", "pici_compress", "pici_decompress", "pici_reduce_sd",
+    "pici_version", "pici_strerror", "pici_sizes", "pici_workspace_init", "pici_compress", "pici_decompress", "pici_reduce_sd",
     "pici_reduce_ss", "pici_nnz", "pici_nnz_dense", "pici_maybe_densify", "pici_compress_gated",
     "pici_reduce_ss_gated", "pici_maybe_densify_gated", "pici_dense_add_gated", "pici_reduce_sd_out_gated",
     "pici_decompress_gated", "pici_dense_copy_gated", "pici_compress_host", "pici_decompress_host",
@@ -52,6 +52,7 @@ def lib() -> ctypes.CDLL:
             "pici_version": ([], ci),
             "pici_strerror": ([ci], ctypes.c_char_p),
             "pici_sizes": ([u64, ci, p, p, p, p], ci),
+            "pici_workspace_init": ([p, u64, p], ci),
             "pici_compress": ([p, u64, ci, p, p, p, u64, p, u64, p], ci),
             "pici_compress_gated": ([p, u64, ci, p, p, p, u64, p, u64, p, i32, p], ci),
             "pici_decompress": ([p, p, p, u64, ci, p, p], ci),
@@ -154,8 +155,11 @@ def alloc_pici(n: int, dtype: int = F32, device="cuda") -> Pici:
                 torch.empty(max(cap, 8), dtype=tdt, device=device))
 
 
-def alloc_workspace(n: int, device="cuda") -> torch.Tensor:
-    return torch.empty(max(sizes(n, F32)[3], 16), dtype=torch.uint8, device=device)
+def alloc_workspace(n: int, device="cuda", stream=None) -> torch.Tensor:
+    """Scratch for compress / reduce_ss of up to n elements, cleared once (pici_workspace_init)."""
+    ws = torch.empty(max(sizes(n, F32)[3], 16), dtype=torch.uint8, device=device)
+    _check(lib().pici_workspace_init(_p(ws), ws.numel(), _stream(stream)), "pici_workspace_init")
+    return ws
 
 
 def compress(dense: torch.Tensor, out: Pici, ws: torch.Tensor, stream=None, gate=None, gate_value: int = 0) -> Pici:
