@@ -58,7 +58,7 @@ namespace pici {
 constexpr int kCtasPerSm = PICI_MERGE_CTAS;
 constexpr int kWorkers = 16 / kCtasPerSm;                    // worker warps per CTA
 constexpr int kFlushers = 4 / kCtasPerSm;                    // flusher warps per CTA
-constexpr int kMergeThreads = 32 * (kWorkers + 2 + kFlushers);   // + the producer and the publisher warp
+constexpr int kMergeThreads = 32 * (kWorkers + 3 + kFlushers);   // + the planner, the issuer and the publisher warp
 constexpr int kDesc = 8;                                     // items in flight per CTA
 constexpr uint32_t kTileWords = 2 * kSide;                   // u32 words of B per tile
 constexpr uint32_t kMaxBlockTiles = 32;                      // m <= 32: one producer / flusher lane per tile
@@ -67,9 +67,7 @@ constexpr uint32_t kEnd = 0xFFFFFFFFu;
 constexpr uint32_t kMaxTileIn = 2 * kTileWords + 2 * kTile + 16;
 constexpr uint32_t kMaxTileOut = 2 * kTile + 4;        // candidates are bounded by |x| + |y| (cheap to prefix)
 constexpr uint32_t kPoolWords = kCtasPerSm == 2 ? 26624 : 55296;   // 104 KB (two CTAs per SM) or 216 KB of dynamic shared memory
-constexpr uint32_t kMinIn = kMaxTileIn, kMinOut = kMaxTileOut;   // one worst-case tile fits each ring
-constexpr uint32_t kDepth = 4;                               // an average block takes <= 1/kDepth of a ring
-static_assert(kMinIn + kMinOut <= kPoolWords, "pool too small for two full tiles in flight");
+static_assert(kMaxTileIn + kMaxTileOut <= kPoolWords, "pool too small for one worst-case tile");
 
 struct MergeHeader {          // first 64 bytes of the workspace; persistent across launches
     uint32_t epoch;           // tag of the last finished launch
@@ -96,13 +94,25 @@ struct alignas(16) IndexSlot {  // index entries of one block, copied ahead by t
     uint32_t g;                                // the block
 };
 
+constexpr int kPlans = 4;      // planner -> issuer FIFO
+constexpr int kIndexSlots = 8; // index entries stay until the issuer has used them (lead 3 + kPlans behind)
+struct Plan {                  // one item, everything the issuer needs besides the index entries
+    uint32_t islot;            // IndexSlot of the item's block
+    uint32_t i0, i1;           // tiles [i0, i1) of the block
+    uint32_t ts;               // first tile of the block, kEnd = no more items
+    uint32_t xs, ys, nx, ny;   // first value / number of values of x and y
+    uint32_t in_words, out_words;
+    uint32_t flusher;
+};
+
 struct MergeShared {
     uint64_t full[kDesc];      // mbarrier: the item's copies have landed, its descriptor is valid
     uint64_t done[kDesc];      // mbarrier: all workers are through with the item
     uint64_t flushed[kDesc];   // mbarrier: all flushers are through with the item
     ItemDesc desc[kDesc];
-    uint32_t in_end[kDesc], out_end[kDesc];   // producer only: ring heads after the item's allocations
-    IndexSlot idx[4];
+    IndexSlot idx[kIndexSlots];
+    uint64_t plan_full[kPlans], plan_free[kPlans];   // mbarriers of the plan FIFO
+    Plan plan[kPlans];
 };
 
 struct MergeArgs {
@@ -193,40 +203,18 @@ __device__ __forceinline__ Window window_of(uint32_t beg, uint32_t cnt, uint64_t
     return w;
 }
 
-// ---- rings (producer only; every lane computes the same) -------------------------------------------
-struct Ring {
-    uint32_t cap, head, tail, live;
-};
-__device__ __forceinline__ bool ring_alloc(Ring &r, uint32_t n, uint32_t &at) {
-    if (r.live == 0) r.head = r.tail = 0;
-    if (r.live != 0 && r.head == r.tail) return false;   // full
-    if (r.head >= r.tail) {                              // free: [head, cap) and [0, tail)
-        if (r.cap - r.head >= n) {
-            at = r.head;
-            r.head += n;
-            if (r.head == r.cap) r.head = 0;
-        } else if (r.tail >= n) {                        // skip the rest of the buffer
-            at = 0;
-            r.head = n;
-        } else {
-            return false;
-        }
-    } else {                                             // free: [head, tail)
-        if (r.tail - r.head < n) return false;
-        at = r.head;
-        r.head += n;
-    }
-    ++r.live;
-    return true;
-}
-
 // ---- launch-wide geometry, computed identically by every thread ---------------------------------------
 struct Geometry {
     uint32_t m;          // tiles per block
     uint32_t lb;         // bits per lane of a piece: 128, 64, 32, 16 or 8
-    uint32_t in_cap, out_cap;
+    uint32_t slot_in, n_in;     // input slots: words per slot, how many (item j uses slot j mod n_in)
+    uint32_t slot_out, n_out;   // output slots, behind the input slots
+    uint32_t out_base;          // first word of the output slots
     uint32_t blocks;
 };
+// An average block plus 1/8 and a little must fit a slot; at least 4 input and 6 output slots for the block length
+// to be taken (output words live two to three times as long as input words: publish + prefix + flush against load
+// + merge), then as many slots as the pool holds, up to kDesc each.
 __device__ __forceinline__ Geometry geometry(const MergeArgs &a, uint32_t G) {
     Geometry g;
     const uint32_t T = a.T;
@@ -234,53 +222,47 @@ __device__ __forceinline__ Geometry geometry(const MergeArgs &a, uint32_t G) {
     const uint64_t avg = (nx + ny + T - 1) / T;                     // values per tile, X and Y together
     const uint64_t in_tile = 2 * kTileWords + avg + 8;
     const uint64_t out_tile = avg + 4;
-    // output words live two to three times as long as input words (publish + prefix + flush against load + merge)
-    uint64_t oc = (uint64_t)kPoolWords * 2 * out_tile / (in_tile + 2 * out_tile);
-    oc = max(oc, (uint64_t)kMinOut);
-    oc = min(oc, (uint64_t)(kPoolWords - kMinIn));
-    g.out_cap = (uint32_t)oc & ~3u;
-    g.in_cap = kPoolWords - g.out_cap;
+    auto slot_of = [](uint64_t words, uint32_t floor_words) -> uint32_t {
+        const uint64_t v = words + words / 8 + 32;
+        return (uint32_t)((max(v, (uint64_t)floor_words) + 3) & ~3ull);
+    };
+    constexpr uint32_t kFloorIn = 512, kFloorOut = 256;
     uint32_t m = 1;
 #pragma unroll
     for (uint32_t mm = kMaxBlockTiles; mm >= 2; mm /= 2)
-        if (m == 1 && mm * in_tile <= g.in_cap / kDepth && mm * out_tile <= g.out_cap / kDepth) m = mm;
+        if (m == 1 && 4ull * slot_of(mm * in_tile, kFloorIn) + 6ull * slot_of(mm * out_tile, kFloorOut) <= kPoolWords) m = mm;
     while (m > 1 && (T + m - 1) / m < 2u * G) m /= 2;               // small inputs: keep every CTA busy
+    uint32_t si = slot_of(m * in_tile, kFloorIn), so = slot_of(m * out_tile, kFloorOut);
+    uint32_t ni = 1, no = 1;
+    for (;;) {   // output slots first (about two per input slot: their words live longer), up to kDesc of each
+        if (no < kDesc && no < 2u * ni + 2u && (uint64_t)ni * si + (uint64_t)(no + 1u) * so <= kPoolWords) ++no;
+        else if (ni < kDesc && (uint64_t)(ni + 1u) * si + (uint64_t)no * so <= kPoolWords) ++ni;
+        else if (no < kDesc && (uint64_t)ni * si + (uint64_t)(no + 1u) * so <= kPoolWords) ++no;
+        else break;
+    }
     g.m = m;
     g.lb = min(16u * m, 128u);
+    g.slot_in = si; g.n_in = ni; g.slot_out = so; g.n_out = no;
+    g.out_base = ni * si;
     g.blocks = (T + m - 1) / m;
     return g;
 }
 
 // =========================================== producer ===========================================
-__device__ __forceinline__ void producer(const MergeArgs &a, MergeShared &sh, uint32_t *pool, const Geometry &geo,
-                                         uint32_t tk0, int lane) {
-    const uint32_t T = a.T, m = geo.m, ppt = 128u / geo.lb;
-    const uint32_t full0 = smem_u32(&sh.full[0]), done0 = smem_u32(&sh.done[0]), fl0 = smem_u32(&sh.flushed[0]);
-    Ring rin = {geo.in_cap, 0, 0, 0}, rout = {geo.out_cap, 0, 0, 0};
-    const uint32_t in_limit = max(geo.in_cap / 2, kMaxTileIn), out_limit = max(geo.out_cap / 2, kMaxTileOut);
-    uint32_t j = 0;                 // items emitted
-    uint32_t in_tail = 0, out_tail = 0;   // oldest item whose input / output words are still allocated
-    uint32_t blk_seq = 0, piece_base = 0;
-
-    auto free_in = [&]() {          // wait for the oldest item's workers, release its input words
-        const uint32_t d = in_tail % kDesc;
-        mbar_wait_idle(done0 + 8 * d, (in_tail / kDesc) & 1u);
-        rin.tail = sh.in_end[d];
-        --rin.live;
-        ++in_tail;
-    };
-    auto free_out = [&]() {
-        const uint32_t d = out_tail % kDesc;
-        mbar_wait_idle(fl0 + 8 * d, (out_tail / kDesc) & 1u);
-        rout.tail = sh.out_end[d];
-        --rout.live;
-        ++out_tail;
-    };
+// The producer is two warps, because one warp's instruction latency per item (about 1.3 us) was what bounded the
+// whole kernel: the PLANNER takes tickets, fetches index entries and cuts blocks into items (plans); the ISSUER
+// waits for the item's slots, fills the descriptor and starts the copies.
+__device__ __forceinline__ void planner(const MergeArgs &a, MergeShared &sh, const Geometry &geo, uint32_t tk0, int lane) {
+    const uint32_t T = a.T, m = geo.m;
+    const uint32_t pfull0 = smem_u32(&sh.plan_full[0]), pfree0 = smem_u32(&sh.plan_free[0]);
+    const uint32_t in_limit = geo.slot_in, out_limit = geo.slot_out;
+    uint32_t j = 0;                 // items planned
+    uint32_t blk_seq = 0;
     // ---- block pipeline --------------------------------------------------------------------------------------
     // A ticket costs an L2 round trip and so does a block's index entries, each about as long as the CTA has for a
     // whole block in the sparse regime, so both run well ahead of the block in hand (n): tickets are requested
     // five blocks ahead (two atomics in flight, all by lane 0, hence increasing), index entries are copied to
-    // shared memory by cp.async three blocks ahead (slot n & 3).
+    // shared memory by cp.async three blocks ahead (slot n mod kIndexSlots).
     const bool wide = m >= 4u && ((reinterpret_cast<uintptr_t>(a.Ix) | reinterpret_cast<uintptr_t>(a.Iy)) & 15u) == 0u;
     auto issue_index = [&](uint32_t slot, uint32_t g) {
         IndexSlot &S = sh.idx[slot];
@@ -342,16 +324,16 @@ __device__ __forceinline__ void producer(const MergeArgs &a, MergeShared &sh, ui
         // blocks from now (a select between the atomic's result and kEnd would wait for the round trip here)
         tk = kEnd;
         ticket_if(!dry && lane == 0, &a.hdr->ticket + (uint32_t)lane * a.zero, tk);
-        issue_index((n + lead) & 3u, g3);
+        issue_index((n + lead) & (kIndexSlots - 1), g3);
         if (lead == 3u) asm volatile("cp.async.wait_group 3;" ::: "memory");   // block n's entries have landed
         else asm volatile("cp.async.wait_group 1;" ::: "memory");
-        const IndexSlot &S = sh.idx[n & 3u];
+        const IndexSlot &S = sh.idx[n & (kIndexSlots - 1)];
         __syncwarp();
         const uint32_t g_cur = S.g;
         if (g_cur >= geo.blocks) return false;
         const uint32_t ts = g_cur * m, mt = min(m, T - ts);
-        const uint32_t l0 = min((uint32_t)lane, mt), l1 = min((uint32_t)lane + 1u, mt);
-        const uint32_t cx0 = S.ix[l0], cx1 = S.ix[l1], cy0 = S.iy[l0], cy1 = S.iy[l1];
+        const uint32_t l1 = min((uint32_t)lane + 1u, mt);
+        const uint32_t cx1 = S.ix[l1], cy1 = S.iy[l1];
         ++n;
         {
         uint32_t i0 = 0;
@@ -365,57 +347,20 @@ __device__ __forceinline__ void producer(const MergeArgs &a, MergeShared &sh, ui
             const bool fits = need_in <= in_limit && vals + 4u <= out_limit;
             const unsigned bad = __ballot_sync(kFull, in_range && !fits);
             uint32_t i1 = bad ? (uint32_t)__ffs(bad) - 1u : mt;
-            if (i1 <= i0) i1 = i0 + 1;                      // one tile always fits (kMinIn, kMinOut)
-            const uint32_t k = i1 - i0;
+            if (i1 <= i0) i1 = i0 + 1;                      // a tile that fits no slot goes alone, across the slots
             const uint32_t xe = S.ix[i1], ye = S.iy[i1];
             const uint32_t nx = xe - xs, ny = ye - ys;
-            const Window wx = window_of(xs, nx, a.a_limit), wy = window_of(ys, ny, a.a_limit);
-            const uint32_t in_words = 2u * kTileWords * k + wx.words + wy.words;
-            const uint32_t out_words = max((nx + ny + 3u) & ~3u, 4u);
-
-            // ---- descriptor slot and ring space -----------------------------------------------------------
-            const uint32_t d = j % kDesc;
-            while (out_tail + kDesc <= j) free_out();       // item j - kDesc has left slot d
-            while (in_tail + kDesc <= j) free_in();
-            uint32_t ib = 0, ob = 0;
-            while (!ring_alloc(rin, in_words, ib)) free_in();
-            while (!ring_alloc(rout, out_words, ob)) free_out();
-            ob += geo.in_cap;
-            ItemDesc &D = sh.desc[d];
-            const uint32_t V = ib + 2u * kTileWords * k;
-            const uint32_t Xb = V + wx.first, Yb = V + wx.words + wy.first;
-            if ((uint32_t)lane >= i0 && (uint32_t)lane < i1) {
-                const uint32_t i = (uint32_t)lane - i0;
-                D.tile_x[i] = Xb + (cx0 - xs);
-                D.tile_y[i] = Yb + (cy0 - ys);
-                D.tile_out[i] = ob + (cx0 - xs) + (cy0 - ys);
-            }
+            // ---- the plan ---------------------------------------------------------------------------------------
+            const uint32_t q = j % kPlans;
+            if (j >= (uint32_t)kPlans) mbar_wait_idle(pfree0 + 8 * q, ((j / kPlans) - 1u) & 1u);
             if (lane == 0) {
-                D.t0 = ts + i0;
-                D.k = k;
-                D.npieces = k * ppt;
-                D.bx = ib;
-                D.by = ib + kTileWords * k;
-                D.flusher = blk_seq % kFlushers;
-                D.piece_base = piece_base;
-                sh.in_end[d] = rin.head;
-                sh.out_end[d] = rout.head;
+                Plan &P = sh.plan[q];
+                P.islot = (n - 1u) & (kIndexSlots - 1);
+                P.i0 = i0; P.i1 = i1; P.ts = ts;
+                P.xs = xs; P.ys = ys; P.nx = nx; P.ny = ny;
+                P.flusher = blk_seq % kFlushers;
+                mbar_arrive(pfull0 + 8 * q);
             }
-            // tail elements (plain stores, < 4 per operand) before lane 0's arrive, which releases them
-            if (wx.tail_beg + lane < nx) pool[Xb + wx.tail_beg + lane] = a.Ax[xs + wx.tail_beg + lane];
-            if (wy.tail_beg + lane < ny) pool[Yb + wy.tail_beg + lane] = a.Ay[ys + wy.tail_beg + lane];
-            __syncwarp();
-            if (lane == 0) {
-                const uint32_t bar = full0 + 8 * d;
-                const uint32_t bbytes = k * kTileWords * 4u;
-                mbar_expect_tx(bar, 2u * bbytes + wx.bulk + wy.bulk);
-                bulk_g2s(smem_u32(pool + ib), a.Bx + (size_t)(ts + i0) * kSide, bbytes, bar);
-                bulk_g2s(smem_u32(pool + ib + kTileWords * k), a.By + (size_t)(ts + i0) * kSide, bbytes, bar);
-                if (wx.bulk) bulk_g2s(smem_u32(pool + V), reinterpret_cast<const unsigned char *>(a.Ax) + wx.g_beg, wx.bulk, bar);
-                if (wy.bulk)
-                    bulk_g2s(smem_u32(pool + V + wx.words), reinterpret_cast<const unsigned char *>(a.Ay) + wy.g_beg, wy.bulk, bar);
-            }
-            piece_base = (piece_base + k * ppt) % kWorkers;
             ++j;
             i0 = i1;
         }
@@ -431,12 +376,104 @@ __device__ __forceinline__ void producer(const MergeArgs &a, MergeShared &sh, ui
         }
     }
     asm volatile("cp.async.wait_all;" ::: "memory");
-    // every ticket this warp requested must have returned before the item that ends the CTA is emitted (the
-    // launch's last flusher resets the ticket): both registers are read here
-    if (lane == 0 && (tkA & tkB) == 0x12345678u) sh.in_end[0] = 0;   // never true: tickets are < 2^31 or kEnd
+    // every ticket this warp requested must have returned before the CTA's last item is emitted (the launch's last
+    // flusher resets the ticket): both registers are read here
+    if (lane == 0 && (tkA & tkB) == 0x12345678u) sh.idx[0].g = 0;    // never true: tickets are < 2^31 or kEnd
+    const uint32_t q = j % kPlans;
+    if (j >= (uint32_t)kPlans) mbar_wait_idle(pfree0 + 8 * q, ((j / kPlans) - 1u) & 1u);
+    if (lane == 0) {
+        sh.plan[q].ts = kEnd;
+        mbar_arrive(pfull0 + 8 * q);
+    }
+}
+
+__device__ __forceinline__ void issuer(const MergeArgs &a, MergeShared &sh, uint32_t *pool, const Geometry &geo, int lane) {
+    const uint32_t ppt = 128u / geo.lb;
+    const uint32_t full0 = smem_u32(&sh.full[0]), done0 = smem_u32(&sh.done[0]), fl0 = smem_u32(&sh.flushed[0]);
+    const uint32_t pfull0 = smem_u32(&sh.plan_full[0]), pfree0 = smem_u32(&sh.plan_free[0]);
+    uint32_t j = 0;                 // items emitted
+    uint32_t s_in = 0, s_out = 0;   // j mod n_in, j mod n_out
+    bool prev_big = false;          // item j - 1 did not fit a slot (it lies across the pool, see below)
+    uint32_t piece_base = 0;
+    // the workers / all flushers and the publisher are through with item i (i < j)
+    auto wait_done = [&](uint32_t i) { mbar_wait_idle(done0 + 8 * (i % kDesc), (i / kDesc) & 1u); };
+    auto wait_flushed = [&](uint32_t i) { mbar_wait_idle(fl0 + 8 * (i % kDesc), (i / kDesc) & 1u); };
+    for (;; ++j) {
+        const uint32_t q = j % kPlans;
+        mbar_wait(pfull0 + 8 * q, (j / kPlans) & 1u);
+        const Plan &P = sh.plan[q];
+        const uint32_t ts = P.ts;
+        if (ts == kEnd) break;
+        const uint32_t i0 = P.i0, i1 = P.i1, k = i1 - i0;
+        const uint32_t xs = P.xs, ys = P.ys, nx = P.nx, ny = P.ny, flusher = P.flusher;
+        const IndexSlot &S = sh.idx[P.islot];
+        const uint32_t li = min(i0 + (uint32_t)lane, i1);
+        const uint32_t cx0 = S.ix[li], cy0 = S.iy[li];            // lane i < k: tile i0 + i of the block
+        const Window wx = window_of(xs, nx, a.a_limit), wy = window_of(ys, ny, a.a_limit);
+        const uint32_t in_words = 2u * kTileWords * k + wx.words + wy.words;
+        const uint32_t out_words = max((nx + ny + 3u) & ~3u, 4u);
+        // ---- descriptor slot, input slot, output slot ------------------------------------------------------
+        // Item j lives in descriptor j mod kDesc, input slot j mod n_in, output slot j mod n_out: it may start once
+        // the items that had them before are through.  An item that does not fit a slot (a tile much denser than
+        // the launch's average) is laid across the pool from word 0, alone (one worst-case tile always fits):
+        // everything before it has drained, and the item behind it waits for it.
+        const uint32_t d = j % kDesc;
+        const bool big = in_words > geo.slot_in || out_words > geo.slot_out;
+        if (big || prev_big) {
+            for (uint32_t r = 1; r <= min(j, (uint32_t)kDesc); ++r) wait_flushed(j - r);
+        } else {
+            if (j >= geo.n_in) wait_done(j - geo.n_in);
+            if (j >= geo.n_out) wait_flushed(j - geo.n_out);
+            if (j >= (uint32_t)kDesc) wait_flushed(j - kDesc);
+        }
+        prev_big = big;
+        const uint32_t ib = big ? 0u : s_in * geo.slot_in;   // alone in the pool: inputs from word 0, outputs behind
+        const uint32_t ob = big ? in_words : geo.out_base + s_out * geo.slot_out;
+        s_in = s_in + 1u == geo.n_in ? 0u : s_in + 1u;
+        s_out = s_out + 1u == geo.n_out ? 0u : s_out + 1u;
+        ItemDesc &D = sh.desc[d];
+        const uint32_t V = ib + 2u * kTileWords * k;
+        const uint32_t Xb = V + wx.first, Yb = V + wx.words + wy.first;
+        if ((uint32_t)lane < k) {
+            D.tile_x[lane] = Xb + (cx0 - xs);
+            D.tile_y[lane] = Yb + (cy0 - ys);
+            D.tile_out[lane] = ob + (cx0 - xs) + (cy0 - ys);
+        }
+        if (lane == 0) {
+            D.t0 = ts + i0;
+            D.k = k;
+            D.npieces = k * ppt;
+            D.bx = ib;
+            D.by = ib + kTileWords * k;
+            D.flusher = flusher;
+            D.piece_base = piece_base;
+        }
+        // tail elements (plain stores, < 4 per operand) before lane 0's arrive, which releases them
+        if (wx.tail_beg + lane < nx) pool[Xb + wx.tail_beg + lane] = a.Ax[xs + wx.tail_beg + lane];
+        if (wy.tail_beg + lane < ny) pool[Yb + wy.tail_beg + lane] = a.Ay[ys + wy.tail_beg + lane];
+        __syncwarp();
+        {
+            // the four bulk copies (Bx words, By words, X values, Y values) leave as ONE instruction: lane c issues
+            // copy c
+            const uint32_t bar = full0 + 8 * d;
+            const uint32_t bbytes = k * kTileWords * 4u;
+            if (lane == 0) {
+                mbar_arrive(pfree0 + 8 * q);                  // the plan and its index entries have been read
+                mbar_expect_tx(bar, 2u * bbytes + wx.bulk + wy.bulk);
+            }
+            __syncwarp();
+            const unsigned char *src = nullptr;
+            uint32_t dstw = 0, bytes = 0;
+            if (lane == 0) { src = reinterpret_cast<const unsigned char *>(a.Bx + (size_t)(ts + i0) * kSide); dstw = ib; bytes = bbytes; }
+            else if (lane == 1) { src = reinterpret_cast<const unsigned char *>(a.By + (size_t)(ts + i0) * kSide); dstw = ib + kTileWords * k; bytes = bbytes; }
+            else if (lane == 2) { src = reinterpret_cast<const unsigned char *>(a.Ax) + wx.g_beg; dstw = V; bytes = wx.bulk; }
+            else if (lane == 3) { src = reinterpret_cast<const unsigned char *>(a.Ay) + wy.g_beg; dstw = V + wx.words; bytes = wy.bulk; }
+            if (bytes) bulk_g2s(smem_u32(pool + dstw), src, bytes, bar);
+        }
+        piece_base = (piece_base + k * ppt) % kWorkers;
+    }
     const uint32_t d = j % kDesc;
-    while (out_tail + kDesc <= j) free_out();
-    while (in_tail + kDesc <= j) free_in();
+    if (j >= (uint32_t)kDesc) wait_flushed(j - kDesc);
     if (lane == 0) {
         sh.desc[d].t0 = kEnd;
         mbar_arrive(full0 + 8 * d);
@@ -902,6 +939,10 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
             mbar_init(smem_u32(&sh.done[d]), kWorkers);
             mbar_init(smem_u32(&sh.flushed[d]), kFlushers + 1);
         }
+        for (int q = 0; q < kPlans; ++q) {
+            mbar_init(smem_u32(&sh.plan_full[q]), 1);
+            mbar_init(smem_u32(&sh.plan_free[q]), 1);
+        }
     }
     __syncthreads();
 
@@ -913,11 +954,13 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
             default: worker<16>(a, sh, pool, warp, lane); break;
         }
     } else if (warp == kWorkers) {
-        producer(a, sh, pool, geo, tk0, lane);
+        planner(a, sh, geo, tk0, lane);
     } else if (warp == kWorkers + 1) {
+        issuer(a, sh, pool, geo, lane);
+    } else if (warp == kWorkers + 2) {
         publisher(a, sh, geo, tag, lane);
     } else {
-        flusher(a, sh, pool, geo, tag, warp - kWorkers - 2, lane);
+        flusher(a, sh, pool, geo, tag, warp - kWorkers - 3, lane);
     }
 }
 
