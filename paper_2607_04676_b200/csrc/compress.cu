@@ -39,12 +39,16 @@ struct CompressCfg<PICI_BF16> {
 template <int DT>
 __global__ void __launch_bounds__(kCompressWarps * 32, CompressCfg<DT>::kMinBlocks)
 compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict__ B,
-                uint32_t *__restrict__ I, void *__restrict__ A, uint32_t *ticket, uint64_t *status,
+                uint32_t *__restrict__ I, void *__restrict__ A, void *ws, uint64_t *status,
                 const int32_t *gate, int32_t gate_value) {
     using Cfg = CompressCfg<DT>;
     using Elem = typename Cfg::Elem;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (gate_closed(gate, gate_value)) return;
+    // [ticket, warps that have left] live behind the workspace header; the launch's last warp resets them and
+    // advances the epoch, so no launch starts with a memset (status words carry the epoch, pici_common.cuh)
+    uint32_t *const ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + kWsCompressTicket);
+    const uint32_t tag = launch_tag(ws);
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -105,7 +109,7 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
     uint32_t pt = 0, pnnz = 0;
     auto flush_pending = [&]() {
         if (pending) {
-            const uint32_t excl = lookback_prefix(status, pt, pnnz, T, I, lane);
+            const uint32_t excl = lookback_prefix(status, tag, pt, pnnz, T, I, lane);
             Elem *dst = Aout + excl;
             for (uint32_t i = lane; i < pnnz; i += 32) dst[i] = stage[i];
             __syncwarp();
@@ -146,7 +150,7 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
         const uint32_t tile_nnz = __shfl_sync(kFull, incl, 31);
 
         // ---- Phase 2: publish this tile's count (the look-back itself is deferred, see above) ----
-        publish_count(status, t, tile_nnz, lane);
+        publish_count(status, tag, t, tile_nnz, lane);
 
         // B: lane l holds words 2l, 2l+1 -> one 16-byte store per lane, 512 contiguous bytes per warp
         {
@@ -194,6 +198,19 @@ compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict
         if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
     }
     flush_pending();
+    // ---- the last warp of the launch to leave resets the ticket and advances the epoch ------------------------
+    uint32_t last = 0;
+    if (lane == 0) {
+        __threadfence();
+        last = atomicAdd(ticket + 1, 1u) + 1u == gridDim.x * (uint32_t)kCompressWarps;
+    }
+    if (__shfl_sync(kFull, last, 0)) {
+        if (lane == 0) {
+            ticket[0] = 0;
+            ticket[1] = 0;
+        }
+        finish_epoch(ws, tag, status, T, lane);
+    }
 }
 
 int num_sms() {
@@ -228,18 +245,11 @@ static cudaError_t launch_compress_t(const void *dense, uint64_t n, uint64_t *B,
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    // bytes [0, 64) of the workspace hold reduce_ss's persistent header (epoch, merge.cu): never cleared here
-    unsigned char *wsb = reinterpret_cast<unsigned char *>(ws);
-    uint64_t *status = reinterpret_cast<uint64_t *>(wsb + kWsHeaderBytes) + kWsAccWords;
-    cudaError_t e = cudaMemsetAsync(wsb + kWsCompressTicket, 0, kWsHeaderBytes - kWsCompressTicket, s);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(status, 0, T * 8, s);
-    if (e != cudaSuccess) return e;
+    uint64_t *status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes) + kWsAccWords;
     uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
     const uint64_t cap = (uint64_t)num_sms() * Cfg::kMinBlocks;           // persistent: one resident wave
     if (blocks > cap) blocks = cap;
-    uint32_t *ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + kWsCompressTicket);
-    compress_kernel<DT><<<(unsigned)blocks, kCompressWarps * 32, smem, s>>>(dense, n, B, I, A, ticket, status,
+    compress_kernel<DT><<<(unsigned)blocks, kCompressWarps * 32, smem, s>>>(dense, n, B, I, A, ws, status,
                                                                           g.ptr, g.value);
     return cudaGetLastError();
 }

@@ -69,11 +69,7 @@ constexpr uint32_t kMaxTileOut = 2 * kTile + 4;        // candidates are bounded
 constexpr uint32_t kPoolWords = kCtasPerSm == 2 ? 26624 : 55296;   // 104 KB (two CTAs per SM) or 216 KB of dynamic shared memory
 static_assert(kMaxTileIn + kMaxTileOut <= kPoolWords, "pool too small for one worst-case tile");
 
-struct MergeHeader {          // first 64 bytes of the workspace; persistent across launches
-    uint32_t epoch;           // tag of the last finished launch
-    uint32_t ticket;          // next block
-    uint32_t finished;        // flusher warps that have left
-};
+using MergeHeader = WsHeader;   // epoch, ticket, flusher warps that have left (pici_common.cuh)
 
 struct ItemDesc {
     uint32_t t0;                       // first tile, kEnd = no more items
@@ -902,21 +898,14 @@ __device__ __forceinline__ void flusher(const MergeArgs &a, MergeShared &sh, con
         last = atomicAdd(&a.hdr->finished, 1u) + 1u == gridDim.x * (uint32_t)kFlushers;
     }
     if (__shfl_sync(kFull, last, 0)) {
-        uint32_t e = tag & 0x7FFFFFFFu;
         const uint32_t ngrp = (a.T + 31u) / 32u, nblk = (a.T + 1023u) / 1024u;
         for (uint32_t q = lane; q < ngrp; q += 32) a.grp_acc[q] = 0;
         for (uint32_t q = lane; q < nblk; q += 32) a.blk_acc[q] = 0;
-        if (e == 0x7FFFFFFFu) {   // the 31-bit epoch wraps: forget every tagged word (once per 2^31 launches)
-            for (uint64_t q = lane; q < a.tile_words; q += 32) a.tile_word[q] = 0;
-            e = 0;
-        }
-        __syncwarp();
         if (lane == 0) {
             a.hdr->ticket = 0;
             a.hdr->finished = 0;
-            __threadfence();
-            a.hdr->epoch = e;
         }
+        finish_epoch(a.hdr, tag, a.tile_word, a.tile_words, lane);
     }
 }
 
@@ -927,8 +916,7 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     if (gate_closed(gate, gate_value)) return;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // tag of this launch: epoch + 1 with the top bit set (compress's status flags 1 / 2 never have it)
-    const uint32_t tag = ((*reinterpret_cast<const volatile uint32_t *>(&a.hdr->epoch) + 1u) & 0x7FFFFFFFu) | 0x80000000u;
+    const uint32_t tag = launch_tag(a.hdr);   // this launch's tag for the tile words (pici_common.cuh)
     // the producer's first ticket is requested before anything else: it returns while the geometry loads do
     uint32_t tk0 = 0;
     if (warp == kWorkers && lane == 0) tk0 = atomicAdd(&a.hdr->ticket, 1u);

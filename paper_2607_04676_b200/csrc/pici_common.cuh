@@ -80,42 +80,70 @@ __device__ __forceinline__ bool gate_closed(const int32_t *gate, int32_t gate_va
 // Decoupled look-back at TILE granularity (one partition = one 64x64 tile = one warp's unit of work).
 // One 64-bit status word per tile: high 32 bits = flag, low 32 bits = value; flag and value travel in
 // ONE 64-bit access, so relaxed gpu-scope accesses suffice (nothing else is published through it).
-//   kStAggregate : value = nnz of the tile               (published right after Phase 1)
-//   kStPrefix    : value = nnz of tiles 0..t inclusive   (published after the tile's look-back)
+//   aggregate : value = nnz of the tile               (published right after Phase 1)
+//   prefix    : value = nnz of tiles 0..t inclusive   (published after the tile's look-back)
 // A tile's look-back reads the 32 status words before it in one coalesced request (lane l <-> tile
-// pos-1-l), takes everything up to the closest kStPrefix, or - if the window holds aggregates only -
+// pos-1-l), takes everything up to the closest prefix, or - if the window holds aggregates only -
 // adds all 32 and moves one window further back.  Aggregates do not depend on any other tile, so a
 // look-back never waits on another look-back, only on Phase 1 of earlier tiles; tiles are handed out
 // by a dynamic ticket, so every earlier tile is owned by a warp that is already running (forward
 // progress without any residency assumption).  All sums are integers: the result does not depend on
 // scheduling.
-constexpr uint64_t kStEmpty = 0, kStAggregate = 1, kStPrefix = 2;
-constexpr int kWsHeaderBytes = 128;       // [0, 64): reduce_ss's persistent header; [64, 128): compress's ticket
+// Status words are tagged with the launch epoch kept in the workspace header (WsHeader below), so a workspace
+// is never cleared between launches: high 32 bits = 1 (bit 31) | kind (bit 30: 0 aggregate, 1 prefix) | epoch tag
+// (30 bits), low 32 bits = value.  A word of an earlier launch (or a zero word) never carries the current tag.
+constexpr uint32_t kTagValid = 0x80000000u, kTagPrefix = 0x40000000u, kTagMask = 0x3FFFFFFFu;
+constexpr int kWsHeaderBytes = 128;       // [0, 64): WsHeader; [64, 128): compress's ticket and exit counter
 constexpr int kWsCompressTicket = 64;
 // Behind the header, at FIXED offsets (so that calls with different n can share a workspace): reduce_ss's
 // accumulators - one word per 1024 tiles and one per 32 tiles, sized for the largest n (2^20 tiles), zero between
 // launches - then one word per tile: compress's status words / reduce_ss's tagged tile counts.
 constexpr uint32_t kWsBlkWords = 1024, kWsGrpWords = 32768, kWsAccWords = kWsBlkWords + kWsGrpWords;
 
+struct WsHeader {             // first bytes of the workspace; persistent across launches (pici_workspace_init: 0)
+    uint32_t epoch;           // tag of the last finished launch (compress and reduce_ss share it)
+    uint32_t ticket;          // reduce_ss: next block
+    uint32_t finished;        // reduce_ss: flusher warps that have left
+};
+// Tag of the launch that starts now (read by every thread at kernel entry; 1 .. kTagMask).
+__device__ __forceinline__ uint32_t launch_tag(const void *ws) {
+    const uint32_t e = *reinterpret_cast<const volatile uint32_t *>(ws);
+    return kTagValid | ((e + 1u) & kTagMask);
+}
+// The launch's last warp: every tagged word of an earlier launch is stale from now on.  When the 30-bit tag is
+// about to wrap, the `words` tagged words are cleared first (once per 2^30 launches), by the calling warp.
+__device__ __forceinline__ void finish_epoch(void *ws, uint32_t tag, uint64_t *tagged, uint64_t words, int lane) {
+    uint32_t e = tag & kTagMask;
+    if (e == kTagMask) {
+        for (uint64_t q = lane; q < words; q += 32) tagged[q] = 0;
+        e = 0;
+    }
+    __syncwarp();
+    if (lane == 0) {
+        __threadfence();
+        *reinterpret_cast<volatile uint32_t *>(ws) = e;
+    }
+}
+
 __device__ __forceinline__ uint64_t ld_status(const uint64_t *p) {
     uint64_t v;
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_status(uint64_t *p, uint64_t flag, uint32_t value) {
-    uint64_t v = (flag << 32) | value;
+__device__ __forceinline__ void st_status(uint64_t *p, uint64_t tag, uint32_t value) {
+    uint64_t v = (tag << 32) | value;
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
 // Step 1 (warp-collective): make tile t's count visible.  Tile 0 has no predecessor: its aggregate
 // is its inclusive prefix.
-__device__ __forceinline__ void publish_count(uint64_t *status, uint32_t t, uint32_t count, int lane) {
-    if (lane == 0) st_status(status + t, t == 0 ? kStPrefix : kStAggregate, count);
+__device__ __forceinline__ void publish_count(uint64_t *status, uint32_t tag, uint32_t t, uint32_t count, int lane) {
+    if (lane == 0) st_status(status + t, t == 0 ? (tag | kTagPrefix) : tag, count);
 }
 
 // Step 2 (warp-collective): exclusive prefix of tile t = sum of the counts of tiles 0..t-1; publishes
 // the tile's inclusive prefix and writes I[t] (and I[T] from the last tile).
-__device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t t, uint32_t count, uint32_t T,
+__device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t tag, uint32_t t, uint32_t count, uint32_t T,
                                                     uint32_t *__restrict__ I, int lane) {
     uint32_t excl = 0;
     int64_t pos = t;  // tiles [0, pos) are not yet accounted for
@@ -125,10 +153,11 @@ __device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t t
         unsigned pm, em;
         unsigned ns = 8;
         for (;;) {
-            s = idx >= 0 ? ld_status(status + idx) : (kStPrefix << 32);
-            const uint32_t flag = (uint32_t)(s >> 32);
-            pm = __ballot_sync(kFull, flag == (uint32_t)kStPrefix);
-            em = __ballot_sync(kFull, flag == (uint32_t)kStEmpty);
+            s = idx >= 0 ? ld_status(status + idx) : ((uint64_t)(tag | kTagPrefix) << 32);
+            const uint32_t hi = (uint32_t)(s >> 32);
+            const bool valid = (hi & ~kTagPrefix) == tag;
+            pm = __ballot_sync(kFull, valid && (hi & kTagPrefix) != 0u);
+            em = __ballot_sync(kFull, !valid);
             // lanes that matter: up to and including the closest prefix (all 32 if there is none)
             const unsigned rel = pm ? ((pm & (0u - pm)) | ((pm & (0u - pm)) - 1u)) : kFull;
             if ((em & rel) == 0u) {
@@ -143,71 +172,16 @@ __device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t t
         pos -= 32;
     }
     if (lane == 0) {
-        if (t != 0) st_status(status + t, kStPrefix, excl + count);
+        if (t != 0) st_status(status + t, tag | kTagPrefix, excl + count);
         I[t] = excl;
         if (t + 1 == T) I[T] = excl + count;
     }
     return excl;
 }
 
-// ---- round-robin scan: exclusive prefix of per-unit counts in ONE L2 round trip --------------------
-// For persistent grids launched cooperatively (every worker resident) whose W workers take units
-// round-robin: worker c handles units c, c + W, c + 2W, ...; "iteration" it covers units
-// [it*W, (it+1)*W).  A worker publishes its unit's count as (a) a per-unit word (1 << 32 | count),
-// (b) a 64-bit atomic add of (1 << 48) + count into the word of its group of 32 units and (c) into the
-// word of its iteration; each word carries (number of adds, sum) in one 64-bit access, so relaxed
-// gpu-scope accesses suffice.  prefix(it, c) = complete iterations below it + complete groups below
-// c's + the units of c's own group below c: independent loads, 32 + 64 + 32 words at most.  The workers
-// run nearly in lock-step, so a flat decoupled look-back would find no prefix among the W - 1 units
-// of its own iteration and walk W / 32 dependent hops (measured in reduce_ss: ~8 us per iteration).
-constexpr uint32_t kRoundRobinMaxUnits = 2048;   // W <= 2048: two group words per lane
-struct RoundRobinScan {
-    uint64_t *unit_word;   // [units]
-    uint64_t *grp_word;    // [iterations][ngrp], ngrp = ceil(W / 32)
-    uint64_t *iter_word;   // [iterations]
-    uint32_t ngrp;
-};
 constexpr uint64_t kOneAdd = 1ull << 48;
 __device__ __forceinline__ void red_add_u64(uint64_t *p, uint64_t v) {
     asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-// One thread: publish the count of unit u = it * W + c.
-__device__ __forceinline__ void rr_publish(const RoundRobinScan &sc, uint64_t u, uint32_t it, uint32_t c, uint32_t count) {
-    st_status(sc.unit_word + u, 1u, count);
-    red_add_u64(sc.grp_word + (size_t)it * sc.ngrp + (c >> 5), kOneAdd + count);
-    red_add_u64(sc.iter_word + it, kOneAdd + count);
-}
-// One warp: sum of the counts of all units below (it, c).  E = running sum of the complete iterations
-// [0, E_it), carried by the caller from call to call (up to 32 iteration words are added per call).
-// All W units of an iteration below `it` exist, and so do all 32 units of a group below c's.
-__device__ __forceinline__ uint32_t rr_lookback(const RoundRobinScan &sc, uint32_t W, uint32_t it, uint32_t c, uint32_t &E,
-                                                uint32_t &E_it, int lane) {
-    const uint32_t nfull = c >> 5, rem = c & 31u;
-    const uint64_t *gw = sc.grp_word + (size_t)it * sc.ngrp;
-    const uint64_t *uw = sc.unit_word + (size_t)it * W + (size_t)nfull * 32;
-    while (E_it + 32 < it) {   // not taken when a worker sees consecutive iterations
-        uint64_t v;
-        do { v = ld_status(sc.iter_word + E_it); } while ((uint32_t)(v >> 48) != W);
-        E += (uint32_t)v;
-        ++E_it;
-    }
-    const uint32_t nit = it - E_it;
-    uint64_t vi, vg, vh, vs;
-    unsigned ns = 8;
-    for (;;) {
-        vi = (uint32_t)lane < nit ? ld_status(sc.iter_word + E_it + lane) : ((uint64_t)W << 48);
-        vg = (uint32_t)lane < nfull ? ld_status(gw + lane) : (32ull << 48);
-        vh = (uint32_t)lane + 32u < nfull ? ld_status(gw + 32 + lane) : (32ull << 48);
-        vs = (uint32_t)lane < rem ? ld_status(uw + lane) : (1ull << 32);
-        const bool ok = (uint32_t)(vi >> 48) == W && (uint32_t)(vg >> 48) == 32u && (uint32_t)(vh >> 48) == 32u &&
-                        (uint32_t)(vs >> 32) != 0u;
-        if (__all_sync(kFull, ok)) break;
-        __nanosleep(ns);
-        if (ns < 128) ns += ns;
-    }
-    E += warp_sum((uint32_t)vi);
-    E_it = it;
-    return E + warp_sum((uint32_t)vg + (uint32_t)vh + (uint32_t)vs);
 }
 
 // ---- TMA 1-D bulk copy global -> shared, completion on an mbarrier (UBLKCP in SASS) -------------
