@@ -168,21 +168,14 @@ def run_reference(args):
     x = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 0)).numpy()
     y = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 1)).numpy()
 
-    def step():
-        px = po.compress(x.view(np.uint32), "f32")
-        py = po.compress(y.view(np.uint32), "f32")
-        pz = po.reduce_ss(px, py)
-        po.nnz_pici(pz)
-        dense = np.empty(n, np.uint32)
-        po.maybe_densify(pz, 0, dense)
-        po.reduce_sd(px, dense.view(np.float32))
-
-    for _ in range(args.warmup):
-        step()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        step()
-    dt = time.perf_counter() - t0
+    with PinnedCore() as pin:
+        for _ in range(args.warmup):
+            oracle_step(po, np, x, y, n)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            oracle_step(po, np, x, y, n)
+        dt = time.perf_counter() - t0
+        where = pin.describe()
     val = OPS_PER_STEP * n * 4 * args.steps / dt / 1e9
     sample = f"first-principles sample: N=2^{n.bit_length() - 1} elements of the same recipe per step (full workload N=2^28)"
     print(json.dumps({
@@ -192,7 +185,7 @@ def run_reference(args):
         "config": {"workload": f"configs[1] Pici hot path, fp32, sparsity {args.sparsity}, seeds 0/1; oracle on host cores",
                    "sample": sample},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-                         "host_cores_available": os.cpu_count()},
+                         "host_cores_available": os.cpu_count(), **where},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -243,61 +236,99 @@ def touched_sectors_f32(mask_dense: torch.Tensor) -> int:
     return int((mask_dense[:n8].view(-1, 8) != 0).any(dim=1).sum().item())
 
 
-def time_op(fn, iters: int, warm: int = 2):
-    for _ in range(warm):
-        fn()
+def graph_time(fns, launches: int, replays: int = 5, warm: int = 5):
+    """Per-launch time of a kernel with no host cost inside the timed region: `launches` calls - call i uses
+    fns[i % len(fns)], i.e. the buffer sets are rotated so that nothing is re-read from L2 - are captured into ONE
+    CUDA graph, replayed `replays` times between CUDA events (after `warm` eager calls per set and one replay).
+    Returns (median, min) over the replays of ms per launch."""
+    for _ in range(max(1, (warm + len(fns) - 1) // len(fns))):
+        for f in fns:
+            f()
     torch.cuda.synchronize()
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
-    for a, b in evs:
-        a.record(); fn(); b.record()
+    st = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(g, stream=st):
+            for i in range(launches):
+                fns[i % len(fns)]()
+    g.replay()
     torch.cuda.synchronize()
-    ts = sorted(a.elapsed_time(b) for a, b in evs)
+    ts = []
+    for _ in range(replays):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); g.replay(); b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b) / launches)
+    ts.sort()
     return ts[len(ts) // 2], ts[0]
 
 
-def run_sweep(pk, n: int, peak: float, iters: int, device, dtypes=("f32", "bf16"), sparsities=None,
-              ops=("compress", "decompress", "reduce_ss", "reduce_sd")) -> list[dict]:
-    """Every kernel alone at every sparsity of configs[1] (seed 0; fp32: all ops, bf16: compress/decompress)."""
+L2_BYTES = 126e6                     # B200 L2 (B200_PROFILING.md)
+
+
+def run_sweep(pk, n: int, peak: float, launches: int, device, dtypes=("f32", "bf16"), sparsities=None,
+              ops=("compress", "decompress", "reduce_ss", "reduce_sd"), seeds=(0, 1, 2, 3, 4)) -> list[dict]:
+    """Every kernel alone at every sparsity of configs[1], fp32: all ops, bf16: compress / decompress.
+    Seeds 0-4 of the config are five buffer sets; launch i of the timed CUDA graph works on set i mod 5, so every
+    launch reads inputs that at least four other launches' traffic (> 2x L2 for every op) has pushed out of L2,
+    and the reported time is the mean over the seeds (SURVEY.md S8(d) Timing: >= 5 warm-ups, >= 100 timed launches,
+    rotate buffer sets when the working set is < 2x L2)."""
     rows = []
     for dtype in dtypes:
         s = 4 if dtype == "f32" else 2
         D = pk.F32 if dtype == "f32" else pk.BF16
+        ws = pk.alloc_workspace(n, device)
         for sp in (sparsities or wl.CONFIG2_SPARSITIES):
             d = 1.0 - sp
-            x = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 0), dtype=dtype, device=device)
-            px = pk.alloc_pici(n, D, device)
-            ws = pk.alloc_workspace(n, device)
-            out = torch.empty_like(x)
+            merge = dtype == "f32" and ("reduce_ss" in ops or "reduce_sd" in ops)
+            sets = []
+            for sd in seeds:
+                S = {"x": wl.sparse_buffer(n, d, seed=wl.stream_seed(sd, 0), dtype=dtype, device=device),
+                     "px": pk.alloc_pici(n, D, device)}
+                pk.compress(S["x"], S["px"], ws)
+                if "decompress" in ops:
+                    S["out"] = torch.empty_like(S["x"])
+                if merge:
+                    S["y"] = wl.sparse_buffer(n, d, seed=wl.stream_seed(sd, 1), dtype=dtype, device=device)
+                    S["py"], S["po"] = pk.alloc_pici(n, D, device), pk.alloc_pici(n, D, device)
+                    pk.compress(S["y"], S["py"], ws)
+                    pk.reduce_ss(S["px"], S["py"], S["po"], ws)
+                sets.append(S)
+            torch.cuda.synchronize()
+            for S in sets:
+                S["nx"] = S["px"].nnz_host()
+                if merge:
+                    S["ny"], S["no"] = S["py"].nnz_host(), S["po"].nnz_host()
+            mean = lambda vals: sum(vals) / len(vals)
 
-            def row(op, ms, ms_min, nbytes):
-                rows.append({"dtype": dtype, "sparsity": sp, "op": op, "ms": round(ms, 4), "ms_min": round(ms_min, 4),
-                             "dense_equiv_gbs": round(n * s / ms / 1e6, 1), "bytes_moved_gbs": round(nbytes / ms / 1e6, 1),
-                             "frac": round(nbytes / ms / 1e6 / peak, 3)})
+            def row(op, fns, nbytes, extra=None):
+                ms, mn = graph_time(fns, launches)
+                r = {"dtype": dtype, "sparsity": sp, "op": op, "ms": round(ms, 4), "ms_min": round(mn, 4),
+                     "dense_equiv_gbs": round(n * s / ms / 1e6, 1), "alg_bytes": int(nbytes),
+                     "bytes_moved_gbs": round(nbytes / ms / 1e6, 1), "frac": round(nbytes / ms / 1e6 / peak, 3),
+                     "seeds": list(seeds), "launches_timed": launches * 5,
+                     "l2": f"defeated: {len(seeds)} rotated buffer sets, {nbytes * (len(seeds) - 1) / L2_BYTES:.1f}x L2 between reuses"}
+                if extra:
+                    r.update(extra)
+                rows.append(r)
 
-            pk.compress(x, px, ws)
-            nx = px.nnz_host()
             if "compress" in ops:
-                ms, mn = time_op(lambda: pk.compress(x, px, ws), iters)
-                row("compress", ms, mn, bytes_compress(n, s, nx))
+                row("compress", [lambda S=S: pk.compress(S["x"], S["px"], ws) for S in sets],
+                    mean([bytes_compress(n, s, S["nx"]) for S in sets]))
             if "decompress" in ops:
-                ms, mn = time_op(lambda: pk.decompress(px, out), iters)
-                row("decompress", ms, mn, bytes_decompress(n, s, nx))
-            if dtype == "f32" and ("reduce_ss" in ops or "reduce_sd" in ops):
-                y = wl.sparse_buffer(n, d, seed=wl.stream_seed(0, 1), dtype=dtype, device=device)
-                py, po = pk.alloc_pici(n, D, device), pk.alloc_pici(n, D, device)
-                pk.compress(y, py, ws)
-                pk.reduce_ss(px, py, po, ws)
-                ny, no = py.nnz_host(), po.nnz_host()
-                if "reduce_ss" in ops:
-                    ms, mn = time_op(lambda: pk.reduce_ss(px, py, po, ws), iters)
-                    row("reduce_ss", ms, mn, bytes_reduce_ss(n, nx, ny, no))
-                if "reduce_sd" in ops:
-                    sect = touched_sectors_f32(x)
-                    ms, mn = time_op(lambda: pk.reduce_sd(px, y), iters)      # in place into a 2^28 dense buffer
-                    row("reduce_sd", ms, mn, bytes_reduce_sd(n, nx, sect))
-                    rows[-1]["touched_sector_frac"] = round(sect / (n / 8), 4)
-                del y, py, po
-            del x, px, out, ws
+                row("decompress", [lambda S=S: pk.decompress(S["px"], S["out"]) for S in sets],
+                    mean([bytes_decompress(n, s, S["nx"]) for S in sets]))
+            if merge and "reduce_ss" in ops:
+                row("reduce_ss", [lambda S=S: pk.reduce_ss(S["px"], S["py"], S["po"], ws) for S in sets],
+                    mean([bytes_reduce_ss(n, S["nx"], S["ny"], S["no"]) for S in sets]))
+            if merge and "reduce_sd" in ops:
+                sect = mean([touched_sectors_f32(S["x"]) for S in sets])
+                elem = mean([meta_bytes(n) + 12 * S["nx"] for S in sets])      # S8(d): 0.126 + 12 d bytes per element
+                # in place into the (dense) y buffer of the set: every launch adds x once more
+                row("reduce_sd", [lambda S=S: pk.reduce_sd(S["px"], S["y"]) for S in sets],
+                    mean([bytes_reduce_sd(n, S["nx"], sect) for S in sets]),
+                    {"touched_sector_frac": round(sect / (n / 8), 4), "alg_bytes_element_level": int(elem)})
+            del sets
             torch.cuda.empty_cache()
     return rows
 
@@ -329,30 +360,60 @@ def run_e2e(pk, n: int, density: float, steps: int, device, seed: int) -> dict:
             "path": "pici_compress_host + pici_decompress_host (pinned host buffers; 2 buffers of N*4 bytes per step)"}
 
 
+class PinnedCore:
+    """The oracle leg runs single-threaded on ONE host core (SURVEY.md S8(d) "Oracle timing": 1 thread, pinned as
+    `taskset -c` would, nproc printed beside the result)."""
+
+    def __enter__(self):
+        self.saved, self.core = None, None
+        try:
+            self.saved = os.sched_getaffinity(0)
+            self.core = max(self.saved)
+            os.sched_setaffinity(0, {self.core})
+        except Exception:
+            self.saved = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.saved is not None:
+            try:
+                os.sched_setaffinity(0, self.saved)
+            except Exception:
+                pass
+
+    def describe(self) -> dict:
+        return {"pinned_core": self.core, "nproc": os.cpu_count()}
+
+
+def oracle_step(po, np, x, y, n):
+    px = po.compress(x.view(np.uint32), "f32")
+    py = po.compress(y.view(np.uint32), "f32")
+    pz = po.reduce_ss(px, py)
+    po.nnz_pici(pz)
+    dense = np.empty(n, np.uint32)
+    po.maybe_densify(pz, 0, dense)
+    po.reduce_sd(px, dense.view(np.float32))
+
+
 def run_cpu_baseline(n: int, density: float) -> dict:
     import numpy as np
     from oracle import pici_oracle as po
     x = wl.sparse_buffer(n, density, seed=wl.stream_seed(0, 0)).numpy()
     y = wl.sparse_buffer(n, density, seed=wl.stream_seed(0, 1)).numpy()
     best = None
-    t_all = time.perf_counter()
-    reps = 0
-    while reps < 2 or (time.perf_counter() - t_all < 8.0 and reps < 6):
-        t0 = time.perf_counter()
-        px = po.compress(x.view(np.uint32), "f32")
-        py = po.compress(y.view(np.uint32), "f32")
-        pz = po.reduce_ss(px, py)
-        po.nnz_pici(pz)
-        dense = np.empty(n, np.uint32)
-        po.maybe_densify(pz, 0, dense)
-        po.reduce_sd(px, dense.view(np.float32))
-        dt = time.perf_counter() - t0
-        best = dt if best is None else min(best, dt)
-        reps += 1
-    return {"value": OPS_PER_STEP * n * 4 / best / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"same step on N=2^{n.bit_length() - 1} elements of the same recipe (fp32, same sparsity, seeds 0/1), "
-                      f"best of {reps}; oracle/pici_oracle.c single thread, gcc -O2",
-            "host_cores_available": os.cpu_count()}
+    with PinnedCore() as pin:
+        for _ in range(3):                       # best of 3 (BASELINE.md S4)
+            t0 = time.perf_counter()
+            oracle_step(po, np, x, y, n)
+            dt = time.perf_counter() - t0
+            best = dt if best is None else min(best, dt)
+        where = pin.describe()
+    out = {"value": OPS_PER_STEP * n * 4 / best / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"same step on N=2^{n.bit_length() - 1} elements of the same recipe (fp32, same sparsity, seeds 0/1), "
+                     f"best of 3; oracle/pici_oracle.c single thread pinned to one core, gcc -O2",
+           "host_cores_available": os.cpu_count()}
+    out.update(where)
+    return out
 
 
 def run_ring(pk, name: str, iters: int, device) -> None:
@@ -433,7 +494,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--sweep-iters", type=int, default=7)
+    ap.add_argument("--sweep-iters", type=int, default=20, help="launches per timed CUDA graph (x5 replays)")
     ap.add_argument("--sweep-only", action="store_true",
                     help="time single kernels only (one JSON line per row); filters: --ops --dtypes --sparsities")
     ap.add_argument("--ops", default="compress,decompress,reduce_ss,reduce_sd")
