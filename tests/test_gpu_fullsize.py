@@ -74,11 +74,14 @@ def _check_index(p, dense: torch.Tensor):
     assert int(s_dense.item()) == int(s_A.item())
 
 
-@pytest.mark.parametrize("dtype,sparsity", [("f32", 0.99), ("f32", 0.5), ("f32", 0.9999), ("bf16", 0.99), ("bf16", 0.75)])
-def test_config2_compress_decompress_full_size(mods, dtype, sparsity):
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("sparsity", wl.CONFIG2_SPARSITIES)
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_config2_compress_decompress_full_size(mods, dtype, sparsity, seed):
+    """configs[1] as BASELINE.md S4 states it: all seven sparsities x {fp32, bf16} x seeds 0-4."""
     pk, _ = mods
     n = N_FULL
-    x = wl.sparse_buffer(n, 1.0 - sparsity, seed=wl.stream_seed(0, 0), dtype=dtype, device="cuda")
+    x = wl.sparse_buffer(n, 1.0 - sparsity, seed=wl.stream_seed(seed, 0), dtype=dtype, device="cuda")
     p = pk.alloc_pici(n, pk.F32 if dtype == "f32" else pk.BF16)
     ws = pk.alloc_workspace(n)
     pk.compress(x, p, ws)
@@ -92,7 +95,7 @@ def test_config2_compress_decompress_full_size(mods, dtype, sparsity):
     assert torch.equal(_ibits(back), _ibits(x))            # round trip is the identity (no -0.0 in the recipe)
 
 
-@pytest.mark.parametrize("sparsity", [0.99, 0.9, 0.5])
+@pytest.mark.parametrize("sparsity", wl.CONFIG2_SPARSITIES)
 def test_config2_reductions_full_size(mods, sparsity):
     pk, _ = mods
     n = N_FULL
@@ -169,6 +172,109 @@ def test_config3_ring_reduce_scatter_full_size(mods):
         else:
             assert all(v is not None for v in sw.values())  # 1 - 0.99^5 = 4.9 % > 4 %
     _check_fold_samples(X, res.outputs, n, P, seed=3)
+
+
+def _expected_switch_window(theta: float, n: int, P: int, d0: float = 0.01):
+    """Steps s (0-based; the message of step s carries s + 1 contributions) at which a chunk of n elements with
+    independent Bernoulli(d0) supports may first reach density theta: Eq. 7 gives density
+    1 - (1 - d0)^k after k contributions; 6 standard deviations of the count separate "must" from "may"."""
+    lo = hi = None
+    for s_ in range(P - 1):                     # reduce-scatter sends P - 1 messages per chunk (steps 0 .. P-2)
+        dk = 1.0 - (1.0 - d0) ** (s_ + 1)
+        sd = 6.0 * (dk * (1.0 - dk) / n) ** 0.5
+        if lo is None and dk + sd >= theta:
+            lo = s_
+        if hi is None and dk - sd >= theta:
+            hi = s_
+    return lo, hi                               # None = not before the collective ends
+
+
+@pytest.mark.parametrize("strategy", ["fused", "paper"])
+def test_config3_threshold_sweep_full_size(mods, strategy):
+    """configs[2] as written: theta in {10 .. 90 %} (flat at 99 % sparsity: densities 0.0100 .. 0.0679 never reach
+    10 %), plus the extension {2, 4, 6, 8 %} where the switch does occur; both strategies; switch steps against the
+    fill-in law 1 - 0.99^k (Eq. 7); outputs against the dense left fold in ring order."""
+    pk, ring = mods
+    cfg = wl.config3()
+    X = cfg.buffers(device="cuda")
+    P, n = cfg.ranks, cfg.chunk
+    folds = [_left_fold(X, c, n, P) for c in range(P)]
+    drv = ring.RingDriver(P, n, strategy=strategy)
+    for permille in (20, 40, 60, 80, 100, 200, 300, 400, 500, 600, 700, 800, 900):
+        res = drv.reduce_scatter(X, wl.nnz_switch_from_permille(n, permille))
+        torch.cuda.synchronize()
+        for c in range(P):
+            assert torch.equal(_ibits(res.outputs[c]), _ibits(folds[c])), (permille, c)
+        lo, hi = _expected_switch_window(permille / 1000.0, n, P)
+        for c, got in res.switch_steps("rs").items():
+            if lo is None:
+                assert got is None, (permille, c, got)
+            else:
+                assert got is not None or hi is None, (permille, c, got)
+                if got is not None:
+                    assert lo <= got and (hi is None or got <= hi), (permille, c, got, lo, hi)
+        if permille >= 100:
+            assert all(v is None for v in res.switch_steps("rs").values())
+
+
+@pytest.mark.parametrize("sparsity", wl.CONFIG2_SPARSITIES)
+def test_reduce_ss_full_size_stress(mods, sparsity):
+    """No race tool runs on this pool, so the merge's hand-offs (tickets, mbarrier rings, tagged counts) are
+    exercised the blunt way: N = 2^28, 20 launches per sparsity into DIRTIED outputs, every launch compared in
+    full with the first one, whose result is checked against the dense sum."""
+    pk, _ = mods
+    n = N_FULL
+    d = 1.0 - sparsity
+    x = wl.sparse_buffer(n, d, seed=wl.stream_seed(1, 0), device="cuda")
+    y = wl.sparse_buffer(n, d, seed=wl.stream_seed(1, 1), device="cuda")
+    px, py, ref, out = (pk.alloc_pici(n, pk.F32) for _ in range(4))
+    ws = pk.alloc_workspace(n)
+    pk.compress(x, px, ws)
+    pk.compress(y, py, ws)
+    pk.reduce_ss(px, py, ref, ws)
+    total = x + y
+    total = torch.where(total == 0, torch.zeros((), device="cuda"), total)
+    _check_index(ref, total)
+    back = torch.empty_like(x)
+    pk.decompress(ref, back)
+    assert torch.equal(_ibits(back), _ibits(total))
+    del back, total, x, y
+    T = n // wl.TILE
+    nnz = ref.nnz_host()
+    for rep in range(20):
+        out.B.fill_(-1 - rep); out.I.fill_(-7); out.A[:nnz + 64].fill_(float(rep) + 0.5)
+        pk.reduce_ss(px, py, out, ws)
+        assert torch.equal(out.I[:T + 1], ref.I[:T + 1]), rep
+        assert torch.equal(out.B[:64 * T], ref.B[:64 * T]), rep
+        assert torch.equal(_ibits(out.A[:nnz]), _ibits(ref.A[:nnz])), rep
+
+
+def test_config3_ring_graph_replay_stress(mods):
+    """A config-3 ring reduce-scatter captured into ONE CUDA graph (per-rank streams become parallel branches) and
+    replayed 20 times into dirtied outputs: every replay equals the dense left fold."""
+    pk, ring = mods
+    cfg = wl.config3()
+    X = cfg.buffers(device="cuda")
+    P, n = cfg.ranks, cfg.chunk
+    folds = [_left_fold(X, c, n, P) for c in range(P)]
+    for strategy, permille in (("fused", 400), ("fused", 40), ("paper", 40)):
+        drv = ring.RingDriver(P, n, strategy=strategy)
+        outs = [torch.empty(n, dtype=torch.float32, device="cuda") for _ in range(P)]
+        sw = wl.nnz_switch_from_permille(n, permille)
+        drv.reduce_scatter(X, sw, outputs=outs)            # warm-up (also builds the pooled buffers)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            drv.reduce_scatter(X, sw, outputs=outs)
+        for rep in range(20):
+            for o in outs:
+                o.fill_(float(rep) - 3.0)
+            g.replay()
+            torch.cuda.synchronize()
+            for c in range(P):
+                assert torch.equal(_ibits(outs[c]), _ibits(folds[c])), (strategy, permille, rep, c)
+        del g, drv, outs
+        torch.cuda.empty_cache()
 
 
 def test_config4_ring_all_reduce_full_size(mods):
