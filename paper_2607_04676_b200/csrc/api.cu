@@ -15,7 +15,7 @@ inline uint64_t tiles(uint64_t n) { return (n + kTile - 1) / kTile; }
 inline size_t esize(int dt) { return dt == PICI_F32 ? 4 : 2; }
 inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? PICI_OK : PICI_ERR_CUDA; }
 constexpr uint64_t kMaxN = 1ull << 32;
-const Gate kOpen = {nullptr, 0};
+const Gate kOpen = {nullptr, 0, 0};
 
 int check_pici(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype) {
     if (bad_dtype(dtype)) return PICI_ERR_DTYPE;
@@ -108,7 +108,7 @@ int pici_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_
 int pici_compress_gated(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,
                         uint64_t A_capacity, void *ws, uint64_t ws_bytes, const int32_t *d_gate, int32_t gate_value,
                         void *stream) {
-    return do_compress(dense, n, dtype, B, I, A, A_capacity, ws, ws_bytes, Gate{d_gate, gate_value}, stream);
+    return do_compress(dense, n, dtype, B, I, A, A_capacity, ws, ws_bytes, gate_eq(d_gate, gate_value), stream);
 }
 
 int pici_decompress(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype, void *dense_out,
@@ -118,7 +118,7 @@ int pici_decompress(const uint64_t *B, const uint32_t *I, const void *A, uint64_
 
 int pici_decompress_gated(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype, void *dense_out,
                           const int32_t *d_gate, int32_t gate_value, void *stream) {
-    return do_expand(B, I, A, n, dtype, nullptr, dense_out, 0, DensifyCtl{nullptr, 0, 0, 0}, Gate{d_gate, gate_value},
+    return do_expand(B, I, A, n, dtype, nullptr, dense_out, 0, DensifyCtl{nullptr, 0, 0, 0}, gate_eq(d_gate, gate_value),
                      stream);
 }
 
@@ -129,7 +129,7 @@ int pici_reduce_sd(const uint64_t *B, const uint32_t *I, const void *A, uint64_t
 
 int pici_reduce_sd_out_gated(const uint64_t *B, const uint32_t *I, const void *A, const void *local, uint64_t n,
                              int dtype, void *out, const int32_t *d_gate, int32_t gate_value, void *stream) {
-    return do_expand(B, I, A, n, dtype, local, out, 1, DensifyCtl{nullptr, 0, 0, 0}, Gate{d_gate, gate_value}, stream);
+    return do_expand(B, I, A, n, dtype, local, out, 1, DensifyCtl{nullptr, 0, 0, 0}, gate_eq(d_gate, gate_value), stream);
 }
 
 int pici_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void *Ax, const uint64_t *By, const uint32_t *Iy,
@@ -143,7 +143,7 @@ int pici_reduce_ss_gated(const uint64_t *Bx, const uint32_t *Ix, const void *Ax,
                          void *Ao, uint64_t Ao_capacity, void *ws, uint64_t ws_bytes, const int32_t *d_gate,
                          int32_t gate_value, void *stream) {
     return do_reduce_ss(Bx, Ix, Ax, By, Iy, Ay, n, dtype, Bo, Io, Ao, Ao_capacity, ws, ws_bytes,
-                        Gate{d_gate, gate_value}, stream);
+                        gate_eq(d_gate, gate_value), stream);
 }
 
 int pici_nnz(const uint32_t *I, uint64_t n, uint32_t *d_nnz, void *stream) {
@@ -173,7 +173,7 @@ int pici_maybe_densify_gated(const uint64_t *B, const uint32_t *I, const void *A
                              int32_t gate_value, void *stream) {
     if (d_fmt_out == nullptr || d_fmt_out == d_gate) return PICI_ERR_INVALID_ARG;
     return do_expand(B, I, A, n, dtype, nullptr, dense_out, 0,
-                     DensifyCtl{d_fmt_out, nnz_switch, PICI_FMT_DENSE, PICI_FMT_PICI}, Gate{d_gate, gate_value}, stream);
+                     DensifyCtl{d_fmt_out, nnz_switch, PICI_FMT_DENSE, PICI_FMT_PICI}, gate_eq(d_gate, gate_value), stream);
 }
 
 int pici_dense_add_gated(const void *recv, const void *local, uint64_t n, int dtype, void *out, int32_t *d_fmt_out,
@@ -183,7 +183,7 @@ int pici_dense_add_gated(const void *recv, const void *local, uint64_t n, int dt
     if (n >= kMaxN || (n != 0 && (recv == nullptr || local == nullptr || out == nullptr))) return PICI_ERR_INVALID_ARG;
     if (d_fmt_out != nullptr && d_fmt_out == d_gate) return PICI_ERR_INVALID_ARG;
     if (!aligned(recv, 16) || !aligned(local, 16) || !aligned(out, 16)) return PICI_ERR_ALIGN;
-    return cuda_rc(launch_dense_add(recv, local, n, out, d_fmt_out, Gate{d_gate, gate_value},
+    return cuda_rc(launch_dense_add(recv, local, n, out, d_fmt_out, gate_eq(d_gate, gate_value),
                                     static_cast<cudaStream_t>(stream)));
 }
 
@@ -193,7 +193,7 @@ int pici_dense_copy_gated(const void *src, void *dst, uint64_t n, int dtype, con
     if (n >= kMaxN || (n != 0 && (src == nullptr || dst == nullptr))) return PICI_ERR_INVALID_ARG;
     if (!aligned(src, 16) || !aligned(dst, 16)) return PICI_ERR_ALIGN;
     if (n == 0) return PICI_OK;
-    return cuda_rc(launch_dense_copy(src, dst, n * esize(dtype), Gate{d_gate, gate_value}, static_cast<cudaStream_t>(stream)));
+    return cuda_rc(launch_dense_copy(src, dst, n * esize(dtype), gate_eq(d_gate, gate_value), static_cast<cudaStream_t>(stream)));
 }
 
 int pici_compress_host(const void *h_dense, uint64_t n, int dtype, uint64_t *h_B, uint32_t *h_I, void *h_A,

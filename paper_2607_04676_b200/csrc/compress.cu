@@ -41,13 +41,19 @@ struct CompressCfg<PICI_BF16> {
 
 template <int DT>
 __global__ void __launch_bounds__(kCompressWarps * 32, CompressCfg<DT>::kMinBlocks)
-compress_kernel(const void *__restrict__ dense, uint64_t n, uint64_t *__restrict__ B,
-                uint32_t *__restrict__ I, void *__restrict__ A, void *ws, uint64_t *status,
-                const int32_t *gate, int32_t gate_value) {
+compress_kernel(const Batch<CompressJob> batch) {
     using Cfg = CompressCfg<DT>;
     using Elem = typename Cfg::Elem;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    if (gate_closed(gate, gate_value)) return;
+    const CompressJob &job = batch.job[blockIdx.y];
+    if (gate_closed(job.gate.ptr, job.gate.mask, job.gate.value)) return;
+    const void *__restrict__ dense = job.dense;
+    const uint64_t n = job.n;
+    uint64_t *__restrict__ B = job.B;
+    uint32_t *__restrict__ I = job.I;
+    void *__restrict__ A = job.A;
+    void *const ws = job.ws;
+    uint64_t *const status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes) + kWsAccWords;
     // [ticket, warps that have left] live behind the workspace header; the launch's last warp resets them and
     // advances the epoch, so no launch starts with a memset (status words carry the epoch, pici_common.cuh)
     uint32_t *const ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + kWsCompressTicket);
@@ -266,10 +272,8 @@ uint64_t scan_workspace_bytes(uint64_t n) {
 }
 
 template <int DT>
-static cudaError_t launch_compress_t(const void *dense, uint64_t n, uint64_t *B, uint32_t *I, void *A,
-                                     void *ws, Gate g, cudaStream_t s) {
+static cudaError_t launch_compress_t(const CompressJob *jobs, int count, cudaStream_t s) {
     using Cfg = CompressCfg<DT>;
-    const uint64_t T = (n + kTile - 1) / kTile;
     const size_t smem = (size_t)kCompressWarps * kTile * sizeof(typename Cfg::Elem);
     static bool configured_on[64] = {false};
     bool &configured = configured_on[current_device_slot()];
@@ -278,20 +282,31 @@ static cudaError_t launch_compress_t(const void *dense, uint64_t n, uint64_t *B,
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    uint64_t *status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes) + kWsAccWords;
+    Batch<CompressJob> batch;
+    uint64_t T = 0;
+    for (int j = 0; j < count; ++j) {
+        batch.job[j] = jobs[j];
+        T = max(T, (jobs[j].n + kTile - 1) / kTile);
+    }
     uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
-    const uint64_t cap = (uint64_t)num_sms() * Cfg::kMinBlocks;           // persistent: one resident wave
+    const uint64_t cap = max((uint64_t)num_sms() * Cfg::kMinBlocks / count, (uint64_t)1);   // persistent: one resident wave
     if (blocks > cap) blocks = cap;
-    compress_kernel<DT><<<(unsigned)blocks, kCompressWarps * 32, smem, s>>>(dense, n, B, I, A, ws, status,
-                                                                          g.ptr, g.value);
+    compress_kernel<DT><<<dim3((unsigned)blocks, (unsigned)count), kCompressWarps * 32, smem, s>>>(batch);
     return cudaGetLastError();
+}
+
+// jobs with n == 0 are not supported here (the single entry point handles them)
+cudaError_t launch_compress_batch(const CompressJob *jobs, int count, int dtype, cudaStream_t s) {
+    if (count <= 0) return cudaSuccess;
+    if (count > kMaxBatch) return cudaErrorInvalidValue;
+    return dtype == PICI_F32 ? launch_compress_t<PICI_F32>(jobs, count, s) : launch_compress_t<PICI_BF16>(jobs, count, s);
 }
 
 cudaError_t launch_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,
                             void *ws, Gate g, cudaStream_t s) {
     if (n == 0) return launch_set_u32(I, 0u, g, s);
-    return dtype == PICI_F32 ? launch_compress_t<PICI_F32>(dense, n, B, I, A, ws, g, s)
-                             : launch_compress_t<PICI_BF16>(dense, n, B, I, A, ws, g, s);
+    const CompressJob job = {dense, n, B, I, A, ws, g};
+    return launch_compress_batch(&job, 1, dtype, s);
 }
 
 }  // namespace pici

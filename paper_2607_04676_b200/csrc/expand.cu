@@ -77,14 +77,20 @@ __device__ __forceinline__ ulonglong2 ldg_nc_u64x2(const uint64_t *p) {
 
 template <int DT, int MODE>
 __global__ void __launch_bounds__(kExpandWarps * 32)
-expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, const void *__restrict__ A,
-              uint64_t n, const void *local, void *out, DensifyCtl ctl, const int32_t *gate,
-              int32_t gate_value) {
+expand_kernel(const Batch<ExpandJob> batch) {
     using Elem = typename ExpandCfg<DT>::Elem;
     constexpr uint32_t ES = sizeof(Elem);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t mbar_mem[kExpandWarps];
-    if (gate_closed(gate, gate_value)) return;
+    const ExpandJob &job = batch.job[blockIdx.y];
+    if (gate_closed(job.gate.ptr, job.gate.mask, job.gate.value)) return;
+    const uint64_t *__restrict__ B = job.B;
+    const uint32_t *__restrict__ I = job.I;
+    const void *__restrict__ A = job.A;
+    const uint64_t n = job.n;
+    const void *local = job.local;
+    void *out = job.out;
+    const DensifyCtl ctl = job.ctl;
 
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
     if constexpr (MODE == kModeAdd) {  // in place: the sparse regime belongs to scatter_add_sparse_kernel
@@ -299,10 +305,9 @@ expand_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I, co
 constexpr int kSparseWarps = 8;
 __global__ void __launch_bounds__(kSparseWarps * 32, 5)
 scatter_add_sparse_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I,
-                          const uint32_t *__restrict__ A, uint64_t n, uint32_t *dense, const int32_t *gate,
-                          int32_t gate_value) {
+                          const uint32_t *__restrict__ A, uint64_t n, uint32_t *dense, Gate gate) {
     __shared__ uint16_t lists[kSparseWarps][kSparseListMax];
-    if (gate_closed(gate, gate_value)) return;
+    if (gate_closed(gate.ptr, gate.mask, gate.value)) return;
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
     if (!sparse_regime(I, T)) return;
     const int lane = threadIdx.x & 31;
@@ -369,14 +374,12 @@ cudaError_t launch_scatter_add_sparse(const uint64_t *B, const uint32_t *I, cons
     if (blocks > cap) blocks = cap;
     if (blocks == 0) return cudaSuccess;
     scatter_add_sparse_kernel<<<(unsigned)blocks, kSparseWarps * 32, 0, s>>>(
-        B, I, reinterpret_cast<const uint32_t *>(A), n, reinterpret_cast<uint32_t *>(dense), g.ptr, g.value);
+        B, I, reinterpret_cast<const uint32_t *>(A), n, reinterpret_cast<uint32_t *>(dense), g);
     return cudaGetLastError();
 }
 
 template <int DT, int MODE>
-static cudaError_t launch_expand_t(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n,
-                                   const void *local, void *out, DensifyCtl ctl, Gate g, cudaStream_t s) {
-    const uint64_t T = (n + kTile - 1) / kTile;
+static cudaError_t launch_expand_t(const ExpandJob *jobs, int count, cudaStream_t s) {
     const size_t smem = (size_t)kExpandWarps * ExpandCfg<DT>::kStageBytes;
     static bool configured_on[64] = {false};
     bool &configured = configured_on[current_device_slot()];
@@ -385,28 +388,41 @@ static cudaError_t launch_expand_t(const uint64_t *B, const uint32_t *I, const v
         if (e != cudaSuccess) return e;
         configured = true;
     }
+    Batch<ExpandJob> batch;
+    uint64_t T = 0;
+    bool flag_only = true;
+    for (int j = 0; j < count; ++j) {
+        batch.job[j] = jobs[j];
+        T = max(T, (jobs[j].n + kTile - 1) / kTile);
+        flag_only = flag_only && jobs[j].out == nullptr;
+    }
     uint64_t per_sm = (227u * 1024u) / (smem + 1024);
     if (per_sm > 32) per_sm = 32;
     uint64_t blocks = (T + kExpandWarps - 1) / kExpandWarps;
-    const uint64_t cap = (uint64_t)num_sms() * (per_sm ? per_sm : 1);
+    const uint64_t cap = max((uint64_t)num_sms() * (per_sm ? per_sm : 1) / count, (uint64_t)1);
     if (blocks > cap) blocks = cap;
-    if (blocks == 0) blocks = 1;  // n == 0 with a densify flag still has to write the flag
-    expand_kernel<DT, MODE><<<(unsigned)blocks, kExpandWarps * 32, smem, s>>>(B, I, A, n, local, out, ctl, g.ptr, g.value);
+    if (blocks == 0 || flag_only) blocks = 1;  // n == 0 or no output: only the densify flag is written (by block 0)
+    expand_kernel<DT, MODE><<<dim3((unsigned)blocks, (unsigned)count), kExpandWarps * 32, smem, s>>>(batch);
     return cudaGetLastError();
+}
+
+cudaError_t launch_expand_batch(const ExpandJob *jobs, int count, int dtype, int mode, cudaStream_t s) {
+    if (count <= 0) return cudaSuccess;
+    if (count > kMaxBatch) return cudaErrorInvalidValue;
+    if (mode == kModeAdd) return launch_expand_t<PICI_F32, kModeAdd>(jobs, count, s);
+    return dtype == PICI_F32 ? launch_expand_t<PICI_F32, kModeDecompress>(jobs, count, s)
+                             : launch_expand_t<PICI_BF16, kModeDecompress>(jobs, count, s);
 }
 
 cudaError_t launch_expand(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
                           const void *local, void *out, int mode, DensifyCtl ctl, Gate g, cudaStream_t s) {
     if (n == 0 && ctl.d_flag == nullptr) return cudaSuccess;
-    if (mode == kModeAdd) {
-        if (local == out) {  // in place: the sparse-regime kernel and the streaming kernel pick on the device
-            cudaError_t e = launch_scatter_add_sparse(B, I, A, n, out, g, s);
-            if (e != cudaSuccess) return e;
-        }
-        return launch_expand_t<PICI_F32, kModeAdd>(B, I, A, n, local, out, ctl, g, s);
+    if (mode == kModeAdd && local == out) {  // in place: the sparse-regime kernel and the streaming kernel pick on the device
+        cudaError_t e = launch_scatter_add_sparse(B, I, A, n, out, g, s);
+        if (e != cudaSuccess) return e;
     }
-    return dtype == PICI_F32 ? launch_expand_t<PICI_F32, kModeDecompress>(B, I, A, n, local, out, ctl, g, s)
-                             : launch_expand_t<PICI_BF16, kModeDecompress>(B, I, A, n, local, out, ctl, g, s);
+    const ExpandJob job = {B, I, A, n, local, out, ctl, g};
+    return launch_expand_batch(&job, 1, dtype, mode, s);
 }
 
 }  // namespace pici

@@ -125,6 +125,7 @@ struct MergeArgs {
     uint32_t zero;         // 0, but only the host knows: keeps the ticket's address non-uniform for ptxas, which
                            // otherwise makes the atomic warp-aggregated - with a shuffle that waits for its result
     uint64_t a_limit;      // bytes of Ax / Ay that may be read: (n * 4) & ~15 (capacity >= n elements)
+    Gate gate;
 };
 
 __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
@@ -910,10 +911,11 @@ __device__ __forceinline__ void flusher(const MergeArgs &a, MergeShared &sh, con
 }
 
 __global__ void __launch_bounds__(kMergeThreads, kCtasPerSm)
-reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
+reduce_ss_kernel(const Batch<MergeArgs> batch) {
     extern __shared__ __align__(128) uint32_t pool[];
     __shared__ MergeShared sh;
-    if (gate_closed(gate, gate_value)) return;
+    const MergeArgs &a = batch.job[blockIdx.y];
+    if (gate_closed(a.gate.ptr, a.gate.mask, a.gate.value)) return;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tag = launch_tag(a.hdr);   // this launch's tag for the tile words (pici_common.cuh)
@@ -952,11 +954,9 @@ reduce_ss_kernel(MergeArgs a, const int32_t *gate, int32_t gate_value) {
     }
 }
 
-cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void *Ax, const uint64_t *By,
-                             const uint32_t *Iy, const void *Ay, uint64_t n, uint64_t *Bo, uint32_t *Io,
-                             void *Ao, void *ws, Gate g, cudaStream_t s) {
-    if (n == 0) return launch_set_u32(Io, 0u, g, s);
-    const uint64_t T = (n + kTile - 1) / kTile;
+cudaError_t launch_reduce_ss_batch(const MergeJob *jobs, int count, cudaStream_t s) {
+    if (count <= 0) return cudaSuccess;
+    if (count > kMaxBatch) return cudaErrorInvalidValue;
     const size_t smem = (size_t)kPoolWords * sizeof(uint32_t);
     static bool configured_on[64] = {false};
     bool &configured = configured_on[current_device_slot()];
@@ -965,25 +965,41 @@ cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void 
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    // the block length is chosen on the device.  A chunk of a few thousand tiles does not need the whole GPU:
-    // one CTA per 16 tiles leaves SMs to the other logical ranks' launches of the same ring step
-    uint64_t blocks = (T + kWorkers - 1) / kWorkers;
-    const uint64_t cap = (uint64_t)kCtasPerSm * (uint64_t)num_sms();
+    Batch<MergeArgs> batch;
+    uint64_t Tmax = 0;
+    for (int j = 0; j < count; ++j) {
+        const MergeJob &q = jobs[j];
+        const uint64_t n = q.n, T = (n + kTile - 1) / kTile;
+        Tmax = max(Tmax, T);
+        if ((uint64_t)kWsHeaderBytes + ((uint64_t)kWsAccWords + T) * 8 > scan_workspace_bytes(n)) return cudaErrorInvalidValue;   // cannot happen
+        uint64_t *base = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(q.ws) + kWsHeaderBytes);
+        MergeArgs &a = batch.job[j];
+        a.Bx = q.Bx; a.By = q.By; a.Ix = q.Ix; a.Iy = q.Iy;
+        a.Ax = reinterpret_cast<const uint32_t *>(q.Ax); a.Ay = reinterpret_cast<const uint32_t *>(q.Ay);
+        a.Bo = q.Bo; a.Io = q.Io; a.Ao = reinterpret_cast<uint32_t *>(q.Ao);
+        a.hdr = reinterpret_cast<MergeHeader *>(q.ws);
+        a.blk_acc = base; a.grp_acc = base + kWsBlkWords; a.tile_word = base + kWsAccWords;
+        a.tile_words = (scan_workspace_bytes(n) - kWsHeaderBytes) / 8 - kWsAccWords;
+        a.T = (uint32_t)T;
+        a.zero = 0;
+        a.a_limit = (n * 4) & ~15ull;
+        a.gate = q.gate;
+    }
+    // the block length is chosen on the device.  A chunk of a few thousand tiles does not need the whole GPU, and
+    // the jobs of a batch (the logical ranks of one ring step) share it
+    uint64_t blocks = (Tmax + kWorkers - 1) / kWorkers;
+    const uint64_t cap = max((uint64_t)kCtasPerSm * (uint64_t)num_sms() / count, (uint64_t)1);
     if (blocks > cap) blocks = cap;
-    if ((uint64_t)kWsHeaderBytes + ((uint64_t)kWsAccWords + T) * 8 > scan_workspace_bytes(n)) return cudaErrorInvalidValue;   // cannot happen
-    uint64_t *base = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);
-    MergeArgs a;
-    a.Bx = Bx; a.By = By; a.Ix = Ix; a.Iy = Iy;
-    a.Ax = reinterpret_cast<const uint32_t *>(Ax); a.Ay = reinterpret_cast<const uint32_t *>(Ay);
-    a.Bo = Bo; a.Io = Io; a.Ao = reinterpret_cast<uint32_t *>(Ao);
-    a.hdr = reinterpret_cast<MergeHeader *>(ws);
-    a.blk_acc = base; a.grp_acc = base + kWsBlkWords; a.tile_word = base + kWsAccWords;
-    a.tile_words = (scan_workspace_bytes(n) - kWsHeaderBytes) / 8 - kWsAccWords;
-    a.T = (uint32_t)T;
-    a.zero = 0;
-    a.a_limit = (n * 4) & ~15ull;
-    reduce_ss_kernel<<<(unsigned)blocks, kMergeThreads, smem, s>>>(a, g.ptr, g.value);
+    reduce_ss_kernel<<<dim3((unsigned)blocks, (unsigned)count), kMergeThreads, smem, s>>>(batch);
     return cudaGetLastError();
+}
+
+cudaError_t launch_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void *Ax, const uint64_t *By,
+                             const uint32_t *Iy, const void *Ay, uint64_t n, uint64_t *Bo, uint32_t *Io,
+                             void *Ao, void *ws, Gate g, cudaStream_t s) {
+    if (n == 0) return launch_set_u32(Io, 0u, g, s);
+    const MergeJob job = {Bx, Ix, Ax, By, Iy, Ay, n, Bo, Io, Ao, ws, g};
+    return launch_reduce_ss_batch(&job, 1, s);
 }
 
 }  // namespace pici

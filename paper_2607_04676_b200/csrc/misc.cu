@@ -7,13 +7,13 @@
 
 namespace pici {
 
-__global__ void set_u32_kernel(uint32_t *p, uint32_t v, const int32_t *gate, int32_t gate_value) {
-    if (gate_closed(gate, gate_value)) return;
+__global__ void set_u32_kernel(uint32_t *p, uint32_t v, Gate gate) {
+    if (gate_closed(gate.ptr, gate.mask, gate.value)) return;
     *p = v;
 }
 
 cudaError_t launch_set_u32(uint32_t *p, uint32_t v, Gate g, cudaStream_t s) {
-    set_u32_kernel<<<1, 1, 0, s>>>(p, v, g.ptr, g.value);
+    set_u32_kernel<<<1, 1, 0, s>>>(p, v, g);
     return cudaGetLastError();
 }
 
@@ -77,9 +77,13 @@ cudaError_t launch_nnz_dense(const void *dense, uint64_t n, int dtype, uint32_t 
 }
 
 // out[i] = recv[i] + local[i], one fp32 add each, order "received + local" (C9 #7).
-__global__ void __launch_bounds__(256) dense_add_kernel(const float *recv, const float *local, uint64_t n, float *out,
-                                                        int32_t *d_fmt_out, const int32_t *gate, int32_t gate_value) {
-    if (gate_closed(gate, gate_value)) return;
+__global__ void __launch_bounds__(256) dense_add_kernel(const Batch<DenseAddJob> batch) {
+    const DenseAddJob &job = batch.job[blockIdx.y];
+    if (gate_closed(job.gate.ptr, job.gate.mask, job.gate.value)) return;
+    const float *recv = reinterpret_cast<const float *>(job.recv), *local = reinterpret_cast<const float *>(job.local);
+    float *out = reinterpret_cast<float *>(job.out);
+    const uint64_t n = job.n;
+    int32_t *d_fmt_out = job.d_fmt_out;
     if (d_fmt_out != nullptr && blockIdx.x == 0 && threadIdx.x == 0) *d_fmt_out = PICI_FMT_DENSE;
     const uint64_t nvec = n / 4;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
@@ -105,22 +109,36 @@ __global__ void __launch_bounds__(256) dense_add_kernel(const float *recv, const
         for (uint64_t j = nvec * 4; j < n; ++j) out[j] = __fadd_rn(recv[j], local[j]);
 }
 
-cudaError_t launch_dense_add(const void *recv, const void *local, uint64_t n, void *out, int32_t *d_fmt_out, Gate g,
-                             cudaStream_t s) {
-    const uint64_t nvec = n / 4;
+cudaError_t launch_dense_add_batch(const DenseAddJob *jobs, int count, cudaStream_t s) {
+    if (count <= 0) return cudaSuccess;
+    if (count > kMaxBatch) return cudaErrorInvalidValue;
+    Batch<DenseAddJob> batch;
+    uint64_t nvec = 0;
+    for (int j = 0; j < count; ++j) {
+        batch.job[j] = jobs[j];
+        nvec = max(nvec, jobs[j].n / 4);
+    }
     uint64_t blocks = (nvec + 256 * 2 - 1) / (256 * 2);
-    const uint64_t cap = (uint64_t)num_sms() * 8;
+    const uint64_t cap = max((uint64_t)num_sms() * 8 / count, (uint64_t)1);
     if (blocks > cap) blocks = cap;
     if (blocks == 0) blocks = 1;
-    dense_add_kernel<<<(unsigned)blocks, 256, 0, s>>>(reinterpret_cast<const float *>(recv), reinterpret_cast<const float *>(local),
-                                                      n, reinterpret_cast<float *>(out), d_fmt_out, g.ptr, g.value);
+    dense_add_kernel<<<dim3((unsigned)blocks, (unsigned)count), 256, 0, s>>>(batch);
     return cudaGetLastError();
 }
 
+cudaError_t launch_dense_add(const void *recv, const void *local, uint64_t n, void *out, int32_t *d_fmt_out, Gate g,
+                             cudaStream_t s) {
+    const DenseAddJob job = {recv, local, n, out, d_fmt_out, g};
+    return launch_dense_add_batch(&job, 1, s);
+}
+
 // dst[i] = src[i] (bit copy), gated: a dense message landing in its all-gather slot.
-__global__ void __launch_bounds__(256) dense_copy_kernel(const uint4 *src, uint4 *dst, uint64_t nbytes, const int32_t *gate,
-                                                         int32_t gate_value) {
-    if (gate_closed(gate, gate_value)) return;
+__global__ void __launch_bounds__(256) dense_copy_kernel(const Batch<DenseCopyJob> batch) {
+    const DenseCopyJob &job = batch.job[blockIdx.y];
+    if (gate_closed(job.gate.ptr, job.gate.mask, job.gate.value)) return;
+    const uint4 *src = reinterpret_cast<const uint4 *>(job.src);
+    uint4 *dst = reinterpret_cast<uint4 *>(job.dst);
+    const uint64_t nbytes = job.nbytes;
     const uint64_t nvec = nbytes / 16;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -140,15 +158,26 @@ __global__ void __launch_bounds__(256) dense_copy_kernel(const uint4 *src, uint4
     }
 }
 
-cudaError_t launch_dense_copy(const void *src, void *dst, uint64_t nbytes, Gate g, cudaStream_t s) {
-    const uint64_t nvec = nbytes / 16;
+cudaError_t launch_dense_copy_batch(const DenseCopyJob *jobs, int count, cudaStream_t s) {
+    if (count <= 0) return cudaSuccess;
+    if (count > kMaxBatch) return cudaErrorInvalidValue;
+    Batch<DenseCopyJob> batch;
+    uint64_t nvec = 0;
+    for (int j = 0; j < count; ++j) {
+        batch.job[j] = jobs[j];
+        nvec = max(nvec, jobs[j].nbytes / 16);
+    }
     uint64_t blocks = (nvec + 256 * 4 - 1) / (256 * 4);
-    const uint64_t cap = (uint64_t)num_sms() * 8;
+    const uint64_t cap = max((uint64_t)num_sms() * 8 / count, (uint64_t)1);
     if (blocks > cap) blocks = cap;
     if (blocks == 0) blocks = 1;
-    dense_copy_kernel<<<(unsigned)blocks, 256, 0, s>>>(reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), nbytes,
-                                                       g.ptr, g.value);
+    dense_copy_kernel<<<dim3((unsigned)blocks, (unsigned)count), 256, 0, s>>>(batch);
     return cudaGetLastError();
+}
+
+cudaError_t launch_dense_copy(const void *src, void *dst, uint64_t nbytes, Gate g, cudaStream_t s) {
+    const DenseCopyJob job = {src, dst, nbytes, g};
+    return launch_dense_copy_batch(&job, 1, s);
 }
 
 }  // namespace pici

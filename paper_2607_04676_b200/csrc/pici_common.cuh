@@ -72,8 +72,8 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 }
 
 // ---- gate (include/pici.h "Gating") ------------------------------------------------------------
-__device__ __forceinline__ bool gate_closed(const int32_t *gate, int32_t gate_value) {
-    return gate != nullptr && *reinterpret_cast<const volatile int32_t *>(gate) != gate_value;
+__device__ __forceinline__ bool gate_closed(const int32_t *gate, int32_t mask, int32_t value) {
+    return gate != nullptr && (*reinterpret_cast<const volatile int32_t *>(gate) & mask) != value;
 }
 
 // ---- single-pass device-wide exclusive scan of per-tile counts (Phase 2) ------------------------
