@@ -174,6 +174,69 @@ int pici_decompress_gated(const uint64_t *B, const uint32_t *I, const void *A, u
                           void *dense_out, const int32_t *d_gate, int32_t gate_value, void *stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * Ring engine (a9): SpCCL's sparse ring collectives (PAPER.md:207 all-gather; 219 reduce-scatter and
+ * all-reduce = RS + AG; 227-247 the dense switch and the adaptive policy) over P LOGICAL ranks whose buffers
+ * all live in this GPU's memory - no NCCL, no inter-GPU traffic; a "send" is a pointer hand-off inside the
+ * arena.  Schedule (NCCL's): rank r sends to r + 1 and ends owning chunk r.
+ * A call enqueues the WHOLE collective on `stream` and returns: one launch per kernel family per ring step
+ * (every launch handles all P ranks), every format decision taken on the device.  fp32 only.
+ *
+ * X / shards / out are HOST arrays of P DEVICE pointers (16-byte aligned):
+ *   reduce_scatter: X[r] = rank r's P*chunk elements; out[r] = chunk elements (reduced chunk r).
+ *   all_gather:     shards[r] = chunk elements;       out[r] = P*chunk elements, identical on every rank.
+ *   all_reduce:     X[r] = P*chunk elements;          out[r] = P*chunk elements.
+ * Sums are taken in ring order, acc = received + local: out_c = ((X_{c+1}[c] + X_{c+2}[c]) + ...) + X_c[c].
+ * arena: device scratch of pici_ring_arena_bytes() bytes, 256-byte aligned, cleared ONCE after allocation
+ * (pici_workspace_init) and then reusable by any number of collectives of the same config on one stream.
+ * It also holds the log: per message a format word, the measured nnz (0xFFFFFFFF for a dense send, for which
+ * no count is computed) and, in policy mode, the sparsity the decision was taken on (pici_ring_layout()).
+ * h_launches (host, may be NULL) receives the number of kernel launches enqueued.
+ * Errors: PICI_ERR_INVALID_ARG (NULL, ranks outside 2..16, chunk not a positive multiple of 4096 or >= 2^32,
+ * unknown strategy / decision), PICI_ERR_ALIGN, PICI_ERR_WORKSPACE (arena too small), PICI_ERR_CUDA.
+ * ---------------------------------------------------------------------------------------------- */
+enum { PICI_RING_FUSED = 0,  /* RS step = compress local chunk + sparse+sparse merge (pici_reduce_ss)          */
+       PICI_RING_PAPER = 1   /* RS step = scatter-add into dense + recompress, as PAPER.md:219 has it           */ };
+enum { PICI_RING_DECIDE_MEASURED = 0, /* dense once the measured nnz >= nnz_switch (readings C9 #9/#10)        */
+       PICI_RING_DECIDE_POLICY = 1    /* the paper's policy: Eq. 7 extrapolation, intra / inter / ag thresholds */ };
+
+typedef struct pici_ring_config {
+    int32_t  ranks;            /* P, 2 .. 16                                                                    */
+    int32_t  strategy;         /* PICI_RING_FUSED | PICI_RING_PAPER                                             */
+    int32_t  decision;         /* PICI_RING_DECIDE_MEASURED | PICI_RING_DECIDE_POLICY                           */
+    int32_t  keep_messages;    /* != 0: every message keeps its own slot (tests compare them with the oracle)   */
+    uint64_t chunk;            /* n: elements per chunk, a multiple of 4096                                     */
+    uint64_t nnz_switch_rs;    /* MEASURED: a reduce-scatter message travels dense once nnz >= this             */
+    uint64_t nnz_switch_ag;    /* MEASURED: same for the all-gather's messages (chunk + 1 = never)              */
+    double   intra_thresh;     /* POLICY: dense when the decision sparsity <= threshold of the outgoing link;   */
+    double   inter_thresh;     /*         0.6 / 0.5 for Pici fp32 reduce-scatter                  */
+    double   ag_thresh;        /* POLICY: all-reduce's RS -> AG transition (0.1)                  */
+    int32_t  ranks_per_node;   /* POLICY: ranks r with equal r / ranks_per_node share a node (intra link)       */
+    int32_t  reserved;
+} pici_ring_config;
+
+typedef struct pici_ring_layout_info {   /* byte offsets into the arena */
+    uint64_t records;          /* messages logged: rs_records + ranks                                            */
+    uint64_t rs_records;       /* reduce-scatter: record of (step s < P-1, rank r) = s * P + r                   */
+    uint64_t off_fmt;          /* int32  [records]: PICI_FMT_PICI | PICI_FMT_DENSE; all-gather step 0: rs_records + r */
+    uint64_t off_nnz;          /* uint32 [records]                                                               */
+    uint64_t off_sigma;        /* double [records] (policy mode)                                                 */
+    uint64_t off_messages;     /* message slot k at off_messages + k * message_bytes: B at +0, I at +message_I,
+                                  A at +message_A, the dense form at +message_dense                              */
+    uint64_t message_bytes, message_I, message_A, message_dense;
+    uint64_t off_reduced, reduced_bytes;   /* all-reduce: reduced chunk of rank r at off_reduced + r * reduced_bytes */
+    uint64_t slots;            /* keep_messages: slot = record; else RS (step & 1) * P + r, AG 2 * P + r         */
+} pici_ring_layout_info;
+
+int pici_ring_arena_bytes(const pici_ring_config *cfg, uint64_t *bytes);
+int pici_ring_layout(const pici_ring_config *cfg, pici_ring_layout_info *info);
+int pici_ring_reduce_scatter(const pici_ring_config *cfg, const void *const *X, void *const *out, void *arena,
+                             uint64_t arena_bytes, int *h_launches, void *stream);
+int pici_ring_all_gather(const pici_ring_config *cfg, const void *const *shards, void *const *out, void *arena,
+                         uint64_t arena_bytes, int *h_launches, void *stream);
+int pici_ring_all_reduce(const pici_ring_config *cfg, const void *const *X, void *const *out, void *arena,
+                         uint64_t arena_bytes, int *h_launches, void *stream);
+
+/* ------------------------------------------------------------------------------------------------
  * Host-buffer forms (end-to-end path): h_* are HOST pointers (pinned for full speed), d_* device
  * scratch owned by the caller.  These DO synchronise `stream` before returning.
  * ---------------------------------------------------------------------------------------------- */

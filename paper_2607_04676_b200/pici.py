@@ -26,6 +26,7 @@ EXPORTS = (
     "pici_reduce_ss", "pici_nnz", "pici_nnz_dense", "pici_maybe_densify", "pici_compress_gated",
     "pici_reduce_ss_gated", "pici_maybe_densify_gated", "pici_dense_add_gated", "pici_reduce_sd_out_gated",
     "pici_decompress_gated", "pici_dense_copy_gated", "pici_compress_host", "pici_decompress_host",
+    "pici_ring_arena_bytes", "pici_ring_layout", "pici_ring_reduce_scatter", "pici_ring_all_gather", "pici_ring_all_reduce",
 )
 
 _lib = None
@@ -69,6 +70,11 @@ def lib() -> ctypes.CDLL:
             "pici_dense_copy_gated": ([p, p, u64, ci, p, i32, p], ci),
             "pici_compress_host": ([p, u64, ci, p, p, p, p, p, p, p, p, p, u64, p], ci),
             "pici_decompress_host": ([p, p, p, u64, u64, ci, p, p, p, p, p, p], ci),
+            "pici_ring_arena_bytes": ([p, p], ci),
+            "pici_ring_layout": ([p, p], ci),
+            "pici_ring_reduce_scatter": ([p, p, p, p, u64, p, p], ci),
+            "pici_ring_all_gather": ([p, p, p, p, u64, p, p], ci),
+            "pici_ring_all_reduce": ([p, p, p, p, u64, p, p], ci),
         }
         for name, (args, res) in sig.items():
             f = getattr(L, name)

@@ -1,37 +1,54 @@
-"""Host driver: SpCCL's sparse ring collectives over P LOGICAL ranks held as separate buffers in one
-B200's HBM (BASELINE.json north_star).  No NCCL, no inter-GPU traffic:
-a "send" is a pointer hand-off.  This file is host logic only - every byte of data is touched by
-the libpici_b200 kernels (through `pici`), and every format decision is taken ON THE DEVICE:
+"""Ring collectives over P LOGICAL ranks held as separate buffers in one B200's HBM (BASELINE.json north_star;
+SURVEY.md S8(a) a9, S8(c) C8): a thin binding of the C ring engine (include/pici.h "Ring engine",
+csrc/ring.cu).  No NCCL, no inter-GPU traffic: a "send" is a pointer hand-off inside the engine's arena.
 
-  * each message carries a device-side format word (PICI_FMT_PICI / PICI_FMT_DENSE, the fact the
-    paper's 48-byte header carries);
-  * for every step the driver enqueues both the sparse-path and the dense-path kernels, each gated
-    on the incoming message's format word, so nothing is read back and no stream is synchronised
-    until the caller asks for the log (SURVEY.md S7 hard part 6).
+This file marshals arguments and exposes the engine's log - it enqueues nothing itself.  One call =
+one C call = the whole collective on the current stream: one kernel launch per kernel family per ring step
+(each launch handles all P ranks' jobs), every format decision taken on the device.
 
-Schedule (NCCL's, inherited silently by the paper; S8(c) C8): rank r sends to r+1 and ends owning
-chunk r.  reduce-scatter step 0 encodes chunk (r-1) mod P; at step s rank r receives chunk
-(r-1-s) mod P, forms acc = received + local and, unless it is the last step, re-encodes.
-Two equivalent ways to take the step, both bit-identical to the oracle's messages:
-  strategy="paper": scatter-add the received Pici into a dense scratch (pici_reduce_sd), recompress
-                    it (pici_compress), PAPER.md:219;
-  strategy="fused": compress the local chunk and merge sparse+sparse (pici_reduce_ss), never
-                    touching a dense buffer while the chunk stays sparse (north_star).
-A chunk that reached nnz >= nnz_switch travels dense from then on (pici_maybe_densify, PAPER.md:227;
-once dense it stays dense within the reduce-scatter, C8).
+    drv = RingDriver(P, n, strategy="fused" | "paper", keep_messages=False, policy=None | Policy(...))
+    res = drv.reduce_scatter(X, nnz_switch)          # X[r]: rank r's P*n fp32 elements -> res.outputs[r]: chunk r
+    res = drv.all_gather(shards, nnz_switch=None)    # -> res.outputs[r]: P*n elements, identical on every rank
+    res = drv.all_reduce(X, nnz_switch_rs, nnz_switch_ag)
 
-The P ranks' kernels of one ring step are independent of one another, and a chunk is a few thousand tiles -
-too little to fill 148 SMs from one launch - so with concurrent=True every logical rank enqueues on its own
-CUDA stream and the streams join after every step (SURVEY.md S7 hard part 5).  The whole collective can be
-captured into ONE CUDA graph (the cross-stream events become graph edges): bench.py --ring times both.
+policy=None decides on the MEASURED nnz (a message travels dense once nnz >= nnz_switch, PAPER.md:227 with the
+readings C9 #9/#10); policy=Policy(intra, inter, ag, ranks_per_node) is the paper's adaptive rule (Eq. 7
+extrapolation, link-aware and phase-aware thresholds) and ignores the nnz_switch arguments.
 """
 from __future__ import annotations
 
+import ctypes
 from dataclasses import dataclass, field
 
 import torch
 
 from . import pici as pk
+
+FUSED, PAPER = 0, 1
+MEASURED, POLICY = 0, 1
+NO_COUNT = 0xFFFFFFFF
+
+
+class _Config(ctypes.Structure):
+    _fields_ = [("ranks", ctypes.c_int32), ("strategy", ctypes.c_int32), ("decision", ctypes.c_int32),
+                ("keep_messages", ctypes.c_int32), ("chunk", ctypes.c_uint64), ("nnz_switch_rs", ctypes.c_uint64),
+                ("nnz_switch_ag", ctypes.c_uint64), ("intra_thresh", ctypes.c_double), ("inter_thresh", ctypes.c_double),
+                ("ag_thresh", ctypes.c_double), ("ranks_per_node", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+class _Layout(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_uint64) for k in
+                ("records", "rs_records", "off_fmt", "off_nnz", "off_sigma", "off_messages", "message_bytes", "message_I",
+                 "message_A", "message_dense", "off_reduced", "reduced_bytes", "slots")]
+
+
+@dataclass
+class Policy:
+    """The paper's thresholds (sparsities): PAPER.md:237 intra 0.6 / inter 0.5 (Pici, fp32 RS), :239 ag 0.1."""
+    intra_thresh: float = 0.6
+    inter_thresh: float = 0.5
+    ag_thresh: float = 0.1
+    ranks_per_node: int = 2
 
 
 @dataclass
@@ -46,8 +63,8 @@ class StepRecord:
     step: int
     rank: int
     chunk: int
-    msg: _Msg | None          # buffers holding the message sent at this step (valid until reused)
-    fmt_index: int            # index of its format word in the driver's flag array
+    msg: _Msg | None          # views of the message's slot in the arena (keep_messages only)
+    fmt_index: int            # index of its format word / nnz / decision sparsity in the log arrays
     nnz_index: int
 
 
@@ -55,8 +72,10 @@ class StepRecord:
 class RingResult:
     outputs: list[torch.Tensor]
     records: list[StepRecord] = field(default_factory=list)
-    fmt: torch.Tensor | None = None       # int32 flags, one per record (device)
-    nnz: torch.Tensor | None = None       # int32 measured nnz, one per record (device)
+    fmt: torch.Tensor | None = None       # int32 format words, one per record index (device)
+    nnz: torch.Tensor | None = None       # int32 (uint32 bits) measured nnz; NO_COUNT after a dense send
+    sigma: torch.Tensor | None = None     # float64 decision sparsities (policy mode)
+    launches: int = 0                     # kernel launches the collective enqueued
 
     def formats(self) -> list[str]:
         f = self.fmt.cpu().tolist()
@@ -74,166 +93,102 @@ class RingResult:
         return out
 
 
+def _ptr_array(tensors) -> ctypes.Array:
+    return (ctypes.c_void_p * len(tensors))(*[t.data_ptr() for t in tensors])
+
+
 class RingDriver:
-    """Buffers for P logical ranks with chunk length n (elements, multiple of 4096), fp32."""
+    """Arena + configuration for P logical ranks with chunk length n (elements, multiple of 4096), fp32."""
 
     def __init__(self, ranks: int, chunk: int, device="cuda", strategy: str = "fused", keep_messages: bool = False,
-                 concurrent: bool = True):
+                 policy: Policy | None = None, concurrent: bool = True):
         assert chunk % pk.TILE == 0 and ranks >= 2 and strategy in ("fused", "paper")
-        self.P, self.n, self.device, self.strategy = ranks, chunk, device, strategy
-        self.keep = keep_messages
-        self.streams = [torch.cuda.Stream(device=device) for _ in range(ranks)] if concurrent else None
-        self._ev_main = torch.cuda.Event()
-        self._ev_rank = [torch.cuda.Event() for _ in range(ranks)]
-        P = ranks
-        n_sets = (2 * P) if not keep_messages else None
-        self._pool: list[_Msg] = []
-        self._n_sets = n_sets
-        self._cursor = 0
-        self.local = [pk.alloc_pici(chunk, pk.F32, device) for _ in range(P)] if strategy == "fused" else None
-        self.ws = [pk.alloc_workspace(chunk, device) for _ in range(P)]
-        max_records = 4 * P * P + 4 * P
-        self.fmt = torch.zeros(max_records, dtype=torch.int32, device=device)
-        self.nnz = torch.zeros(max_records, dtype=torch.int32, device=device)
-        if n_sets is not None:
-            for _ in range(n_sets):
-                self._pool.append(self._new_msg())
-
-    def _new_msg(self) -> _Msg:
-        return _Msg(pk.alloc_pici(self.n, pk.F32, self.device), torch.empty(self.n, dtype=torch.float32, device=self.device))
-
-    def _msg(self) -> _Msg:
-        if self._n_sets is None:          # keep every message alive (tests compare them with the oracle's log)
-            m = self._new_msg()
-            self._pool.append(m)
-            return m
-        m = self._pool[self._cursor % self._n_sets]
-        self._cursor += 1
-        return m
+        del concurrent   # the engine batches the ranks of a step into one launch; kept for call compatibility
+        self.P, self.n, self.device, self.strategy, self.keep, self.policy = ranks, chunk, device, strategy, keep_messages, policy
+        self.cfg = _Config(ranks, FUSED if strategy == "fused" else PAPER, MEASURED if policy is None else POLICY,
+                           1 if keep_messages else 0, chunk, chunk + 1, chunk + 1,
+                           policy.intra_thresh if policy else 0.0, policy.inter_thresh if policy else 0.0,
+                           policy.ag_thresh if policy else 0.0, policy.ranks_per_node if policy else 1, 0)
+        L = pk.lib()
+        nbytes = ctypes.c_uint64()
+        pk._check(L.pici_ring_arena_bytes(ctypes.byref(self.cfg), ctypes.byref(nbytes)), "pici_ring_arena_bytes")
+        self.layout = _Layout()
+        pk._check(L.pici_ring_layout(ctypes.byref(self.cfg), ctypes.byref(self.layout)), "pici_ring_layout")
+        self.arena = torch.empty(int(nbytes.value), dtype=torch.uint8, device=device)
+        pk._check(L.pici_workspace_init(self.arena.data_ptr(), self.arena.numel(), pk._stream()), "pici_workspace_init")
+        lay, R = self.layout, int(self.layout.records)
+        self.fmt = self.arena[lay.off_fmt:lay.off_fmt + 4 * R].view(torch.int32)
+        self.nnz = self.arena[lay.off_nnz:lay.off_nnz + 4 * R].view(torch.int32)
+        self.sigma = self.arena[lay.off_sigma:lay.off_sigma + 8 * R].view(torch.float64)
 
     # ------------------------------------------------------------------------------------------
-    def _step(self, body) -> None:
-        """Run body(r) for every rank r: on rank r's own stream (all forked from the current stream, all joined
-        back into it afterwards) when concurrent, else in order on the current stream."""
-        if self.streams is None:
-            for r in range(self.P):
-                body(r)
-            return
-        main = torch.cuda.current_stream(self.device)
-        self._ev_main.record(main)
-        for r in range(self.P):
-            st = self.streams[r]
-            st.wait_event(self._ev_main)
-            with torch.cuda.stream(st):
-                body(r)
-            self._ev_rank[r].record(st)
-        for r in range(self.P):
-            main.wait_event(self._ev_rank[r])
+    def _message(self, slot: int, dense_alias: torch.Tensor | None = None) -> _Msg:
+        lay, n = self.layout, self.n
+        T = n // pk.TILE
+        o = int(lay.off_messages + slot * lay.message_bytes)
+        view = lambda off, nbytes, dt: self.arena[o + off:o + off + nbytes].view(dt)
+        p = pk.Pici(n, pk.F32, view(0, 64 * T * 8, torch.int64), view(int(lay.message_I), (T + 1) * 4, torch.int32),
+                    view(int(lay.message_A), n * 4, torch.float32))
+        return _Msg(p, dense_alias if dense_alias is not None else view(int(lay.message_dense), n * 4, torch.float32))
 
-    def _begin(self) -> RingResult:
-        res = RingResult([], [], self.fmt, self.nnz)
-        return res
-
-    def _record(self, res: RingResult, phase, step, rank, chunk, msg) -> StepRecord:
-        idx = len(res.records)
-        assert idx < self.fmt.numel()
-        rec = StepRecord(phase, step, rank, chunk, msg if self.keep else None, idx, idx)
-        res.records.append(rec)
-        return rec
-
-    def _encode(self, res, phase, step, r, chunk, src_dense: torch.Tensor, nnz_switch: int, copy_dense: bool):
-        """compress + decide on the measured nnz (the oracle's _encode).  If copy_dense the dense form is
-        materialised into the message's own buffer, else the message aliases src_dense."""
-        m = self._msg()
-        rec = self._record(res, phase, step, r, chunk, m)
-        pk.compress(src_dense, m.pici, self.ws[r])
-        pk.nnz(m.pici, self.nnz[rec.nnz_index:rec.nnz_index + 1])
-        f = self.fmt[rec.fmt_index:rec.fmt_index + 1]
-        if copy_dense:
-            pk.maybe_densify(m.pici, nnz_switch, m.dense, f)
+    def _records(self, res: RingResult, phase: str, shards=None) -> None:
+        P = self.P
+        if phase == "rs":
+            for s in range(P - 1):
+                for r in range(P):
+                    idx = s * P + r
+                    res.records.append(StepRecord("rs", s, r, (r - 1 - s) % P, self._message(idx) if self.keep else None, idx, idx))
         else:
-            pk.maybe_densify(m.pici, nnz_switch, None, f)
-            m = _Msg(m.pici, src_dense)
-            rec.msg = m if self.keep else None
-        return m, f
+            for r in range(P):
+                idx = int(self.layout.rs_records) + r
+                # a dense all-gather message aliases the shard itself (no copy is made)
+                msg = self._message(idx, shards[r]) if self.keep else None
+                res.records.append(StepRecord(phase, 0, r, r, msg, idx, idx))
+
+    def _call(self, fn, a, b) -> int:
+        launches = ctypes.c_int()
+        pk._check(fn(ctypes.byref(self.cfg), _ptr_array(a), _ptr_array(b), self.arena.data_ptr(), self.arena.numel(),
+                     ctypes.byref(launches), pk._stream()), fn.__name__)
+        return int(launches.value)
+
+    def _result(self, outs, launches) -> RingResult:
+        return RingResult(outs, [], self.fmt, self.nnz, self.sigma, launches)
 
     # ------------------------------------------------------------------------------------------
-    def reduce_scatter(self, X: list[torch.Tensor], nnz_switch: int, outputs: list[torch.Tensor] | None = None,
-                       res: RingResult | None = None) -> RingResult:
+    def reduce_scatter(self, X: list[torch.Tensor], nnz_switch: int | None = None,
+                       outputs: list[torch.Tensor] | None = None) -> RingResult:
         """X[r]: rank r's N = P*n element fp32 buffer.  Returns outputs[r] = reduced chunk r (n elements)."""
         P, n = self.P, self.n
-        assert len(X) == P and all(x.numel() == P * n and x.dtype == torch.float32 and x.is_cuda for x in X)
-        res = res or self._begin()
+        assert len(X) == P and all(x.numel() == P * n and x.dtype == torch.float32 and x.is_cuda and x.is_contiguous() for x in X)
         outs = outputs or [torch.empty(n, dtype=torch.float32, device=self.device) for _ in range(P)]
-        chunk = lambda r, c: X[r][c * n:(c + 1) * n]
-
-        cur = [None] * P
-
-        def step0(r):                                        # step 0: always compress (PAPER.md:233)
-            c = (r - 1) % P
-            cur[r] = self._encode(res, "rs", 0, r, c, chunk(r, c), nnz_switch, copy_dense=True)
-        self._step(step0)
-
-        for s in range(1, P):
-            nxt = [None] * P
-
-            def step(r, s=s, cur=cur, nxt=nxt):
-                (m_in, f_in) = cur[(r - 1) % P]
-                c = (r - 1 - s) % P
-                loc = chunk(r, c)
-                if s == P - 1:                                # last step: acc is rank r's dense output
-                    pk.reduce_sd_out(m_in.pici, loc, outs[r], gate=f_in, gate_value=pk.FMT_PICI)
-                    pk.dense_add(m_in.dense, loc, outs[r], None, gate=f_in, gate_value=pk.FMT_DENSE)
-                    return
-                m = self._msg()
-                rec = self._record(res, "rs", s, r, c, m)
-                f = self.fmt[rec.fmt_index:rec.fmt_index + 1]
-                if self.strategy == "fused":
-                    pk.compress(loc, self.local[r], self.ws[r], gate=f_in, gate_value=pk.FMT_PICI)
-                    pk.reduce_ss(m_in.pici, self.local[r], m.pici, self.ws[r], gate=f_in, gate_value=pk.FMT_PICI)
-                    pk.maybe_densify(m.pici, nnz_switch, m.dense, f, gate=f_in, gate_value=pk.FMT_PICI)
-                else:
-                    pk.reduce_sd_out(m_in.pici, loc, m.dense, gate=f_in, gate_value=pk.FMT_PICI)
-                    pk.compress(m.dense, m.pici, self.ws[r], gate=f_in, gate_value=pk.FMT_PICI)
-                    pk.maybe_densify(m.pici, nnz_switch, None, f, gate=f_in, gate_value=pk.FMT_PICI)
-                pk.nnz(m.pici, self.nnz[rec.nnz_index:rec.nnz_index + 1])
-                pk.dense_add(m_in.dense, loc, m.dense, f, gate=f_in, gate_value=pk.FMT_DENSE)
-                nxt[r] = (m, f)
-            self._step(step)
-            cur = nxt
-        res.outputs = outs
+        self.cfg.nnz_switch_rs = int(nnz_switch) if nnz_switch is not None else n + 1
+        res = self._result(outs, self._call(pk.lib().pici_ring_reduce_scatter, X, outs))
+        self._records(res, "rs")
         return res
 
-    # ------------------------------------------------------------------------------------------
     def all_gather(self, shards: list[torch.Tensor], nnz_switch: int | None = None,
-                   outputs: list[torch.Tensor] | None = None, res: RingResult | None = None,
-                   phase: str = "ag") -> RingResult:
+                   outputs: list[torch.Tensor] | None = None) -> RingResult:
         """shards[r]: rank r's n-element shard.  outputs[r]: P*n elements, identical on every rank."""
         P, n = self.P, self.n
-        assert len(shards) == P and all(x.numel() == n and x.dtype == torch.float32 and x.is_cuda for x in shards)
-        res = res or self._begin()
+        assert len(shards) == P and all(x.numel() == n and x.dtype == torch.float32 and x.is_cuda and x.is_contiguous() for x in shards)
         outs = outputs or [torch.empty(P * n, dtype=torch.float32, device=self.device) for _ in range(P)]
-        switch = nnz_switch if nnz_switch is not None else n + 1
-        msgs = [None] * P
-
-        def step0(r):                                        # step 0: compress once (PAPER.md:207)
-            msgs[r] = self._encode(res, phase, 0, r, r, shards[r], switch, copy_dense=False)
-            pk.dense_copy(shards[r], outs[r][r * n:(r + 1) * n])          # own slot: plain copy (C9 #12)
-        self._step(step0)
-        for s in range(1, P):
-            def step(r, s=s):
-                c = (r - s) % P                               # forwarded unchanged: still rank c's message
-                m, f = msgs[c]
-                slot = outs[r][c * n:(c + 1) * n]
-                pk.decompress(m.pici, slot, gate=f, gate_value=pk.FMT_PICI)
-                pk.dense_copy(m.dense, slot, gate=f, gate_value=pk.FMT_DENSE)
-            self._step(step)
-        res.outputs = outs
+        self.cfg.nnz_switch_ag = int(nnz_switch) if nnz_switch is not None else n + 1
+        res = self._result(outs, self._call(pk.lib().pici_ring_all_gather, shards, outs))
+        self._records(res, "ag", shards)
         return res
 
-    # ------------------------------------------------------------------------------------------
-    def all_reduce(self, X: list[torch.Tensor], nnz_switch_rs: int, nnz_switch_ag: int) -> RingResult:
+    def all_reduce(self, X: list[torch.Tensor], nnz_switch_rs: int | None = None, nnz_switch_ag: int | None = None,
+                   outputs: list[torch.Tensor] | None = None) -> RingResult:
         """RS, then the ag_thresh decision on each reduced chunk, then AG."""
-        res = self.reduce_scatter(X, nnz_switch_rs)
-        reduced = res.outputs
-        return self.all_gather(reduced, nnz_switch_ag, None, res, phase="ar.ag")
+        P, n = self.P, self.n
+        assert len(X) == P and all(x.numel() == P * n and x.dtype == torch.float32 and x.is_cuda and x.is_contiguous() for x in X)
+        outs = outputs or [torch.empty(P * n, dtype=torch.float32, device=self.device) for _ in range(P)]
+        self.cfg.nnz_switch_rs = int(nnz_switch_rs) if nnz_switch_rs is not None else n + 1
+        self.cfg.nnz_switch_ag = int(nnz_switch_ag) if nnz_switch_ag is not None else n + 1
+        res = self._result(outs, self._call(pk.lib().pici_ring_all_reduce, X, outs))
+        lay = self.layout
+        reduced = [self.arena[lay.off_reduced + r * lay.reduced_bytes:lay.off_reduced + r * lay.reduced_bytes + 4 * n].view(torch.float32)
+                   for r in range(P)]
+        self._records(res, "rs")
+        self._records(res, "ar.ag", reduced)
+        return res

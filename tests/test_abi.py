@@ -92,3 +92,34 @@ def test_sizes_and_calls_reject_bad_arguments_without_touching_the_device():
     assert lib.pici_decompress(a, a, a, n, pici.F32, a + 4, None) == ALIGN
     for code in (0, INVALID, DTYPE, ALIGN, CAPACITY, WORKSPACE, -6, -99):
         assert lib.pici_strerror(code)                                               # always a string, never NULL
+
+
+def test_ring_entry_points_validate_before_any_cuda_call():
+    """pici_ring_* reject bad configurations / pointers on the host (no GPU needed: nothing is launched)."""
+    from paper_2607_04676_b200 import ring
+    lib = pici.lib()
+    INVALID, ALIGN, WORKSPACE = -1, -3, -5
+    good = ring._Config(4, 0, 0, 0, 8192, 8193, 8193, 0.6, 0.5, 0.1, 2, 0)
+    nbytes = ctypes.c_uint64()
+    assert lib.pici_ring_arena_bytes(ctypes.byref(good), ctypes.byref(nbytes)) == 0 and nbytes.value % 256 == 0
+    info = ring._Layout()
+    assert lib.pici_ring_layout(ctypes.byref(good), ctypes.byref(info)) == 0
+    assert info.rs_records == 3 * 4 and info.records == 3 * 4 + 4 and info.slots == 3 * 4     # two RS sets + one AG set
+    keep = ring._Config(4, 0, 0, 1, 8192, 8193, 8193, 0.6, 0.5, 0.1, 2, 0)
+    lib.pici_ring_layout(ctypes.byref(keep), ctypes.byref(info))
+    assert info.slots == info.records
+    for bad in (ring._Config(1, 0, 0, 0, 8192, 0, 0, 0, 0, 0, 1, 0), ring._Config(17, 0, 0, 0, 8192, 0, 0, 0, 0, 0, 1, 0),
+                ring._Config(4, 0, 0, 0, 4097, 0, 0, 0, 0, 0, 1, 0), ring._Config(4, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1, 0)):
+        assert lib.pici_ring_arena_bytes(ctypes.byref(bad), ctypes.byref(nbytes)) == INVALID
+    ptrs = (ctypes.c_void_p * 4)(0x1000, 0x2000, 0x3000, 0x4000)
+    arena = 0x10000
+    for fn in (lib.pici_ring_reduce_scatter, lib.pici_ring_all_gather, lib.pici_ring_all_reduce):
+        assert fn(None, ptrs, ptrs, arena, 1 << 40, None, None) == INVALID
+        assert fn(ctypes.byref(good), None, ptrs, arena, 1 << 40, None, None) == INVALID
+        assert fn(ctypes.byref(good), ptrs, ptrs, None, 1 << 40, None, None) == INVALID
+        assert fn(ctypes.byref(good), ptrs, ptrs, arena + 16, 1 << 40, None, None) == ALIGN
+        assert fn(ctypes.byref(good), ptrs, ptrs, arena, 1024, None, None) == WORKSPACE
+        odd = (ctypes.c_void_p * 4)(0x1000, 0x2004, 0x3000, 0x4000)
+        assert fn(ctypes.byref(good), odd, ptrs, arena, 1 << 40, None, None) == ALIGN
+        strat = ring._Config(4, 7, 0, 0, 8192, 0, 0, 0, 0, 0, 1, 0)
+        assert fn(ctypes.byref(strat), ptrs, ptrs, arena, 1 << 40, None, None) == INVALID

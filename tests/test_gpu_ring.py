@@ -188,3 +188,95 @@ def test_ring_is_cuda_graph_capturable(mods):
         torch.cuda.synchronize()
         for r in range(cfg.ranks):
             assert np.array_equal(_u32(res.outputs[r]), want_out[r].view(np.uint32))
+
+
+# ---------------------------------------------------------------------------------------------------
+# The paper's adaptive policy on the device against
+# oracle/ring_oracle.py ring_*_policy: formats, counts, decision sparsities (fp64, bit for bit) and every message.
+# ---------------------------------------------------------------------------------------------------
+def _check_policy_records(pk, res, log: ro.RingLog):
+    fmts = res.formats()
+    nnz = res.nnz.cpu().numpy().view(np.uint32)
+    sigma = res.sigma.cpu().numpy()
+    for rec, f in zip(res.records, fmts):
+        e = log.at(rec.phase, rec.step, rec.rank)
+        key = (rec.phase, rec.step, rec.rank)
+        assert e.chunk == rec.chunk and e.fmt == f, (key, e.fmt, f)
+        assert float(sigma[rec.fmt_index]) == e.extrapolated_sparsity, (key, sigma[rec.fmt_index], e.extrapolated_sparsity)
+        assert int(nnz[rec.nnz_index]) == (e.nnz if e.nnz is not None else 0xFFFFFFFF), key
+        if rec.msg is None or e.msg is None:
+            continue
+        if e.fmt == "pici":
+            B, I, A = rec.msg.pici.to_host()
+            w = e.msg.pici
+            assert np.array_equal(I[:w.I.size], w.I) and np.array_equal(B[:w.B.size], w.B) and np.array_equal(A, w.A), key
+        else:
+            assert np.array_equal(_u32(rec.msg.dense), e.msg.dense.view(np.uint32)), key
+
+
+def _disjoint_inputs(P=4, n=16384):
+    """tests/golden/policy_sandwich_p4.txt: rank r holds a nonzero exactly where i mod 8 == r."""
+    i = np.arange(P * n)
+    return [np.where(i % 8 == r, (1.0 + 0.25 * r + (i % 97) / 128.0).astype(np.float32), np.float32(0.0)).astype(np.float32)
+            for r in range(P)]
+
+
+@pytest.mark.parametrize("strategy", ["fused", "paper"])
+def test_policy_worked_example_sandwich(mods, strategy):
+    """The hand-derived trace: a dense send sandwiched between sparse ones, re-calibrated counts."""
+    pk, ring = mods
+    Xh = _disjoint_inputs()
+    pol = ro.Policy(0.8, 0.6, 0.1, 2)
+    want, log, _, _ = ro.ring_reduce_scatter_policy(Xh, pol)
+    drv = ring.RingDriver(4, 16384, strategy=strategy, keep_messages=True, policy=ring.Policy(0.8, 0.6, 0.1, 2))
+    res = drv.reduce_scatter([torch.from_numpy(x).cuda() for x in Xh])
+    torch.cuda.synchronize()
+    _check_policy_records(pk, res, log)
+    assert [f for rec, f in zip(res.records, res.formats()) if rec.chunk == 0] == ["pici", "dense", "pici"]
+    for r in range(4):
+        assert np.array_equal(_u32(res.outputs[r]), want[r].view(np.uint32))
+
+
+@pytest.mark.parametrize("strategy", ["fused", "paper"])
+@pytest.mark.parametrize("P,rpn,intra,inter,ag", [(4, 2, 0.6, 0.5, 0.1), (8, 2, 0.93, 0.2, 0.85), (8, 4, 0.9, 0.99, 0.5),
+                                                  (3, 2, 0.0, 0.0, 0.0), (2, 1, 1.0, 1.0, 1.0), (8, 2, 0.95, 0.9, 0.7)])
+def test_policy_collectives_message_by_message(mods, strategy, P, rpn, intra, inter, ag):
+    pk, ring = mods
+    cfg = wl.RingConfig("small", P, P * 5 * wl.TILE, 0.02, 0.03, "normal", 1.0, 11 + P)
+    Xh = [b.numpy() for b in cfg.buffers()]
+    Xd = [torch.from_numpy(x).cuda() for x in Xh]
+    n = cfg.chunk
+    pol = ro.Policy(intra, inter, ag, rpn)
+    want, log, _, _ = ro.ring_reduce_scatter_policy(Xh, pol)
+    drv = ring.RingDriver(P, n, strategy=strategy, keep_messages=True, policy=ring.Policy(intra, inter, ag, rpn))
+    res = drv.reduce_scatter(Xd)
+    torch.cuda.synchronize()
+    _check_policy_records(pk, res, log)
+    fold = ro.reduce_scatter_definition(Xh)
+    for r in range(P):
+        assert np.array_equal(_u32(res.outputs[r]), want[r].view(np.uint32))
+        assert np.array_equal(_u32(res.outputs[r]), fold[r].view(np.uint32))
+    # all-reduce: the ag_thresh decision and the gathered result
+    want_ar, log_ar = ro.ring_all_reduce_policy(Xh, pol)
+    res = drv.all_reduce(Xd)
+    torch.cuda.synchronize()
+    _check_policy_records(pk, res, log_ar)
+    for r in range(P):
+        assert np.array_equal(_u32(res.outputs[r]), want_ar[r].view(np.uint32))
+
+
+def test_ring_engine_launch_count_and_reuse(mods):
+    """One launch per kernel family per ring step, whatever P is; the arena is reusable without clearing."""
+    pk, ring = mods
+    for P in (4, 8):
+        cfg = _small(P, 4, 0.05, seed=2)
+        Xd = [b.cuda() for b in cfg.buffers()]
+        drv = ring.RingDriver(P, cfg.chunk, strategy="fused")
+        sw = wl.nnz_switch_from_permille(cfg.chunk, 120)
+        first = drv.reduce_scatter(Xd, sw)
+        assert first.launches == 3 + 5 * (P - 2) + 2                 # step 0: 3, middle steps: 5, last step: 2
+        ref = [o.clone() for o in first.outputs]
+        for _ in range(3):
+            again = drv.reduce_scatter(Xd, sw)
+            torch.cuda.synchronize()
+            assert all(torch.equal(a.view(torch.int32), b.view(torch.int32)) for a, b in zip(again.outputs, ref))
