@@ -416,69 +416,93 @@ def run_cpu_baseline(n: int, density: float) -> dict:
     return out
 
 
-def run_ring(pk, name: str, iters: int, device) -> None:
+def _timed_collective(fn, iters: int):
+    """(median ms of eager enqueues, median ms of CUDA-graph replays of the same enqueues, result)"""
+    fn()                                   # warm-up
+    torch.cuda.synchronize()
+
+    def med(run):
+        ts = []
+        for _ in range(iters):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); run(); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        ts.sort()
+        return ts[len(ts) // 2]
+
+    eager = med(fn)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        res = fn()
+    g.replay()
+    torch.cuda.synchronize()
+    graph_ms = med(g.replay)
+    return eager, graph_ms, res
+
+
+RING_CASES = {
+    "config3": [("reduce_scatter", st, pm) for st in ("fused", "paper") for pm in (400, 80, 40, 20)],
+    "config4": [("all_reduce", st, pm) for st in ("fused", "paper") for pm in (400, 200, 100)],
+    "config5": [("all_gather", "fused", 900), ("all_reduce", "fused", 400), ("all_reduce", "paper", 400)],
+}
+
+
+def run_ring(pk, name: str, iters: int, device, cases=None) -> list[dict]:
     """Ring collectives of configs[2..4] on P logical ranks in one HBM: local-compute time of
-    the whole collective (CUDA events around the driver's enqueues, pointer hand-offs cost nothing) and the step
-    at which each chunk switched to dense.  One JSON line per (collective, strategy, threshold)."""
+    the whole collective - one C call, CUDA events around it; pointer hand-offs cost nothing - eager and as a
+    CUDA-graph replay, the launches it enqueued and the step at which each chunk switched to dense."""
     from paper_2607_04676_b200 import ring
     cfg = {"config3": wl.config3, "config4": wl.config4, "config5": lambda: wl.config5(0)}[name]()
     X = cfg.buffers(device=device)
     P, n = cfg.ranks, cfg.chunk
     dense_bytes = P * P * n * 4
-
-    def timed(fn):
-        """(median ms of eager enqueues, median ms of CUDA-graph replays of the same enqueues, result)"""
-        fn()                                   # warm-up (also builds the pooled buffers)
-        torch.cuda.synchronize()
-
-        def med(run):
-            ts = []
-            for _ in range(iters):
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record(); run(); b.record()
-                torch.cuda.synchronize()
-                ts.append(a.elapsed_time(b))
-            ts.sort()
-            return ts[len(ts) // 2]
-
-        eager = med(fn)
-        graph_ms = None
-        try:                                   # the whole collective as ONE graph launch: no per-kernel host cost
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g):
-                res = fn()
-            g.replay()
-            torch.cuda.synchronize()
-            graph_ms = med(g.replay)
-        except Exception as e:                 # report, do not hide
-            res = fn()
-            graph_ms = f"capture failed: {type(e).__name__}: {e}"[:160]
-        torch.cuda.synchronize()
-        return eager, graph_ms, res
-
-    if name == "config3":
-        cases = [("reduce_scatter", st, pm) for st in ("fused", "paper") for pm in (400, 80, 40, 20)]
-    elif name == "config4":
-        cases = [("all_reduce", st, pm) for st in ("fused", "paper") for pm in (400, 200, 100)]
-    else:
-        cases = [("all_gather", "fused", 900), ("all_reduce", "fused", 400), ("all_reduce", "paper", 400)]
-    for coll, strategy, permille in cases:
+    rows = []
+    for coll, strategy, permille in (cases or RING_CASES[name]):
         drv = ring.RingDriver(P, n, device=device, strategy=strategy)
         sw = wl.nnz_switch_from_permille(n, permille)
         if coll == "reduce_scatter":
-            ms, gms, res = timed(lambda: drv.reduce_scatter(X, sw))
+            outs = [torch.empty(n, dtype=torch.float32, device=device) for _ in range(P)]
+            ms, gms, res = _timed_collective(lambda: drv.reduce_scatter(X, sw, outputs=outs), iters)
         elif coll == "all_reduce":
-            ms, gms, res = timed(lambda: drv.all_reduce(X, sw, wl.nnz_switch_from_permille(n, 900)))
+            outs = [torch.empty(P * n, dtype=torch.float32, device=device) for _ in range(P)]
+            ms, gms, res = _timed_collective(lambda: drv.all_reduce(X, sw, wl.nnz_switch_from_permille(n, 900), outputs=outs), iters)
         else:
-            ms, gms, res = timed(lambda: drv.all_gather([X[r][r * n:(r + 1) * n] for r in range(P)]))
+            outs = [torch.empty(P * n, dtype=torch.float32, device=device) for _ in range(P)]
+            shards = [X[r][r * n:(r + 1) * n] for r in range(P)]
+            ms, gms, res = _timed_collective(lambda: drv.all_gather(shards, outputs=outs), iters)
         steps = res.switch_steps("rs") if coll != "all_gather" else {}
-        print(json.dumps({"config": name, "collective": coll, "strategy": strategy, "theta_permille": permille,
-                          "ranks": P, "chunk": n, "ms_eager": round(ms, 3),
-                          "ms_cuda_graph": round(gms, 3) if isinstance(gms, float) else gms,
-                          "dense_equiv_gbs": round(dense_bytes / (gms if isinstance(gms, float) else ms) / 1e6, 1),   # P ranks x N x 4 bytes
-                          "switch_step_per_chunk": [steps.get(c) for c in range(P)] if steps else None}), flush=True)
-        del drv, res
+        rows.append({"config": name, "collective": coll, "strategy": strategy, "theta_permille": permille, "ranks": P,
+                     "chunk": n, "ms_eager": round(ms, 3), "ms_cuda_graph": round(gms, 3), "launches": res.launches,
+                     "dense_equiv_gbs": round(dense_bytes / gms / 1e6, 1),      # P ranks x N x 4 bytes / graph time
+                     "switch_step_per_chunk": [steps.get(c) for c in range(P)] if steps else None})
+        del drv, res, outs
         torch.cuda.empty_cache()
+    return rows
+
+
+def run_policy_sweep(pk, iters: int, device, density: float = 0.05, ranks_per_node: int = 2) -> list[dict]:
+    """Fig. 2's analogue on logical ranks: reduce-scatter under the paper's policy, P = 8 ranks
+    as 4 "nodes" of 2, N = 2^26 per rank, initial sparsity 95 % (density 0.337 after 8 contributions), every pair of
+    intra_thresh x inter_thresh in 0.1 .. 0.9.  There is no link here, so the time is the LOCAL COMPUTE of the
+    collective: it shows what each switching rule costs in kernels, not what it saves on a wire."""
+    from paper_2607_04676_b200 import ring
+    cfg = wl.config3(density)
+    X = cfg.buffers(device=device)
+    P, n = cfg.ranks, cfg.chunk
+    outs = [torch.empty(n, dtype=torch.float32, device=device) for _ in range(P)]
+    rows = []
+    for strategy in ("fused", "paper"):
+        for intra in range(1, 10):
+            for inter in range(1, 10):
+                drv = ring.RingDriver(P, n, device=device, strategy=strategy,
+                                      policy=ring.Policy(intra / 10.0, inter / 10.0, 0.1, ranks_per_node))
+                _, gms, res = _timed_collective(lambda: drv.reduce_scatter(X, outputs=outs), iters)
+                f = res.formats()
+                rows.append({"strategy": strategy, "intra_thresh": intra / 10.0, "inter_thresh": inter / 10.0,
+                             "ms_cuda_graph": round(gms, 3), "dense_sends": sum(1 for v in f if v == "dense"), "sends": len(f)})
+                del drv, res
+    return rows
 
 
 def main():
@@ -502,6 +526,9 @@ def main():
     ap.add_argument("--sparsities", default="")
     ap.add_argument("--ring", default="", choices=["", "config3", "config4", "config5"],
                     help="time the ring collectives of that config on P logical ranks (one JSON line per case)")
+    ap.add_argument("--policy-sweep", action="store_true",
+                    help="reduce-scatter under the paper's policy for every intra x inter threshold pair (Fig. 2 analogue)")
+    ap.add_argument("--no-rings", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -523,7 +550,13 @@ def main():
     density = 1.0 - args.sparsity
     peak, peak_src = measured_peak()
     if args.ring:
-        return run_ring(pk, args.ring, max(3, args.sweep_iters), device)
+        for r in run_ring(pk, args.ring, 7, device):
+            print(json.dumps(r), flush=True)
+        return
+    if args.policy_sweep:
+        for r in run_policy_sweep(pk, 5, device):
+            print(json.dumps(r), flush=True)
+        return
     if args.sweep_only:   # kernel-by-kernel timing (also the program the single-kernel ncu captures run)
         sp = tuple(float(v) for v in args.sparsities.split(",")) if args.sparsities else None
         for r in run_sweep(pk, n, peak, args.sweep_iters, device, tuple(args.dtypes.split(",")), sp, tuple(args.ops.split(","))):
@@ -617,6 +650,11 @@ def main():
         del hp
         torch.cuda.empty_cache()
         out["sweep"] = run_sweep(pk, n, peak, args.sweep_iters, device)
+    if not args.no_rings and world == 1:    # configs[2..4]: the collectives' local-compute time (graph replay and eager)
+        out["rings"] = (run_ring(pk, "config3", 5, device, [("reduce_scatter", "fused", 400), ("reduce_scatter", "fused", 40),
+                                                             ("reduce_scatter", "paper", 400)]) +
+                        run_ring(pk, "config4", 5, device, [("all_reduce", "fused", 400), ("all_reduce", "fused", 200)]) +
+                        run_ring(pk, "config5", 5, device, [("all_gather", "fused", 900), ("all_reduce", "fused", 400)]))
     if not args.no_cpu and world == 1:
         out["cpu_baseline"] = run_cpu_baseline(args.cpu_n, density)
     print(json.dumps(out))
