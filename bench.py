@@ -328,6 +328,14 @@ def run_sweep(pk, n: int, peak: float, launches: int, device, dtypes=("f32", "bf
                 row("reduce_sd", [lambda S=S: pk.reduce_sd(S["px"], S["y"]) for S in sets],
                     mean([bytes_reduce_sd(n, S["nx"], sect) for S in sets]),
                     {"touched_sector_frac": round(sect / (n / 8), 4), "alg_bytes_element_level": int(elem)})
+                if mean([S["nx"] for S in sets]) <= 224 * (n // TILE):
+                    # read-modify-write regime: what the memory system gives for the bare access pattern - the same
+                    # dense[i] += v on the same index sets, one thread per index, nothing else (pici_probe_random_rmw)
+                    for S in sets:
+                        S["idx"] = torch.nonzero(S["x"]).flatten().to(torch.int32)
+                    pms, _ = graph_time([lambda S=S: pk.probe_random_rmw(S["idx"], S["y"]) for S in sets], launches)
+                    rows[-1]["rmw_probe_ms"] = round(pms, 4)
+                    rows[-1]["speed_vs_rmw_probe"] = round(pms / rows[-1]["ms"], 3)   # > 1: faster than the bare stream
             del sets
             torch.cuda.empty_cache()
     return rows

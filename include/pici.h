@@ -236,6 +236,12 @@ int pici_ring_all_gather(const pici_ring_config *cfg, const void *const *shards,
 int pici_ring_all_reduce(const pici_ring_config *cfg, const void *const *X, void *const *out, void *arena,
                          uint64_t arena_bytes, int *h_launches, void *stream);
 
+/* Measurement aid, not part of the path: dense_inout[d_idx[i]] += 1.0f for i < m (d_idx: m DISTINCT uint32
+ * indices < n on the device), one thread per index, through the same gather instruction as reduce_sd's
+ * read-modify-write regime.  bench.py times it on the index set of a sparse buffer to report what the memory
+ * system gives for that access pattern (the "irregular memory access" of PAPER.md:237) beside reduce_sd. */
+int pici_probe_random_rmw(const uint32_t *d_idx, uint64_t m, void *dense_inout, uint64_t n, void *stream);
+
 /* ------------------------------------------------------------------------------------------------
  * Host-buffer forms (end-to-end path): h_* are HOST pointers (pinned for full speed), d_* device
  * scratch owned by the caller.  These DO synchronise `stream` before returning.

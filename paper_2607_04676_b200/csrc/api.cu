@@ -196,6 +196,13 @@ int pici_dense_copy_gated(const void *src, void *dst, uint64_t n, int dtype, con
     return cuda_rc(launch_dense_copy(src, dst, n * esize(dtype), gate_eq(d_gate, gate_value), static_cast<cudaStream_t>(stream)));
 }
 
+int pici_probe_random_rmw(const uint32_t *d_idx, uint64_t m, void *dense_inout, uint64_t n, void *stream) {
+    if (m != 0 && (d_idx == nullptr || dense_inout == nullptr)) return PICI_ERR_INVALID_ARG;
+    if (n >= kMaxN) return PICI_ERR_INVALID_ARG;
+    if (!aligned(d_idx, 4) || !aligned(dense_inout, 16)) return PICI_ERR_ALIGN;
+    return cuda_rc(launch_probe_rmw(d_idx, m, dense_inout, static_cast<cudaStream_t>(stream)));
+}
+
 int pici_compress_host(const void *h_dense, uint64_t n, int dtype, uint64_t *h_B, uint32_t *h_I, void *h_A,
                        uint64_t *h_nnz, void *d_dense, uint64_t *d_B, uint32_t *d_I, void *d_A, void *ws,
                        uint64_t ws_bytes, void *stream) {

@@ -111,6 +111,7 @@ struct DenseCopyJob {
 cudaError_t launch_dense_copy_batch(const DenseCopyJob *jobs, int count, cudaStream_t s);
 cudaError_t launch_dense_copy(const void *src, void *dst, uint64_t nbytes, Gate g, cudaStream_t s);
 cudaError_t launch_set_u32(uint32_t *p, uint32_t v, Gate g, cudaStream_t s);
+cudaError_t launch_probe_rmw(const uint32_t *idx, uint64_t m, void *dense, cudaStream_t s);
 
 template <class Job>
 struct Batch {

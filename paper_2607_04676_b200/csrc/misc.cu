@@ -180,4 +180,27 @@ cudaError_t launch_dense_copy(const void *src, void *dst, uint64_t nbytes, Gate 
     return launch_dense_copy_batch(&job, 1, s);
 }
 
+// ---- measurement aid: the bare random read-modify-write stream (include/pici.h pici_probe_random_rmw) -------------
+// dense[idx[i]] = dense[idx[i]] + 1.0f for i < m, one thread per index, the gather through the same
+// ld.global.L2::64B instruction reduce_sd's sparse regime uses, nothing else: what the memory system gives for
+// this access pattern, against which bench.py reports reduce_sd's read-modify-write regime.
+__global__ void __launch_bounds__(256) probe_rmw_kernel(const uint32_t *__restrict__ idx, uint64_t m, uint32_t *dense) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += stride) {
+        uint32_t *p = dense + idx[i];
+        uint32_t v;
+        asm volatile("ld.global.L2::64B.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+        *p = __float_as_uint(__fadd_rn(__uint_as_float(v), 1.0f));
+    }
+}
+
+cudaError_t launch_probe_rmw(const uint32_t *idx, uint64_t m, void *dense, cudaStream_t s) {
+    if (m == 0) return cudaSuccess;
+    uint64_t blocks = (m + 255) / 256;
+    const uint64_t cap = (uint64_t)num_sms() * 8;
+    if (blocks > cap) blocks = cap;
+    probe_rmw_kernel<<<(unsigned)blocks, 256, 0, s>>>(idx, m, reinterpret_cast<uint32_t *>(dense));
+    return cudaGetLastError();
+}
+
 }  // namespace pici

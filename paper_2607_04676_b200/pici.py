@@ -26,7 +26,7 @@ EXPORTS = (
     "pici_reduce_ss", "pici_nnz", "pici_nnz_dense", "pici_maybe_densify", "pici_compress_gated",
     "pici_reduce_ss_gated", "pici_maybe_densify_gated", "pici_dense_add_gated", "pici_reduce_sd_out_gated",
     "pici_decompress_gated", "pici_dense_copy_gated", "pici_compress_host", "pici_decompress_host",
-    "pici_ring_arena_bytes", "pici_ring_layout", "pici_ring_reduce_scatter", "pici_ring_all_gather", "pici_ring_all_reduce",
+    "pici_probe_random_rmw", "pici_ring_arena_bytes", "pici_ring_layout", "pici_ring_reduce_scatter", "pici_ring_all_gather", "pici_ring_all_reduce",
 )
 
 _lib = None
@@ -70,6 +70,7 @@ def lib() -> ctypes.CDLL:
             "pici_dense_copy_gated": ([p, p, u64, ci, p, i32, p], ci),
             "pici_compress_host": ([p, u64, ci, p, p, p, p, p, p, p, p, p, u64, p], ci),
             "pici_decompress_host": ([p, p, p, u64, u64, ci, p, p, p, p, p, p], ci),
+            "pici_probe_random_rmw": ([p, u64, p, u64, p], ci),
             "pici_ring_arena_bytes": ([p, p], ci),
             "pici_ring_layout": ([p, p], ci),
             "pici_ring_reduce_scatter": ([p, p, p, p, u64, p, p], ci),
@@ -266,6 +267,15 @@ def dense_copy(src: torch.Tensor, dst: torch.Tensor, stream=None, gate=None, gat
     _check(lib().pici_dense_copy_gated(_p(src), _p(dst), dst.numel(), _DT[dst.dtype], _p(gate), gate_value,
                                        _stream(stream)), "pici_dense_copy_gated")
     return dst
+
+
+def probe_random_rmw(idx: torch.Tensor, dense_inout: torch.Tensor, stream=None) -> torch.Tensor:
+    """Measurement aid (pici_probe_random_rmw): dense_inout[idx[i]] += 1 for distinct int32 indices idx."""
+    _dev(idx, dense_inout)
+    assert idx.dtype == torch.int32 and idx.is_contiguous() and dense_inout.dtype == torch.float32
+    _check(lib().pici_probe_random_rmw(_p(idx), idx.numel(), _p(dense_inout), dense_inout.numel(), _stream(stream)),
+           "pici_probe_random_rmw")
+    return dense_inout
 
 
 @dataclass

@@ -295,3 +295,16 @@ def test_host_end_to_end_forms(pk):
     back = torch.empty(n).pin_memory()
     pk.decompress_host(h, back, scratch, d_dense)
     assert np.array_equal(_bits(back), po.decompress(want))
+
+
+def test_probe_random_rmw_adds_one_at_the_indices(pk):
+    """The measurement aid bench.py times beside reduce_sd (pici_probe_random_rmw): dense[idx[i]] += 1.0f."""
+    n = 5 * wl.TILE + 17
+    x = wl.sparse_buffer(n, 0.01, seed=3)
+    idx = torch.nonzero(x).flatten().to(torch.int32).cuda()
+    d = wl.sparse_buffer(n, 0.5, seed=4)
+    got = d.cuda()
+    pk.probe_random_rmw(idx, got)
+    want = d.clone()
+    want[idx.cpu().long()] += 1.0
+    assert torch.equal(got.cpu().view(torch.int32), want.view(torch.int32))
