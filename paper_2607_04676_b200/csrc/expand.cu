@@ -303,73 +303,114 @@ expand_kernel(const Batch<ExpandJob> batch) {
 // no two threads touch the same element.  A tile with more than kSparseListMax values (rare here:
 // the regime is chosen from the average) is walked lane by lane without the list.
 constexpr int kSparseWarps = 8;
+constexpr uint32_t kSparseGroup = 8;   // tiles whose index entries a warp fetches at once
+constexpr uint32_t kSparseRowMajorNnz = 112;   // tiles with at least this many values get a row-major list
 __global__ void __launch_bounds__(kSparseWarps * 32, 5)
 scatter_add_sparse_kernel(const uint64_t *__restrict__ B, const uint32_t *__restrict__ I,
                           const uint32_t *__restrict__ A, uint64_t n, uint32_t *dense, Gate gate) {
-    __shared__ uint16_t lists[kSparseWarps][kSparseListMax];
+    // per warp: the tile's touched elements as a list in ROW-MAJOR (address) order - dense position and index into
+    // the tile's run of A - so that the 32 lanes of a gather touch ascending, neighbouring addresses
+    __shared__ uint16_t lists[kSparseWarps][kSparseListMax], alists[kSparseWarps][kSparseListMax];
     if (gate_closed(gate.ptr, gate.mask, gate.value)) return;
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
     if (!sparse_regime(I, T)) return;
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    uint16_t *list = lists[warp];
+    uint16_t *list = lists[warp], *alist = alists[warp];
+    const uint32_t ngroups = (T + kSparseGroup - 1) / kSparseGroup;
     const uint32_t stride = gridDim.x * kSparseWarps;
-    uint32_t t = blockIdx.x * kSparseWarps + warp;
-    // lanes 0 and 1 hold I[t], I[t+1] of the NEXT tile (prefetched one iteration ahead)
-    uint32_t inext = (t < T && lane < 2) ? __ldg(I + t + lane) : 0u;
-    for (; t < T; t += stride) {
-        const uint32_t seg = __shfl_sync(kFull, inext, 0);
-        const uint32_t tile_nnz = __shfl_sync(kFull, inext, 1) - seg;
-        if (t + stride < T && lane < 2) inext = __ldg(I + t + stride + lane);
-        if (tile_nnz == 0) continue;
-        const ulonglong2 w = ldg_nc_u64x2(B + (size_t)t * kSide + 2 * lane);
-        const uint32_t cnt0 = __popcll(w.x), cnt1 = __popcll(w.y);
-        const uint32_t excl = warp_incl_scan(cnt0 + cnt1, lane) - cnt0 - cnt1;
-        const uint32_t *Au = A + seg;
-        uint32_t *Du = dense + (size_t)t * kTile;
-        if (tile_nnz > kSparseListMax) {   // outlier tile: every lane walks its own two columns
-            uint32_t k = excl;
-            for (uint64_t u = w.x; u; u &= u - 1) {
-                const uint32_t i = (__ffsll((long long)u) - 1) * kSide + 2 * lane;
-                Du[i] = __float_as_uint(__fadd_rn(__uint_as_float(Du[i]), __uint_as_float(Au[k++])));
+    const unsigned lt = (1u << lane) - 1u;
+    for (uint32_t g = blockIdx.x * kSparseWarps + warp; g < ngroups; g += stride) {
+        // index entries of the group's tiles in one request; empty tiles cost nothing more
+        const uint32_t t0 = g * kSparseGroup;
+        const uint32_t ie = __ldg(I + min(t0 + (uint32_t)lane, T));           // lanes 0 .. kSparseGroup
+        const uint32_t tn = __shfl_down_sync(kFull, ie, 1) - ie;               // lane j < group: values of tile t0 + j
+        unsigned todo = __ballot_sync(kFull, (uint32_t)lane < kSparseGroup && t0 + lane < T && tn != 0u);
+        ulonglong2 wn = make_ulonglong2(0, 0);
+        if (todo) wn = ldg_nc_u64x2(B + (size_t)(t0 + __ffs(todo) - 1) * kSide + 2 * lane);
+        while (todo) {
+            const uint32_t j = __ffs(todo) - 1;
+            todo &= todo - 1;
+            const uint32_t t = t0 + j;
+            const uint32_t seg = __shfl_sync(kFull, ie, j), tile_nnz = __shfl_sync(kFull, tn, j);
+            const ulonglong2 w = wn;
+            if (todo) wn = ldg_nc_u64x2(B + (size_t)(t0 + __ffs(todo) - 1) * kSide + 2 * lane);   // the next tile's words
+            const uint32_t cnt0 = __popcll(w.x), cnt1 = __popcll(w.y);
+            const uint32_t excl = warp_incl_scan(cnt0 + cnt1, lane) - cnt0 - cnt1;
+            const uint32_t *Au = A + seg;
+            uint32_t *Du = dense + (size_t)t * kTile;
+            if (tile_nnz > kSparseListMax) {   // outlier tile: every lane walks its own two columns
+                uint32_t k = excl;
+                for (uint64_t u = w.x; u; u &= u - 1) {
+                    const uint32_t i = (__ffsll((long long)u) - 1) * kSide + 2 * lane;
+                    Du[i] = __float_as_uint(__fadd_rn(__uint_as_float(Du[i]), __uint_as_float(Au[k++])));
+                }
+                for (uint64_t u = w.y; u; u &= u - 1) {
+                    const uint32_t i = (__ffsll((long long)u) - 1) * kSide + 2 * lane + 1;
+                    Du[i] = __float_as_uint(__fadd_rn(__uint_as_float(Du[i]), __uint_as_float(Au[k++])));
+                }
+                continue;
             }
-            for (uint64_t u = w.y; u; u &= u - 1) {
-                const uint32_t i = (__ffsll((long long)u) - 1) * kSide + 2 * lane + 1;
-                Du[i] = __float_as_uint(__fadd_rn(__uint_as_float(Du[i]), __uint_as_float(Au[k++])));
-            }
-            continue;
-        }
-        {
-            uint32_t k = excl;
-            for (uint64_t u = w.x; u; u &= u - 1) list[k++] = (uint16_t)((__ffsll((long long)u) - 1) * kSide + 2 * lane);
-            for (uint64_t u = w.y; u; u &= u - 1) list[k++] = (uint16_t)((__ffsll((long long)u) - 1) * kSide + 2 * lane + 1);
-        }
-        __syncwarp();
-        for (uint32_t b0 = 0; b0 < tile_nnz; b0 += 128) {
-            uint32_t av[4], dv[4], ix[4];
+            // ---- the list.  Few values: every lane walks its own two columns (A order; the gathers are far apart
+            // anyway).  Many: row by row, so that a gather's 32 lanes touch neighbouring addresses ---------------------
+            if (tile_nnz < kSparseRowMajorNnz) {
+                uint32_t k = excl;
+                for (uint64_t u = w.x; u; u &= u - 1) {
+                    list[k] = (uint16_t)((__ffsll((long long)u) - 1) * kSide + 2 * lane);
+                    alist[k] = (uint16_t)k;
+                    ++k;
+                }
+                for (uint64_t u = w.y; u; u &= u - 1) {
+                    list[k] = (uint16_t)((__ffsll((long long)u) - 1) * kSide + 2 * lane + 1);
+                    alist[k] = (uint16_t)k;
+                    ++k;
+                }
+            } else {
+                uint32_t k0 = excl, k1 = excl + cnt0, pos = 0;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t jj = b0 + 32 * j + lane;
-                if (jj < tile_nnz) {
-                    ix[j] = list[jj];
-                    av[j] = ldg_stream_u32(Au + jj);
-                    dv[j] = ld_gather_u32(Du + ix[j]);
+                for (int h = 0; h < 2; ++h) {
+                    const uint32_t x = h ? (uint32_t)(w.x >> 32) : (uint32_t)w.x, y = h ? (uint32_t)(w.y >> 32) : (uint32_t)w.y;
+                    uint32_t rows = __reduce_or_sync(kFull, x | y);
+                    while (rows) {
+                        const uint32_t r = __ffs(rows) - 1;
+                        rows &= rows - 1;
+                        const bool b0 = (x >> r) & 1u, b1 = (y >> r) & 1u;
+                        const unsigned m0 = __ballot_sync(kFull, b0), m1 = __ballot_sync(kFull, b1);
+                        const uint32_t at = pos + __popc(m0 & lt) + __popc(m1 & lt);
+                        const uint32_t e = (32u * h + r) * kSide + 2 * lane;
+                        if (b0) { list[at] = (uint16_t)e; alist[at] = (uint16_t)k0++; }
+                        if (b1) { list[at + (b0 ? 1u : 0u)] = (uint16_t)(e + 1); alist[at + (b0 ? 1u : 0u)] = (uint16_t)k1++; }
+                        pos += __popc(m0) + __popc(m1);
+                    }
                 }
             }
+            __syncwarp();
+            for (uint32_t b0 = 0; b0 < tile_nnz; b0 += 128) {
+                uint32_t av[4], dv[4], ix[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t jj = b0 + 32 * j + lane;
-                if (jj < tile_nnz) Du[ix[j]] = __float_as_uint(__fadd_rn(__uint_as_float(dv[j]), __uint_as_float(av[j])));
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t jj = b0 + 32 * q + lane;
+                    if (jj < tile_nnz) {
+                        ix[q] = list[jj];
+                        av[q] = __ldg(Au + alist[jj]);
+                        dv[q] = ld_gather_u32(Du + ix[q]);
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t jj = b0 + 32 * q + lane;
+                    if (jj < tile_nnz) Du[ix[q]] = __float_as_uint(__fadd_rn(__uint_as_float(dv[q]), __uint_as_float(av[q])));
+                }
             }
+            __syncwarp();   // the list is rebuilt by the next tile
         }
-        __syncwarp();   // the list is rebuilt by the next tile
     }
 }
 
 cudaError_t launch_scatter_add_sparse(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, void *dense,
                                       Gate g, cudaStream_t s) {
     const uint64_t T = (n + kTile - 1) / kTile;
-    uint64_t blocks = (T + kSparseWarps - 1) / kSparseWarps;
+    uint64_t blocks = ((T + kSparseGroup - 1) / kSparseGroup + kSparseWarps - 1) / kSparseWarps;
     const uint64_t cap = (uint64_t)num_sms() * 5;
     if (blocks > cap) blocks = cap;
     if (blocks == 0) return cudaSuccess;
