@@ -33,6 +33,12 @@
  *   - Sizes: B holds 64*T words and I holds T+1 entries even when n % 4096 != 0; A (and Ao) must
  *     have capacity >= n elements - the worst case, mirroring the paper's enlarged FIFOs
  *      - so no device-side overflow can occur.
+ *   - A Pici object handed to decompress / reduce_sd / reduce_ss / maybe_densify must be one that pici_compress
+ *     or pici_reduce_ss produced (or a bit-identical copy): the kernels trust that B, I and A agree with one
+ *     another (popcount of a tile's words == I[t+1] - I[t] <= 4096); an inconsistent object is undefined
+ *     behaviour on the device, not an error code.
+ *   - Thread safety: calls may be made from several host threads (one stream and one workspace per thread); the
+ *     only shared state is a per-device "kernel attributes set" flag, kept in atomics.
  *   - Limits: 0 <= n < 2^32 (I is 32-bit).  n == 0 is valid: I[0] = 0 is written.
  *   - dtype: PICI_F32 or PICI_BF16 for compress / decompress / nnz / maybe_densify;
  *     reductions (reduce_sd, reduce_ss, dense_add) are PICI_F32 only (PICI_ERR_DTYPE otherwise).

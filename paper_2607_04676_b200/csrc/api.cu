@@ -59,6 +59,8 @@ int do_reduce_ss(const uint64_t *Bx, const uint32_t *Ix, const void *Ax, const u
     if (!aligned(ws, 16)) return PICI_ERR_ALIGN;
     if (Ao_capacity < n) return PICI_ERR_CAPACITY;
     if (n != 0 && (ws == nullptr || ws_bytes < scan_workspace_bytes(n))) return PICI_ERR_WORKSPACE;
+    // "Outputs must not alias inputs": the merge reads X and Y while it writes O
+    if (n != 0 && (Bo == Bx || Bo == By || Io == Ix || Io == Iy || Ao == Ax || Ao == Ay)) return PICI_ERR_INVALID_ARG;
     return cuda_rc(launch_reduce_ss(Bx, Ix, Ax, By, Iy, Ay, n, Bo, Io, Ao, ws, g, static_cast<cudaStream_t>(stream)));
 }
 
@@ -209,6 +211,9 @@ int pici_compress_host(const void *h_dense, uint64_t n, int dtype, uint64_t *h_B
     if (bad_dtype(dtype)) return PICI_ERR_DTYPE;
     if (h_I == nullptr || h_nnz == nullptr || (n != 0 && (h_dense == nullptr || h_B == nullptr || h_A == nullptr)))
         return PICI_ERR_INVALID_ARG;
+    if (n >= kMaxN || d_I == nullptr || (n != 0 && (d_dense == nullptr || d_B == nullptr || d_A == nullptr))) return PICI_ERR_INVALID_ARG;
+    if (!aligned(d_dense, 16) || !aligned(d_B, 16) || !aligned(d_A, 16) || !aligned(d_I, 4) || !aligned(ws, 16)) return PICI_ERR_ALIGN;
+    if (n != 0 && (ws == nullptr || ws_bytes < scan_workspace_bytes(n))) return PICI_ERR_WORKSPACE;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const uint64_t T = tiles(n);
     if (n != 0 && cudaMemcpyAsync(d_dense, h_dense, n * esize(dtype), cudaMemcpyHostToDevice, s) != cudaSuccess)
@@ -234,6 +239,8 @@ int pici_decompress_host(const uint64_t *h_B, const uint32_t *h_I, const void *h
     if (bad_dtype(dtype)) return PICI_ERR_DTYPE;
     if (h_I == nullptr || nnz > n || (n != 0 && (h_B == nullptr || h_dense_out == nullptr)) || (nnz != 0 && h_A == nullptr))
         return PICI_ERR_INVALID_ARG;
+    if (n >= kMaxN || d_I == nullptr || (n != 0 && (d_dense == nullptr || d_B == nullptr || d_A == nullptr))) return PICI_ERR_INVALID_ARG;
+    if (!aligned(d_dense, 16) || !aligned(d_B, 16) || !aligned(d_A, 16) || !aligned(d_I, 4)) return PICI_ERR_ALIGN;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const uint64_t T = tiles(n);
     if (cudaMemcpyAsync(d_I, h_I, (T + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, s) != cudaSuccess) return PICI_ERR_CUDA;

@@ -15,6 +15,8 @@
 //     which is then written to A with coalesced stores.
 #include <cuda_bf16.h>
 
+#include <atomic>
+
 #include "launch.h"
 #include "pici_common.cuh"
 #include "../../include/pici.h"
@@ -253,16 +255,17 @@ compress_kernel(const Batch<CompressJob> batch) {
 }
 
 int num_sms() {
-    static int cached[64] = {0};
+    static std::atomic<int> cached[64];
     int dev = 0;
     cudaGetDevice(&dev);
     if (dev < 0 || dev >= 64) dev = 0;
-    if (cached[dev] == 0) {
-        int v = 0;
+    int v = cached[dev].load(std::memory_order_relaxed);
+    if (v == 0) {
         cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
-        cached[dev] = v > 0 ? v : 148;
+        if (v <= 0) v = 148;
+        cached[dev].store(v, std::memory_order_relaxed);
     }
-    return cached[dev];
+    return v;
 }
 
 // Scratch for the scans (layout: pici_common.cuh): header, reduce_ss's accumulators, one word per tile.
@@ -275,12 +278,12 @@ template <int DT>
 static cudaError_t launch_compress_t(const CompressJob *jobs, int count, cudaStream_t s) {
     using Cfg = CompressCfg<DT>;
     const size_t smem = (size_t)kCompressWarps * kTile * sizeof(typename Cfg::Elem);
-    static bool configured_on[64] = {false};
-    bool &configured = configured_on[current_device_slot()];
-    if (!configured) {
+    static std::atomic<bool> configured_on[64];   // one-time setup per device; doing it twice is harmless
+    std::atomic<bool> &configured = configured_on[current_device_slot()];
+    if (!configured.load(std::memory_order_acquire)) {
         cudaError_t e = cudaFuncSetAttribute(compress_kernel<DT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured.store(true, std::memory_order_release);
     }
     Batch<CompressJob> batch;
     uint64_t T = 0;

@@ -23,6 +23,8 @@
 //     with every load of the tile in flight before the first store (sector-granular traffic,
 //     SURVEY.md S7 #4).
 // The next tile's words and I[t] are prefetched into registers while the current tile is processed.
+#include <atomic>
+
 #include "launch.h"
 #include "pici_common.cuh"
 #include "../../include/pici.h"
@@ -422,12 +424,12 @@ cudaError_t launch_scatter_add_sparse(const uint64_t *B, const uint32_t *I, cons
 template <int DT, int MODE>
 static cudaError_t launch_expand_t(const ExpandJob *jobs, int count, cudaStream_t s) {
     const size_t smem = (size_t)kExpandWarps * ExpandCfg<DT>::kStageBytes;
-    static bool configured_on[64] = {false};
-    bool &configured = configured_on[current_device_slot()];
-    if (!configured) {
+    static std::atomic<bool> configured_on[64];   // one-time setup per device; doing it twice is harmless
+    std::atomic<bool> &configured = configured_on[current_device_slot()];
+    if (!configured.load(std::memory_order_acquire)) {
         cudaError_t e = cudaFuncSetAttribute(expand_kernel<DT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured.store(true, std::memory_order_release);
     }
     Batch<ExpandJob> batch;
     uint64_t T = 0;

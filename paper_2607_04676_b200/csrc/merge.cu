@@ -46,6 +46,8 @@
 //     finish, which also resets the ticket: stale words of earlier launches never match the tag, so
 //     nothing has to be cleared between launches (the workspace must have been zeroed ONCE,
 //     pici_workspace_init).
+#include <atomic>
+
 #include "launch.h"
 #include "pici_common.cuh"
 #include "../../include/pici.h"
@@ -958,12 +960,12 @@ cudaError_t launch_reduce_ss_batch(const MergeJob *jobs, int count, cudaStream_t
     if (count <= 0) return cudaSuccess;
     if (count > kMaxBatch) return cudaErrorInvalidValue;
     const size_t smem = (size_t)kPoolWords * sizeof(uint32_t);
-    static bool configured_on[64] = {false};
-    bool &configured = configured_on[current_device_slot()];
-    if (!configured) {
+    static std::atomic<bool> configured_on[64];   // one-time setup per device; doing it twice is harmless
+    std::atomic<bool> &configured = configured_on[current_device_slot()];
+    if (!configured.load(std::memory_order_acquire)) {
         cudaError_t e = cudaFuncSetAttribute(reduce_ss_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured.store(true, std::memory_order_release);
     }
     Batch<MergeArgs> batch;
     uint64_t Tmax = 0;

@@ -20,9 +20,11 @@ def world() -> tuple[int, int]:
 
 
 def rank_seeds(config_seed: int, rank: int, k: int) -> list[int]:
-    """k distinct stream seeds for this rank: rank r of a config with seed S uses S*1000 + r (workloads.py);
-    replica `rank` shifts the config seed so no two replicas share a stream."""
-    return [(config_seed + rank) * 1000 + j for j in range(k)]
+    """k distinct stream seeds for replica `rank` of a config with seed S.  Logical rank j of the config uses
+    stream S*1000 + j (workloads.py, j < 999); replica r > 0 moves to its own block of 1 000 000 seeds, so replica 1
+    of seed 0 can never equal replica 0 of seed 1 (replica 0 keeps the config's own streams)."""
+    assert 0 <= config_seed < 1000 and 0 <= k < 999
+    return [rank * 1_000_000 + config_seed * 1000 + j for j in range(k)]
 
 
 def max_over_ranks(value: float, device="cpu") -> float:

@@ -94,6 +94,35 @@ def test_sizes_and_calls_reject_bad_arguments_without_touching_the_device():
         assert lib.pici_strerror(code)                                               # always a string, never NULL
 
 
+def test_reduce_ss_rejects_aliased_outputs_and_host_forms_check_their_scratch():
+    """include/pici.h: "Outputs must not alias inputs" (pici_reduce_ss) and the *_host calls' device scratch
+    pointers are checked on the host, before any CUDA call."""
+    lib = pici.lib()
+    INVALID, ALIGN, WORKSPACE = -1, -3, -5
+    n = 8192
+    ws_bytes = ctypes.c_uint64()
+    assert lib.pici_sizes(n, pici.F32, None, None, None, ctypes.byref(ws_bytes)) == 0
+    a, b, c, w = 0x10000, 0x20000, 0x30000, 0x40000              # fake, 16-aligned "device pointers"
+    big = 1 << 40
+    ok_args = lambda Bo, Io, Ao: (a, a + 0x1000, a + 0x2000, b, b + 0x1000, b + 0x2000, n, pici.F32, Bo, Io, Ao, n, w, big, None)
+    assert lib.pici_reduce_ss(*ok_args(a, c + 0x1000, c + 0x2000)) == INVALID          # Bo == Bx
+    assert lib.pici_reduce_ss(*ok_args(c, b + 0x1000, c + 0x2000)) == INVALID          # Io == Iy
+    assert lib.pici_reduce_ss(*ok_args(c, c + 0x1000, a + 0x2000)) == INVALID          # Ao == Ax
+    h = (ctypes.c_uint64 * 4)()                                                          # any host memory
+    hp, nnz = ctypes.addressof(h), ctypes.c_uint64()
+    host = lambda d_dense, d_B, d_I, d_A, ws, wsb: lib.pici_compress_host(hp, n, pici.F32, hp, hp, hp, ctypes.byref(nnz),
+                                                                          d_dense, d_B, d_I, d_A, ws, wsb, None)
+    assert host(None, a, b, c, w, big) == INVALID
+    assert host(a, None, b, c, w, big) == INVALID
+    assert host(a, b, None, c, w, big) == INVALID
+    assert host(a + 4, b, c, c + 0x1000, w, big) == ALIGN
+    assert host(a, b, c, c + 0x1000, w, 16) == WORKSPACE
+    back = lambda d_B, d_I, d_A, d_dense: lib.pici_decompress_host(hp, hp, hp, 1, n, pici.F32, hp, d_B, d_I, d_A, d_dense, None)
+    assert back(None, a, b, c) == INVALID
+    assert back(a, b, c, None) == INVALID
+    assert back(a, b + 2, c, w) == ALIGN
+
+
 def test_ring_entry_points_validate_before_any_cuda_call():
     """pici_ring_* reject bad configurations / pointers on the host (no GPU needed: nothing is launched)."""
     from paper_2607_04676_b200 import ring

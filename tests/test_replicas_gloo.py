@@ -54,3 +54,7 @@ def test_single_process_is_identity():
     assert replicas.max_over_ranks(3.5) == 3.5
     assert replicas.whole_job_throughput(10.0, 5.0) == (2000.0, 5.0)
     assert replicas.rank_seeds(0, 0, 2) == [wl.stream_seed(0, 0), wl.stream_seed(0, 1)]
+    # no two (config seed, replica) pairs share a stream: replica 1 of seed 0 is not replica 0 of seed 1
+    seen = [tuple(replicas.rank_seeds(S, r, 8)) for S in range(6) for r in range(8)]
+    flat = [v for t in seen for v in t]
+    assert len(set(flat)) == len(flat)
