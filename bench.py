@@ -236,6 +236,9 @@ def touched_sectors_f32(mask_dense: torch.Tensor) -> int:
     return int((mask_dense[:n8].view(-1, 8) != 0).any(dim=1).sum().item())
 
 
+NO_GRAPH = False      # --no-graph: time eager launches with events (the form the ncu captures profile)
+
+
 def graph_time(fns, launches: int, replays: int = 5, warm: int = 5):
     """Per-launch time of a kernel with no host cost inside the timed region: `launches` calls - call i uses
     fns[i % len(fns)], i.e. the buffer sets are rotated so that nothing is re-read from L2 - are captured into ONE
@@ -245,6 +248,15 @@ def graph_time(fns, launches: int, replays: int = 5, warm: int = 5):
         for f in fns:
             f()
     torch.cuda.synchronize()
+    if NO_GRAPH:
+        ts = []
+        for i in range(launches):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fns[i % len(fns)](); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        ts.sort()
+        return ts[len(ts) // 2], ts[0]
     st = torch.cuda.Stream()
     g = torch.cuda.CUDAGraph()
     with torch.cuda.stream(st):
@@ -537,9 +549,12 @@ def main():
     ap.add_argument("--policy-sweep", action="store_true",
                     help="reduce-scatter under the paper's policy for every intra x inter threshold pair (Fig. 2 analogue)")
     ap.add_argument("--no-rings", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="sweep rows: eager launches timed one by one (for ncu captures)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    global NO_GRAPH
+    NO_GRAPH = args.no_graph
     if args.impl == "reference":
         return run_reference(args)
 
