@@ -1,0 +1,497 @@
+// coo.cu - the COO variant (include/pici_coo.h): flat 32-bit index + fp32 value per
+// nonzero, ascending index, structure of arrays, nnz in a device word.
+//
+// Layout of the work on B200.  The unit is the same 4096-element block Pici calls a tile (here just a contiguous
+// index range [4096 t, 4096 t + 4096)), one warp per block:
+//   * compress: the block sits in 128 registers per lane (32 rows of 128 elements, lane l holds elements
+//     128 i + 4 l .. + 3 of row i: every row is one coalesced 512-byte request, all 32 in flight at once).  The
+//     output order of COO is the input order, so the compaction offset inside a block is a running, warp-uniform
+//     row base plus a popcount of four ballots: count and compaction are ONE pass into a shared-memory stage
+//     (idx, val).  The block's count is published right after it; the device-wide exclusive scan is the same
+//     single-pass decoupled look-back as pici_compress (pici_common.cuh), deferred behind the next block (two
+//     stage buffers per warp), and the flush is coalesced.  A block with more entries than the stage holds (density
+//     above 25 %, not a COO regime) takes its look-back at once and writes from registers;
+//   * decompress / merge find a block's index range in `off` (off[t] = first entry with idx >= 4096 t), built by a
+//     streaming pre-pass over idx (what Pici's I gives for free); decompress assembles the block in shared memory and
+//     writes every dense byte once; the merge scatters X then Y into a shared-memory block with a candidate
+//     bitmap, re-applies the predicate to the sums and emits survivors in ascending order behind a look-back;
+//   * reduce_sd is the bare read-modify-write of the touched elements.
+#include <atomic>
+
+#include "launch.h"
+#include "pici_common.cuh"
+#include "../../include/pici.h"
+#include "../../include/pici_coo.h"
+
+namespace pici {
+
+constexpr int kCooWarps = 4;
+constexpr uint32_t kCooStage = 1024;                 // entries a stage buffer holds before a block goes direct
+constexpr uint32_t kCooStageWords = kCooStage + 128; // + one row of slack (the check is per row)
+
+struct CooWs {            // views into the caller's workspace (layout: coo_workspace_bytes)
+    void *hdr;            // WsHeader + ticket / exit counter (pici_common.cuh)
+    uint64_t *status;     // [T] tagged look-back words
+    uint32_t *excl;       // [T + 1] exclusive prefix per block (scratch the look-back writes)
+    uint32_t *offx, *offy;// [T + 1] each
+};
+
+static uint64_t round16(uint64_t b) { return (b + 15) & ~15ull; }
+uint64_t coo_workspace_bytes(uint64_t n) {
+    const uint64_t T = (n + kTile - 1) / kTile;
+    return scan_workspace_bytes(n) + 3 * round16((T + 1) * 4);
+}
+static CooWs coo_ws(void *ws, uint64_t n) {
+    const uint64_t T = (n + kTile - 1) / kTile;
+    unsigned char *b = reinterpret_cast<unsigned char *>(ws);
+    CooWs w;
+    w.hdr = ws;
+    w.status = reinterpret_cast<uint64_t *>(b + kWsHeaderBytes) + kWsAccWords;
+    unsigned char *tail = b + scan_workspace_bytes(n);
+    w.excl = reinterpret_cast<uint32_t *>(tail);
+    w.offx = reinterpret_cast<uint32_t *>(tail + round16((T + 1) * 4));
+    w.offy = reinterpret_cast<uint32_t *>(tail + 2 * round16((T + 1) * 4));
+    return w;
+}
+
+// The launch's last warp resets the ticket pair and advances the epoch (as pici_compress does).
+__device__ __forceinline__ void coo_leave(void *ws, uint32_t *ticket, uint32_t tag, uint64_t *status, uint32_t T,
+                                          uint32_t warps, int lane) {
+    uint32_t last = 0;
+    if (lane == 0) {
+        __threadfence();
+        last = atomicAdd(ticket + 1, 1u) + 1u == warps;
+    }
+    if (__shfl_sync(kFull, last, 0)) {
+        if (lane == 0) {
+            ticket[0] = 0;
+            ticket[1] = 0;
+        }
+        finish_epoch(ws, tag, status, T, lane);
+    }
+}
+
+// ================================================ compress ================================================
+struct CooCompressArgs {
+    const uint32_t *dense;
+    uint64_t n;
+    uint32_t *idx, *val, *d_nnz;
+    CooWs ws;
+};
+
+__global__ void __launch_bounds__(kCooWarps * 32, 3) coo_compress_kernel(const CooCompressArgs a) {
+    extern __shared__ __align__(16) uint32_t coo_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // per warp: two buffers of (idx[kCooStageWords], val[kCooStageWords])
+    uint32_t *const stage = coo_smem + (size_t)warp * 4 * kCooStageWords;
+    uint32_t *const ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(a.ws.hdr) + kWsCompressTicket);
+    const uint32_t tag = launch_tag(a.ws.hdr);
+    const uint64_t n = a.n;
+    const uint32_t T = (uint32_t)((n + kTile - 1) / kTile), Tfull = (uint32_t)(n / kTile);
+    const uint32_t lt = (1u << lane) - 1u;
+
+    uint4 v[32];
+    auto load_block = [&](uint32_t tt) {
+        const uint32_t *base = a.dense + (size_t)tt * kTile + 4 * lane;
+        if (tt < Tfull) {
+#pragma unroll
+            for (int i = 0; i < 32; ++i) v[i] = ldg_nc_u4(reinterpret_cast<const uint4 *>(base + 128 * i));
+        } else {   // ragged last block: elements >= n are zeros
+            const uint64_t e0 = (uint64_t)tt * kTile + 4 * lane;
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+                const uint64_t e = e0 + 128 * i;
+                uint4 x = make_uint4(0u, 0u, 0u, 0u);
+                if (e + 3 < n) x = ldg_nc_u4(reinterpret_cast<const uint4 *>(base + 128 * i));
+                else {
+                    if (e < n) x.x = base[128 * i];
+                    if (e + 1 < n) x.y = base[128 * i + 1];
+                    if (e + 2 < n) x.z = base[128 * i + 2];
+                }
+                v[i] = x;
+            }
+        }
+    };
+    // rows of the block in registers -> (idx, val) at dst_i / dst_v + running base (shared or global memory);
+    // returns the block's count.  bounded: stop storing (keep counting) once the stage is full.
+    bool stored_all = true;     // compact(bounded): every entry of the block fitted the stage
+    auto compact = [&](uint32_t tt, uint32_t *dst_i, uint32_t *dst_v, bool bounded) -> uint32_t {
+        uint32_t base = 0;
+        bool on = true;
+        const uint32_t e0 = tt * (uint32_t)kTile + 4u * (uint32_t)lane;
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            const bool m0 = nz32(v[i].x), m1 = nz32(v[i].y), m2 = nz32(v[i].z), m3 = nz32(v[i].w);
+            const unsigned b0 = __ballot_sync(kFull, m0), b1 = __ballot_sync(kFull, m1), b2 = __ballot_sync(kFull, m2),
+                           b3 = __ballot_sync(kFull, m3);
+            if ((b0 | b1 | b2 | b3) != 0u) {
+                if (bounded && base > kCooStage) on = false;     // warp-uniform: the rest of the block only counts
+                if (on) {
+                    uint32_t pos = base + __popc(b0 & lt) + __popc(b1 & lt) + __popc(b2 & lt) + __popc(b3 & lt);
+                    const uint32_t e = e0 + 128u * (uint32_t)i;
+                    if (m0) { dst_i[pos] = e; dst_v[pos] = v[i].x; ++pos; }
+                    if (m1) { dst_i[pos] = e + 1u; dst_v[pos] = v[i].y; ++pos; }
+                    if (m2) { dst_i[pos] = e + 2u; dst_v[pos] = v[i].z; ++pos; }
+                    if (m3) { dst_i[pos] = e + 3u; dst_v[pos] = v[i].w; }
+                }
+                base += __popc(b0) + __popc(b1) + __popc(b2) + __popc(b3);
+            }
+        }
+        stored_all = on;
+        return base;
+    };
+
+    bool pending = false;
+    uint32_t pt = 0, pcnt = 0, pbuf = 0, cur = 0;
+    auto finish_block = [&](uint32_t tt, uint32_t cnt) -> uint32_t {   // look-back; the last block writes nnz
+        const uint32_t excl = lookback_prefix(a.ws.status, tag, tt, cnt, T, a.ws.excl, lane);
+        if (tt + 1u == T && lane == 0) *a.d_nnz = excl + cnt;
+        return excl;
+    };
+    auto flush_pending = [&]() {
+        if (pending) {
+            const uint32_t excl = finish_block(pt, pcnt);
+            const uint32_t *si = stage + (size_t)pbuf * 2 * kCooStageWords, *sv = si + kCooStageWords;
+            for (uint32_t i = lane; i < pcnt; i += 32) {
+                a.idx[excl + i] = si[i];
+                a.val[excl + i] = sv[i];
+            }
+            pending = false;
+        }
+    };
+
+    uint32_t t = next_ticket(ticket, lane);
+    if (t < T) load_block(t);
+    uint32_t t_next = 0;
+    if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
+    while (t < T) {
+        const uint32_t tn = __shfl_sync(kFull, t_next, 0);
+        if (tn < Tfull && lane == 0) {   // the next block starts moving HBM -> L2 now (one bulk prefetch)
+            const unsigned char *src = reinterpret_cast<const unsigned char *>(a.dense) + (size_t)tn * kTile * 4;
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(kTile * 4)) : "memory");
+        }
+        uint32_t *si = stage + (size_t)cur * 2 * kCooStageWords;
+        const uint32_t cnt = compact(t, si, si + kCooStageWords, true);
+        __syncwarp();
+        publish_count(a.ws.status, tag, t, cnt, lane);
+        flush_pending();                        // the previous block: its prefix has had an iteration to arrive
+        if (stored_all) {
+            pending = true;
+            pt = t; pcnt = cnt; pbuf = cur;
+            cur ^= 1u;
+        } else {                                // dense block: look-back now, write from the registers
+            const uint32_t excl = finish_block(t, cnt);
+            compact(t, a.idx + excl, a.val + excl, false);
+        }
+        if (tn < T) load_block(tn);
+        t = tn;
+        if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
+    }
+    flush_pending();
+    coo_leave(a.ws.hdr, ticket, tag, a.ws.status, T, gridDim.x * (uint32_t)kCooWarps, lane);
+}
+
+// ============================================ block offsets (pre-pass) ============================================
+// off[t] = number of entries with idx < 4096 t, t = 0 .. T: entry k (and the end sentinel k = nnz) writes the
+// offsets of every block boundary that lies between its predecessor and itself.  One streaming pass over idx.
+struct CooOffsetsArgs {
+    const uint32_t *idx[2];
+    const uint32_t *d_nnz[2];
+    uint32_t *off[2];
+    uint32_t T;
+};
+__global__ void __launch_bounds__(256) coo_offsets_kernel(const CooOffsetsArgs a) {
+    const uint32_t *__restrict__ idx = a.idx[blockIdx.y];
+    uint32_t *__restrict__ off = a.off[blockIdx.y];
+    const uint32_t nnz = *a.d_nnz[blockIdx.y], T = a.T;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k <= nnz; k += stride) {
+        const uint32_t lo = k == 0 ? 0u : (idx[k - 1] >> 12) + 1u;       // first block that starts behind entry k - 1
+        const uint32_t hi = k == nnz ? T : (idx[k] >> 12);               // last block that starts at or before entry k
+        for (uint32_t t = lo; t <= hi; ++t) off[t] = (uint32_t)k;
+    }
+}
+
+// =============================================== decompress ===============================================
+struct CooExpandArgs {
+    const uint32_t *idx, *val, *off;
+    uint32_t *dense;
+    uint64_t n;
+};
+__global__ void __launch_bounds__(kCooWarps * 32, 3) coo_decompress_kernel(const CooExpandArgs a) {
+    extern __shared__ __align__(16) uint32_t coo_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *const blk = coo_smem + (size_t)warp * kTile;
+    const uint32_t T = (uint32_t)((a.n + kTile - 1) / kTile), Tfull = (uint32_t)(a.n / kTile);
+    const uint32_t nwarps = gridDim.x * kCooWarps;
+    for (uint32_t t = blockIdx.x * kCooWarps + warp; t < T; t += nwarps) {
+        const uint32_t k0 = a.off[t], k1 = a.off[t + 1];
+        uint4 *b4 = reinterpret_cast<uint4 *>(blk);
+        uint4 *d4 = reinterpret_cast<uint4 *>(a.dense + (size_t)t * kTile);
+        if (k0 == k1 && t < Tfull) {                 // empty block: a 16 KB zero fill
+#pragma unroll 8
+            for (int i = 0; i < 32; ++i) stg_stream_u4(d4 + 32 * i + lane, make_uint4(0u, 0u, 0u, 0u));
+            continue;
+        }
+#pragma unroll 8
+        for (int i = 0; i < 32; ++i) b4[32 * i + lane] = make_uint4(0u, 0u, 0u, 0u);
+        __syncwarp();
+        for (uint32_t k = k0 + lane; k < k1; k += 32) blk[a.idx[k] & (kTile - 1)] = a.val[k];
+        __syncwarp();
+        if (t < Tfull) {
+#pragma unroll 8
+            for (int i = 0; i < 32; ++i) stg_stream_u4(d4 + 32 * i + lane, b4[32 * i + lane]);
+        } else {
+            const uint32_t rem = (uint32_t)(a.n - (uint64_t)t * kTile);
+            for (uint32_t i = lane; i < rem; i += 32) a.dense[(size_t)t * kTile + i] = blk[i];
+        }
+        __syncwarp();
+    }
+}
+
+// ================================================ reduce_sd ================================================
+__global__ void __launch_bounds__(256) coo_scatter_add_kernel(const uint32_t *__restrict__ idx, const uint32_t *__restrict__ val,
+                                                              const uint32_t *d_nnz, uint32_t *dense) {
+    const uint32_t nnz = *d_nnz;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nnz; k += stride) {
+        uint32_t *p = dense + idx[k];
+        uint32_t d;
+        asm volatile("ld.global.L2::64B.u32 %0, [%1];" : "=r"(d) : "l"(p) : "memory");
+        *p = __float_as_uint(__fadd_rn(__uint_as_float(d), __uint_as_float(val[k])));
+    }
+}
+
+// ============================================== reduce_ss (merge) ==============================================
+struct CooMergeArgs {
+    const uint32_t *ix, *vx, *iy, *vy;
+    uint32_t *io, *vo, *d_no;
+    uint64_t n;
+    CooWs ws;
+};
+constexpr uint32_t kBmWords = kTile / 32;   // candidate bitmap of a block
+
+__global__ void __launch_bounds__(kCooWarps * 32, 3) coo_merge_kernel(const CooMergeArgs a) {
+    extern __shared__ __align__(16) uint32_t coo_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *const blk = coo_smem + (size_t)warp * (kTile + kBmWords);
+    uint32_t *const bm = blk + kTile;
+    uint32_t *const ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(a.ws.hdr) + kWsCompressTicket);
+    const uint32_t tag = launch_tag(a.ws.hdr);
+    const uint32_t T = (uint32_t)((a.n + kTile - 1) / kTile);
+
+    uint32_t t = next_ticket(ticket, lane);
+    while (t < T) {
+        const uint32_t x0 = a.ws.offx[t], x1 = a.ws.offx[t + 1], y0 = a.ws.offy[t], y1 = a.ws.offy[t + 1];
+        uint32_t t_next = 0;
+        if (lane == 0) t_next = atomicAdd(ticket, 1u);       // returns while this block is merged
+        uint32_t cnt = 0;
+        uint32_t keep[4] = {0u, 0u, 0u, 0u};                  // survivors among positions 128 lane .. + 127
+        if (x0 != x1 || y0 != y1) {
+            reinterpret_cast<uint4 *>(bm)[lane] = make_uint4(0u, 0u, 0u, 0u);
+            __syncwarp();
+            for (uint32_t k = x0 + lane; k < x1; k += 32) {   // X first: its entries define the block
+                const uint32_t pos = a.ix[k] & (kTile - 1);
+                blk[pos] = a.vx[k];
+                atomicOr(&bm[pos >> 5], 1u << (pos & 31));
+            }
+            __syncwarp();
+            for (uint32_t k = y0 + lane; k < y1; k += 32) {   // then Y: o = x + y (received + local) where X has an entry
+                const uint32_t pos = a.iy[k] & (kTile - 1);
+                const uint32_t y = a.vy[k];
+                const bool has = (bm[pos >> 5] >> (pos & 31)) & 1u;   // only X (or nobody) can have set this bit
+                blk[pos] = has ? __float_as_uint(__fadd_rn(__uint_as_float(blk[pos]), __uint_as_float(y))) : y;
+                if (!has) atomicOr(&bm[pos >> 5], 1u << (pos & 31));
+            }
+            __syncwarp();
+            const uint4 c = reinterpret_cast<const uint4 *>(bm)[lane];
+            const uint32_t cw[4] = {c.x, c.y, c.z, c.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {                     // predicate re-applied to the sums
+                uint32_t u = cw[q];
+                while (u) {
+                    const uint32_t b = (uint32_t)__ffs(u) - 1u;
+                    u &= u - 1u;
+                    if (nz32(blk[128u * lane + 32u * q + b])) keep[q] |= 1u << b;
+                }
+                cnt += __popc(keep[q]);
+            }
+        }
+        const uint32_t incl = warp_incl_scan(cnt, lane);
+        const uint32_t total = __shfl_sync(kFull, incl, 31);
+        publish_count(a.ws.status, tag, t, total, lane);
+        const uint32_t excl = lookback_prefix(a.ws.status, tag, t, total, T, a.ws.excl, lane);
+        if (t + 1u == T && lane == 0) *a.d_no = excl + total;
+        uint32_t o = excl + incl - cnt;
+        const uint32_t e0 = t * (uint32_t)kTile + 128u * (uint32_t)lane;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            uint32_t u = keep[q];
+            while (u) {
+                const uint32_t b = (uint32_t)__ffs(u) - 1u;
+                u &= u - 1u;
+                a.io[o] = e0 + 32u * q + b;
+                a.vo[o] = blk[128u * lane + 32u * q + b];
+                ++o;
+            }
+        }
+        __syncwarp();
+        t = __shfl_sync(kFull, t_next, 0);
+    }
+    coo_leave(a.ws.hdr, ticket, tag, a.ws.status, T, gridDim.x * (uint32_t)kCooWarps, lane);
+}
+
+// ================================================= launchers =================================================
+template <class K>
+static cudaError_t allow_smem(K kernel, size_t smem, std::atomic<bool> (&done)[64]) {   // one-time per device
+    std::atomic<bool> &flag = done[current_device_slot()];
+    if (!flag.load(std::memory_order_acquire)) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        flag.store(true, std::memory_order_release);
+    }
+    return cudaSuccess;
+}
+static unsigned persistent_grid(uint64_t T) {
+    uint64_t blocks = (T + kCooWarps - 1) / kCooWarps;
+    const uint64_t cap = (uint64_t)num_sms() * 3;
+    return (unsigned)(blocks > cap ? cap : (blocks ? blocks : 1));
+}
+
+static cudaError_t launch_coo_compress(const void *dense, uint64_t n, uint32_t *idx, void *val, uint32_t *d_nnz, void *ws,
+                                       cudaStream_t s) {
+    if (n == 0) return launch_set_u32(d_nnz, 0u, Gate{nullptr, 0, 0}, s);
+    static std::atomic<bool> done[64];
+    const size_t smem = (size_t)kCooWarps * 4 * kCooStageWords * sizeof(uint32_t);
+    cudaError_t e = allow_smem(coo_compress_kernel, smem, done);
+    if (e != cudaSuccess) return e;
+    const CooCompressArgs a = {reinterpret_cast<const uint32_t *>(dense), n, idx, reinterpret_cast<uint32_t *>(val), d_nnz,
+                               coo_ws(ws, n)};
+    coo_compress_kernel<<<persistent_grid((n + kTile - 1) / kTile), kCooWarps * 32, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+static cudaError_t launch_coo_offsets(const uint32_t *ix, const uint32_t *d_nx, uint32_t *offx, const uint32_t *iy,
+                                      const uint32_t *d_ny, uint32_t *offy, uint64_t n, cudaStream_t s) {
+    CooOffsetsArgs a;
+    a.idx[0] = ix; a.d_nnz[0] = d_nx; a.off[0] = offx;
+    a.idx[1] = iy; a.d_nnz[1] = d_ny; a.off[1] = offy;
+    a.T = (uint32_t)((n + kTile - 1) / kTile);
+    coo_offsets_kernel<<<dim3((unsigned)num_sms() * 8, iy ? 2 : 1), 256, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+static cudaError_t launch_coo_decompress(const uint32_t *idx, const void *val, const uint32_t *d_nnz, uint64_t n, void *dense,
+                                         void *ws, cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    static std::atomic<bool> done[64];
+    const size_t smem = (size_t)kCooWarps * kTile * sizeof(uint32_t);
+    cudaError_t e = allow_smem(coo_decompress_kernel, smem, done);
+    if (e != cudaSuccess) return e;
+    const CooWs w = coo_ws(ws, n);
+    e = launch_coo_offsets(idx, d_nnz, w.offx, nullptr, nullptr, nullptr, n, s);
+    if (e != cudaSuccess) return e;
+    const CooExpandArgs a = {idx, reinterpret_cast<const uint32_t *>(val), w.offx, reinterpret_cast<uint32_t *>(dense), n};
+    coo_decompress_kernel<<<persistent_grid((n + kTile - 1) / kTile), kCooWarps * 32, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+static cudaError_t launch_coo_reduce_sd(const uint32_t *idx, const void *val, const uint32_t *d_nnz, uint64_t n, void *dense,
+                                        cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    coo_scatter_add_kernel<<<(unsigned)num_sms() * 8, 256, 0, s>>>(idx, reinterpret_cast<const uint32_t *>(val), d_nnz,
+                                                                   reinterpret_cast<uint32_t *>(dense));
+    return cudaGetLastError();
+}
+
+static cudaError_t launch_coo_merge(const uint32_t *ix, const void *vx, const uint32_t *d_nx, const uint32_t *iy, const void *vy,
+                                    const uint32_t *d_ny, uint64_t n, uint32_t *io, void *vo, uint32_t *d_no, void *ws,
+                                    cudaStream_t s) {
+    if (n == 0) return launch_set_u32(d_no, 0u, Gate{nullptr, 0, 0}, s);
+    static std::atomic<bool> done[64];
+    const size_t smem = (size_t)kCooWarps * (kTile + kBmWords) * sizeof(uint32_t);
+    cudaError_t e = allow_smem(coo_merge_kernel, smem, done);
+    if (e != cudaSuccess) return e;
+    const CooWs w = coo_ws(ws, n);
+    e = launch_coo_offsets(ix, d_nx, w.offx, iy, d_ny, w.offy, n, s);
+    if (e != cudaSuccess) return e;
+    const CooMergeArgs a = {ix, reinterpret_cast<const uint32_t *>(vx), iy, reinterpret_cast<const uint32_t *>(vy), io,
+                            reinterpret_cast<uint32_t *>(vo), d_no, n, w};
+    coo_merge_kernel<<<persistent_grid((n + kTile - 1) / kTile), kCooWarps * 32, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace pici
+
+// =================================================== C ABI ===================================================
+using namespace pici;
+namespace {
+inline bool al(const void *p, uintptr_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
+inline int rc_of(cudaError_t e) { return e == cudaSuccess ? PICI_OK : PICI_ERR_CUDA; }
+constexpr uint64_t kCooMaxN = 1ull << 32;
+int check_coo(const uint32_t *idx, const void *val, const uint32_t *d_nnz, uint64_t n) {
+    if (n >= kCooMaxN || d_nnz == nullptr) return PICI_ERR_INVALID_ARG;
+    if (n != 0 && (idx == nullptr || val == nullptr)) return PICI_ERR_INVALID_ARG;
+    if (!al(idx, 16) || !al(val, 16) || !al(d_nnz, 4)) return PICI_ERR_ALIGN;
+    return PICI_OK;
+}
+int check_ws(void *ws, uint64_t ws_bytes, uint64_t n) {
+    if (!al(ws, 16)) return PICI_ERR_ALIGN;
+    if (n != 0 && (ws == nullptr || ws_bytes < coo_workspace_bytes(n))) return PICI_ERR_WORKSPACE;
+    return PICI_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int pici_coo_sizes(uint64_t n, uint64_t *capacity, uint64_t *workspace_bytes) {
+    if (n >= kCooMaxN) return PICI_ERR_INVALID_ARG;
+    if (capacity) *capacity = n;
+    if (workspace_bytes) *workspace_bytes = coo_workspace_bytes(n);
+    return PICI_OK;
+}
+
+int pici_coo_compress(const void *dense, uint64_t n, uint32_t *idx, void *val, uint64_t capacity, uint32_t *d_nnz,
+                      void *ws, uint64_t ws_bytes, void *stream) {
+    int rc = check_coo(idx, val, d_nnz, n);
+    if (rc != PICI_OK) return rc;
+    if (n != 0 && dense == nullptr) return PICI_ERR_INVALID_ARG;
+    if (!al(dense, 16)) return PICI_ERR_ALIGN;
+    if (capacity < n) return PICI_ERR_CAPACITY;
+    if ((rc = check_ws(ws, ws_bytes, n)) != PICI_OK) return rc;
+    return rc_of(launch_coo_compress(dense, n, idx, val, d_nnz, ws, static_cast<cudaStream_t>(stream)));
+}
+
+int pici_coo_decompress(const uint32_t *idx, const void *val, const uint32_t *d_nnz, uint64_t n, void *dense_out,
+                        void *ws, uint64_t ws_bytes, void *stream) {
+    int rc = check_coo(idx, val, d_nnz, n);
+    if (rc != PICI_OK) return rc;
+    if (n != 0 && dense_out == nullptr) return PICI_ERR_INVALID_ARG;
+    if (!al(dense_out, 16)) return PICI_ERR_ALIGN;
+    if ((rc = check_ws(ws, ws_bytes, n)) != PICI_OK) return rc;
+    return rc_of(launch_coo_decompress(idx, val, d_nnz, n, dense_out, ws, static_cast<cudaStream_t>(stream)));
+}
+
+int pici_coo_reduce_sd(const uint32_t *idx, const void *val, const uint32_t *d_nnz, uint64_t n, void *dense_inout,
+                       void *stream) {
+    int rc = check_coo(idx, val, d_nnz, n);
+    if (rc != PICI_OK) return rc;
+    if (n != 0 && dense_inout == nullptr) return PICI_ERR_INVALID_ARG;
+    if (!al(dense_inout, 16)) return PICI_ERR_ALIGN;
+    return rc_of(launch_coo_reduce_sd(idx, val, d_nnz, n, dense_inout, static_cast<cudaStream_t>(stream)));
+}
+
+int pici_coo_reduce_ss(const uint32_t *ix, const void *vx, const uint32_t *d_nx, const uint32_t *iy, const void *vy,
+                       const uint32_t *d_ny, uint64_t n, uint32_t *io, void *vo, uint64_t capacity, uint32_t *d_no,
+                       void *ws, uint64_t ws_bytes, void *stream) {
+    int rc = check_coo(ix, vx, d_nx, n);
+    if (rc == PICI_OK) rc = check_coo(iy, vy, d_ny, n);
+    if (rc == PICI_OK) rc = check_coo(io, vo, d_no, n);
+    if (rc != PICI_OK) return rc;
+    if (capacity < n) return PICI_ERR_CAPACITY;
+    if ((rc = check_ws(ws, ws_bytes, n)) != PICI_OK) return rc;
+    if (n != 0 && (io == ix || io == iy || vo == vx || vo == vy || d_no == d_nx || d_no == d_ny)) return PICI_ERR_INVALID_ARG;
+    return rc_of(launch_coo_merge(ix, vx, d_nx, iy, vy, d_ny, n, io, vo, d_no, ws, static_cast<cudaStream_t>(stream)));
+}
+
+}  // extern "C"

@@ -8,16 +8,19 @@ import re
 
 import pytest
 
-from paper_2607_04676_b200 import pici
+from paper_2607_04676_b200 import coo, pici
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared() -> list[str]:
-    """Function names declared between the extern "C" braces of include/pici.h."""
-    src = open(os.path.join(ROOT, "include", "pici.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(pici_[a-z_0-9]+)\s*\(", src)))
+    """Function names declared between the extern "C" braces of include/*.h."""
+    names = set()
+    for h in sorted(os.listdir(os.path.join(ROOT, "include"))):
+        src = open(os.path.join(ROOT, "include", h)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(pici_[a-z_0-9]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_every_declared_symbol_is_exported_and_bound():
@@ -27,8 +30,32 @@ def test_every_declared_symbol_is_exported_and_bound():
     lib = pici.lib()
     for n in names:
         assert hasattr(lib, n), f"{n} is declared in include/pici.h but not exported"
-    assert set(names) == set(pici.EXPORTS), "the Python binding and the header disagree on the entry points"
+    assert set(names) == set(pici.EXPORTS) | set(coo.EXPORTS), "the Python binding and the header disagree on the entry points"
     assert lib.pici_version() == 100
+    coo.lib()                                                # binds the pici_coo_* signatures
+
+
+def test_coo_calls_validate_before_any_cuda_call():
+    """include/pici_coo.h: sizes follow the format (capacity n: one index per nonzero in the worst case,
+    PAPER.md:275) and bad arguments are rejected on the host."""
+    lib = coo.lib()
+    INVALID, ALIGN, CAPACITY, WORKSPACE = -1, -3, -4, -5
+    n = 8192
+    cap, ws = coo.sizes(n)
+    assert cap == n and ws % 16 == 0 and ws > pici.sizes(n)[3]
+    assert lib.pici_coo_sizes(1 << 32, None, None) == INVALID
+    a, b, c, w = 0x10000, 0x20000, 0x30000, 0x40000
+    C = lib.pici_coo_compress
+    assert C(None, n, b, c, n, w, w + 0x1000, ws, None) == INVALID
+    assert C(a, n, b, c, n, None, w + 0x1000, ws, None) == INVALID
+    assert C(a, n, b + 4, c, n, w, w + 0x1000, ws, None) == ALIGN
+    assert C(a, n, b, c, n - 1, w, w + 0x1000, ws, None) == CAPACITY
+    assert C(a, n, b, c, n, w, w + 0x1000, ws - 1, None) == WORKSPACE
+    assert lib.pici_coo_decompress(b, c, w, n, None, w + 0x1000, ws, None) == INVALID
+    assert lib.pici_coo_reduce_sd(b, c, w, n, a + 8, None) == ALIGN
+    S = lib.pici_coo_reduce_ss
+    assert S(a, a + 0x1000, w, b, b + 0x1000, w + 16, n, a, c + 0x1000, n, w + 32, w + 0x1000, ws, None) == INVALID   # io == ix
+    assert S(a, a + 0x1000, w, b, b + 0x1000, w + 16, n, c, c + 0x1000, n - 1, w + 32, w + 0x1000, ws, None) == CAPACITY
 
 
 def test_oracle_and_product_share_no_code():
