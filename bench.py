@@ -353,6 +353,61 @@ def run_sweep(pk, n: int, peak: float, launches: int, device, dtypes=("f32", "bf
     return rows
 
 
+def run_coo_sweep(pk, n: int, peak: float, launches: int, device, sparsities=(0.9, 0.95, 0.96875, 0.99, 0.999, 0.9999),
+                  seeds=(0, 1, 2)) -> list[dict]:
+    """Pici against the paper's COO variant, kernel by kernel at
+    N elements, fp32: same buffers, same rotation of seeded buffer sets as run_sweep.  A row gives both formats'
+    time, algorithmic bytes and message size; `coo_over_pici` > 1 means Pici is faster.  There is no wire here, so
+    this is the compute side of Fig. 3's crossover; the size side is `msg_bytes` (equal at 96.875 % sparsity but
+    for Pici's I)."""
+    from paper_2607_04676_b200 import coo as ck
+    ck.lib()
+    rows = []
+    ws = pk.alloc_workspace(n, device)
+    cws = ck.alloc_workspace(n, device)
+    for sp in sparsities:
+        d = 1.0 - sp
+        sets = []
+        for sd in seeds:
+            S = {"x": wl.sparse_buffer(n, d, seed=wl.stream_seed(sd, 0), device=device),
+                 "y": wl.sparse_buffer(n, d, seed=wl.stream_seed(sd, 1), device=device)}
+            S["px"], S["py"], S["po"] = (pk.alloc_pici(n, pk.F32, device) for _ in range(3))
+            S["cx"], S["cy"], S["co"] = (ck.alloc_coo(n, device) for _ in range(3))
+            pk.compress(S["x"], S["px"], ws); pk.compress(S["y"], S["py"], ws)
+            pk.reduce_ss(S["px"], S["py"], S["po"], ws)
+            ck.compress(S["x"], S["cx"], cws); ck.compress(S["y"], S["cy"], cws)
+            ck.reduce_ss(S["cx"], S["cy"], S["co"], cws)
+            S["out"] = torch.empty_like(S["x"])
+            sets.append(S)
+        torch.cuda.synchronize()
+        mean = lambda vals: sum(vals) / len(vals)
+        nx = mean([S["cx"].nnz_host() for S in sets]); ny = mean([S["cy"].nnz_host() for S in sets])
+        no = mean([S["co"].nnz_host() for S in sets])
+        assert all(S["cx"].nnz_host() == S["px"].nnz_host() and S["co"].nnz_host() == S["po"].nnz_host() for S in sets)
+        sect = mean([touched_sectors_f32(S["x"]) for S in sets])
+        cases = {
+            "compress": (lambda S: pk.compress(S["x"], S["px"], ws), lambda S: ck.compress(S["x"], S["cx"], cws),
+                         bytes_compress(n, 4, nx), 4 * n + 8 * nx),
+            "decompress": (lambda S: pk.decompress(S["px"], S["out"]), lambda S: ck.decompress(S["cx"], S["out"], cws),
+                           bytes_decompress(n, 4, nx), 4 * n + 8 * nx),
+            "reduce_ss": (lambda S: pk.reduce_ss(S["px"], S["py"], S["po"], ws), lambda S: ck.reduce_ss(S["cx"], S["cy"], S["co"], cws),
+                          bytes_reduce_ss(n, nx, ny, no), 8 * (nx + ny + no)),
+            "reduce_sd": (lambda S: pk.reduce_sd(S["px"], S["y"]), lambda S: ck.reduce_sd(S["cx"], S["y"]),
+                          bytes_reduce_sd(n, nx, sect), 8 * nx + min(8 * n, 64 * sect)),
+        }
+        for op, (fp, fc, bp, bc) in cases.items():
+            pms, _ = graph_time([lambda S=S: fp(S) for S in sets], launches)
+            cms, _ = graph_time([lambda S=S: fc(S) for S in sets], launches)
+            rows.append({"sparsity": sp, "op": op, "pici_ms": round(pms, 4), "coo_ms": round(cms, 4),
+                         "coo_over_pici": round(cms / pms, 3), "pici_alg_bytes": int(bp), "coo_alg_bytes": int(bc),
+                         "pici_frac": round(bp / pms / 1e6 / peak, 3), "coo_frac": round(bc / cms / 1e6 / peak, 3),
+                         "msg_bytes": {"pici": int(meta_bytes(n) + 4 * nx), "coo": int(8 * nx), "dense": 4 * n},
+                         "seeds": list(seeds), "launches_timed": launches * 5})
+        del sets
+        torch.cuda.empty_cache()
+    return rows
+
+
 def run_e2e(pk, n: int, density: float, steps: int, device, seed: int) -> dict:
     """HOST buffers in, HOST buffers out, through pici_compress_host / pici_decompress_host."""
     h_x = wl.sparse_buffer(n, density, seed=seed).pin_memory()
@@ -549,6 +604,8 @@ def main():
     ap.add_argument("--policy-sweep", action="store_true",
                     help="reduce-scatter under the paper's policy for every intra x inter threshold pair (Fig. 2 analogue)")
     ap.add_argument("--no-rings", action="store_true")
+    ap.add_argument("--coo-sweep", action="store_true", help="Pici vs COO kernel by kernel (one JSON line per row)")
+    ap.add_argument("--no-coo", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="sweep rows: eager launches timed one by one (for ncu captures)")
     args = ap.parse_args()
     if args.warmup < 3:
@@ -578,6 +635,10 @@ def main():
         return
     if args.policy_sweep:
         for r in run_policy_sweep(pk, 5, device):
+            print(json.dumps(r), flush=True)
+        return
+    if args.coo_sweep:
+        for r in run_coo_sweep(pk, n, peak, args.sweep_iters, device):
             print(json.dumps(r), flush=True)
         return
     if args.sweep_only:   # kernel-by-kernel timing (also the program the single-kernel ncu captures run)
@@ -678,6 +739,8 @@ def main():
                                                              ("reduce_scatter", "paper", 400)]) +
                         run_ring(pk, "config4", 5, device, [("all_reduce", "fused", 400), ("all_reduce", "fused", 200)]) +
                         run_ring(pk, "config5", 5, device, [("all_gather", "fused", 900), ("all_reduce", "fused", 400)]))
+    if not args.no_coo and world == 1:      # S8(f) f3: the second format, kernel by kernel against Pici
+        out["coo"] = run_coo_sweep(pk, n, peak, args.sweep_iters, device)
     if not args.no_cpu and world == 1:
         out["cpu_baseline"] = run_cpu_baseline(args.cpu_n, density)
     print(json.dumps(out))

@@ -716,8 +716,6 @@ __device__ __forceinline__ void worker(const MergeArgs &a, MergeShared &sh, uint
     }
 }
 
-__device__ __forceinline__ bool tagged(uint64_t v, uint32_t tag) { return (uint32_t)(v >> 32) == tag; }
-
 // ============================================ publisher ===========================================
 // Phase 2 input.  One warp that does nothing but make counts visible: as soon as an item's workers are done it
 // stores the item's per-tile survivor counts (tagged words) and adds (tiles, survivors) to the accumulators of
@@ -751,40 +749,7 @@ __device__ __forceinline__ void publisher(const MergeArgs &a, MergeShared &sh, c
 }
 
 // ============================================ flushers ============================================
-// Exclusive prefix of tile t0 = survivors of all tiles below it (one warp): complete 1024-tile blocks below
-// (carried in E / E_blk from call to call) + complete groups of 32 below inside the own block + tiles below inside
-// the own group.  Three independent sets of loads; each word says by itself whether it is complete.
-__device__ __forceinline__ uint32_t tile_prefix(const MergeArgs &a, uint32_t tag, uint32_t t0, uint32_t &E,
-                                                uint32_t &E_blk, int lane) {
-    const uint32_t u = t0 & 31u, grp = (t0 >> 5) & 31u, blk = t0 >> 10, gbase = t0 & ~31u;
-    uint64_t va, vg, vb = 0;
-    unsigned ns = 8;
-    for (;;) {
-        va = (uint32_t)lane < u ? ld_status(a.tile_word + gbase + lane) : ((uint64_t)tag << 32);
-        vg = (uint32_t)lane < grp ? ld_status(a.grp_acc + blk * 32u + lane) : (32ull << 48);
-        const bool more = E_blk + (uint32_t)lane < blk;
-        vb = more ? ld_status(a.blk_acc + E_blk + lane) : (1024ull << 48);
-        if (__all_sync(kFull, tagged(va, tag) && (vg >> 48) == 32u && (vb >> 48) == 1024u)) break;
-        __nanosleep(ns);
-        if (ns < 128) ns += ns;
-    }
-    const uint32_t nb = min(32u, blk - E_blk);
-    E += __reduce_add_sync(kFull, (uint32_t)lane < nb ? (uint32_t)vb : 0u);
-    E_blk += nb;
-    while (E_blk < blk) {   // more than 32 new blocks since this warp's last prefix (first call on a huge input)
-        const uint32_t c = min(32u, blk - E_blk);
-        uint64_t v;
-        for (;;) {
-            v = (uint32_t)lane < c ? ld_status(a.blk_acc + E_blk + lane) : (1024ull << 48);
-            if (__all_sync(kFull, (v >> 48) == 1024u)) break;
-            __nanosleep(64);
-        }
-        E += __reduce_add_sync(kFull, (uint32_t)lane < c ? (uint32_t)v : 0u);
-        E_blk += c;
-    }
-    return E + __reduce_add_sync(kFull, (uint32_t)va + (uint32_t)vg);
-}
-
+// (the exclusive prefix of a tile: hier_prefix, pici_common.cuh)
 // One warp copies cnt words from shared memory (word index src in pool) to global memory dst (4-byte aligned, any
 // 16-byte phase): a few single words up to the first 16-byte boundary of dst, then aligned 16-byte stores whose
 // four words come from two aligned 16-byte shared-memory reads (the phase difference is a whole number of words,
@@ -845,7 +810,7 @@ __device__ __forceinline__ void flusher(const MergeArgs &a, MergeShared &sh, con
             const uint32_t incl = warp_incl_scan(cnt, lane);
             const uint32_t total = __shfl_sync(kFull, incl, 31);
             const uint32_t lo = __shfl_sync(kFull, incl - cnt, ((uint32_t)lane * ppt) & 31u);   // lane i: before tile i
-            const uint32_t base = tile_prefix(a, tag, t0, E, E_blk, lane);
+            const uint32_t base = hier_prefix(a.blk_acc, a.grp_acc, a.tile_word, tag, t0, E, E_blk, lane);
             if ((uint32_t)lane < k) {
                 a.Io[t0 + lane] = base + lo;
                 if (t0 + lane + 1u == a.T) a.Io[a.T] = base + total;

@@ -184,6 +184,52 @@ __device__ __forceinline__ void red_add_u64(uint64_t *p, uint64_t v) {
     asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
+// ---- store-only hierarchical exclusive scan of per-tile counts (reduce_ss, the COO merge) ---------------------------
+// Three levels over tiles: one tagged word per tile, one accumulator per group of 32 tiles, one per block of 1024
+// tiles, each accumulator (tiles << 48) + count, added to by 64-bit red.add and zero between launches (the launch's
+// last warp clears them).  prefix(t0) = [complete 1024-blocks below, carried in E / E_blk from call to call: t0 must
+// not decrease per warp] + [complete groups below inside the own block] + [tiles below inside the own group]: three
+// independent sets of loads, each word says by itself whether it is complete, so a prefix only ever waits for COUNTS
+// of lower tiles - never for another prefix - and there is no chain of look-backs however many tiles are in flight.
+__device__ __forceinline__ bool tagged(uint64_t v, uint32_t tag) { return (uint32_t)(v >> 32) == tag; }
+__device__ __forceinline__ void hier_publish(uint64_t *blk_acc, uint64_t *grp_acc, uint64_t *tile_word, uint32_t tag,
+                                             uint32_t t, uint32_t count) {   // one lane
+    st_status(tile_word + t, tag, count);
+    const uint64_t v = kOneAdd + count;
+    red_add_u64(grp_acc + (t >> 5), v);
+    red_add_u64(blk_acc + (t >> 10), v);
+}
+__device__ __forceinline__ uint32_t hier_prefix(const uint64_t *blk_acc, const uint64_t *grp_acc, const uint64_t *tile_word,
+                                                uint32_t tag, uint32_t t0, uint32_t &E, uint32_t &E_blk, int lane) {
+    const uint32_t u = t0 & 31u, grp = (t0 >> 5) & 31u, blk = t0 >> 10, gbase = t0 & ~31u;
+    uint64_t va, vg, vb = 0;
+    unsigned ns = 8;
+    for (;;) {
+        va = (uint32_t)lane < u ? ld_status(tile_word + gbase + lane) : ((uint64_t)tag << 32);
+        vg = (uint32_t)lane < grp ? ld_status(grp_acc + blk * 32u + lane) : (32ull << 48);
+        const bool more = E_blk + (uint32_t)lane < blk;
+        vb = more ? ld_status(blk_acc + E_blk + lane) : (1024ull << 48);
+        if (__all_sync(kFull, tagged(va, tag) && (vg >> 48) == 32u && (vb >> 48) == 1024u)) break;
+        __nanosleep(ns);
+        if (ns < 128) ns += ns;
+    }
+    const uint32_t nb = min(32u, blk - E_blk);
+    E += __reduce_add_sync(kFull, (uint32_t)lane < nb ? (uint32_t)vb : 0u);
+    E_blk += nb;
+    while (E_blk < blk) {   // more than 32 new blocks since this warp's last prefix (first call on a huge input)
+        const uint32_t c = min(32u, blk - E_blk);
+        uint64_t v;
+        for (;;) {
+            v = (uint32_t)lane < c ? ld_status(blk_acc + E_blk + lane) : (1024ull << 48);
+            if (__all_sync(kFull, (v >> 48) == 1024u)) break;
+            __nanosleep(64);
+        }
+        E += __reduce_add_sync(kFull, (uint32_t)lane < c ? (uint32_t)v : 0u);
+        E_blk += c;
+    }
+    return E + __reduce_add_sync(kFull, (uint32_t)va + (uint32_t)vg);
+}
+
 // ---- TMA 1-D bulk copy global -> shared, completion on an mbarrier (UBLKCP in SASS) -------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
