@@ -41,9 +41,15 @@ struct CompressCfg<PICI_BF16> {
     static constexpr int kMinBlocks = 5;
 };
 
-template <int DT>
-__global__ void __launch_bounds__(kCompressWarps * 32, CompressCfg<DT>::kMinBlocks)
+// PRUNE (fp32 only): the tile that is compressed is not read but MADE while it is loaded - sampled top-k pruning with
+// leaky error feedback fused into the same pass (include/pici_prune.h): acc = g + leak * e (two
+// roundings), sent = |acc| >= tau ? acc : +0, e <- sent ? +0 : acc written back in place; Pici(sent) is what the
+// three phases below then emit.  One pass over g and e instead of prune (read g, e; write sent, e) + compress (read
+// sent): 12 instead of 20 bytes per element.
+template <int DT, bool PRUNE>
+__global__ void __launch_bounds__(kCompressWarps * 32, PRUNE ? 2 : CompressCfg<DT>::kMinBlocks)
 compress_kernel(const Batch<CompressJob> batch) {
+    static_assert(!PRUNE || DT == PICI_F32, "prune-and-compress is fp32");
     using Cfg = CompressCfg<DT>;
     using Elem = typename Cfg::Elem;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -68,10 +74,41 @@ compress_kernel(const Batch<CompressJob> batch) {
     const uint32_t Tfull = (uint32_t)(n / kTile);
     Elem *Aout = reinterpret_cast<Elem *>(A);
 
+    float *const resid = job.resid;
+    float tau = 0.0f;
+    if constexpr (PRUNE) tau = *job.d_tau;
+    const float leak = job.leak;
+    auto prune1 = [&](uint32_t gbits, uint32_t ebits, uint32_t &e_new) -> uint32_t {
+        const float acc = __fadd_rn(__uint_as_float(gbits), __fmul_rn(leak, __uint_as_float(ebits)));
+        const bool keep = fabsf(acc) >= tau;            // IEEE compare: a NaN is never sent
+        e_new = keep ? 0u : __float_as_uint(acc);
+        return keep ? __float_as_uint(acc) : 0u;
+    };
     // Loads of a full tile: row r of the tile is one coalesced request; all 64 are issued back to back.
     auto load_full = [&](uint32_t tt, uint32_t (&v)[Cfg::kRegs]) {
         const size_t base = (size_t)tt * kTile;
-        if constexpr (DT == PICI_F32) {
+        if constexpr (PRUNE) {
+            const uint2 *pg = reinterpret_cast<const uint2 *>(reinterpret_cast<const uint32_t *>(dense) + base) + lane;
+            uint2 *pe = reinterpret_cast<uint2 *>(reinterpret_cast<uint32_t *>(resid) + base) + lane;
+            constexpr int kChunk = 16;                  // rows of g and e in flight together
+#pragma unroll
+            for (int c = 0; c < kSide / kChunk; ++c) {
+                uint2 gg[kChunk], ee[kChunk];
+#pragma unroll
+                for (int j = 0; j < kChunk; ++j) {
+                    gg[j] = ldg_stream_u2(pg + 32 * (kChunk * c + j));
+                    ee[j] = ldg_stream_u2(pe + 32 * (kChunk * c + j));
+                }
+#pragma unroll
+                for (int j = 0; j < kChunk; ++j) {
+                    const int r = kChunk * c + j;
+                    uint2 en;
+                    v[2 * r] = prune1(gg[j].x, ee[j].x, en.x);
+                    v[2 * r + 1] = prune1(gg[j].y, ee[j].y, en.y);
+                    stg_stream_u2(pe + 32 * r, en);
+                }
+            }
+        } else if constexpr (DT == PICI_F32) {
             const uint2 *p = reinterpret_cast<const uint2 *>(reinterpret_cast<const uint32_t *>(dense) + base) + lane;
 #pragma unroll
             for (int r = 0; r < kSide; ++r) {
@@ -89,7 +126,20 @@ compress_kernel(const Batch<CompressJob> batch) {
     auto load_ragged = [&](uint32_t tt, uint32_t (&v)[Cfg::kRegs]) {
         const size_t base = (size_t)tt * kTile;
         const Elem *p = reinterpret_cast<const Elem *>(dense);
-        for (int i = lane; i < kTile; i += 32) stage[i] = (base + i < n) ? p[base + i] : (Elem)0;
+        if constexpr (PRUNE) {
+            uint32_t *pe = reinterpret_cast<uint32_t *>(resid);
+            for (int i = lane; i < kTile; i += 32) {
+                uint32_t s = 0;
+                if (base + i < n) {
+                    uint32_t en;
+                    s = prune1(p[base + i], pe[base + i], en);
+                    pe[base + i] = en;
+                }
+                stage[i] = s;
+            }
+        } else {
+            for (int i = lane; i < kTile; i += 32) stage[i] = (base + i < n) ? p[base + i] : (Elem)0;
+        }
         __syncwarp();
         if constexpr (DT == PICI_F32) {
             const uint2 *q = reinterpret_cast<const uint2 *>(stage) + lane;
@@ -137,6 +187,10 @@ compress_kernel(const Batch<CompressJob> batch) {
         if (tn < Tfull && lane == 0) {
             const unsigned char *src = reinterpret_cast<const unsigned char *>(dense) + (size_t)tn * kTile * sizeof(Elem);
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(kTile * sizeof(Elem))) : "memory");
+            if constexpr (PRUNE) {
+                const unsigned char *se = reinterpret_cast<const unsigned char *>(resid) + (size_t)tn * kTile * sizeof(Elem);
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(se), "r"((uint32_t)(kTile * sizeof(Elem))) : "memory");
+            }
         }
 
         // ---- Phase 1: column words (bit r <-> row r) and counts --------------------------------
@@ -281,7 +335,7 @@ static cudaError_t launch_compress_t(const CompressJob *jobs, int count, cudaStr
     static std::atomic<bool> configured_on[64];   // one-time setup per device; doing it twice is harmless
     std::atomic<bool> &configured = configured_on[current_device_slot()];
     if (!configured.load(std::memory_order_acquire)) {
-        cudaError_t e = cudaFuncSetAttribute(compress_kernel<DT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(compress_kernel<DT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured.store(true, std::memory_order_release);
     }
@@ -294,7 +348,26 @@ static cudaError_t launch_compress_t(const CompressJob *jobs, int count, cudaStr
     uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
     const uint64_t cap = max((uint64_t)num_sms() * Cfg::kMinBlocks / count, (uint64_t)1);   // persistent: one resident wave
     if (blocks > cap) blocks = cap;
-    compress_kernel<DT><<<dim3((unsigned)blocks, (unsigned)count), kCompressWarps * 32, smem, s>>>(batch);
+    compress_kernel<DT, false><<<dim3((unsigned)blocks, (unsigned)count), kCompressWarps * 32, smem, s>>>(batch);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_prune_compress(const CompressJob &job, cudaStream_t s) {
+    const size_t smem = (size_t)kCompressWarps * kTile * sizeof(uint32_t);
+    static std::atomic<bool> configured_on[64];
+    std::atomic<bool> &configured = configured_on[current_device_slot()];
+    if (!configured.load(std::memory_order_acquire)) {
+        cudaError_t e = cudaFuncSetAttribute(compress_kernel<PICI_F32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured.store(true, std::memory_order_release);
+    }
+    Batch<CompressJob> batch;
+    batch.job[0] = job;
+    const uint64_t T = (job.n + kTile - 1) / kTile;
+    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
+    const uint64_t cap = (uint64_t)num_sms() * 2;
+    if (blocks > cap) blocks = cap;
+    compress_kernel<PICI_F32, true><<<dim3((unsigned)blocks, 1u), kCompressWarps * 32, smem, s>>>(batch);
     return cudaGetLastError();
 }
 
@@ -308,7 +381,7 @@ cudaError_t launch_compress_batch(const CompressJob *jobs, int count, int dtype,
 cudaError_t launch_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,
                             void *ws, Gate g, cudaStream_t s) {
     if (n == 0) return launch_set_u32(I, 0u, g, s);
-    const CompressJob job = {dense, n, B, I, A, ws, g};
+    const CompressJob job = {dense, n, B, I, A, ws, g, nullptr, nullptr, 0.0f};
     return launch_compress_batch(&job, 1, dtype, s);
 }
 

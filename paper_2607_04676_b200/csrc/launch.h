@@ -41,8 +41,14 @@ struct CompressJob {
     void *A;
     void *ws;
     Gate gate;
+    // prune-and-compress (pici_prune_compress, include/pici_prune.h): `dense` is the gradient g, resid the error-
+    // feedback buffer e (updated in place), *d_tau the magnitude threshold; unused (nullptr) by plain compress
+    float *resid;
+    const float *d_tau;
+    float leak;
 };
 cudaError_t launch_compress_batch(const CompressJob *jobs, int count, int dtype, cudaStream_t s);
+cudaError_t launch_prune_compress(const CompressJob &job, cudaStream_t s);   // fp32, one job
 cudaError_t launch_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,
                             void *ws, Gate g, cudaStream_t s);
 

@@ -8,7 +8,7 @@ import re
 
 import pytest
 
-from paper_2607_04676_b200 import coo, pici
+from paper_2607_04676_b200 import coo, pici, prune
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -30,9 +30,21 @@ def test_every_declared_symbol_is_exported_and_bound():
     lib = pici.lib()
     for n in names:
         assert hasattr(lib, n), f"{n} is declared in include/pici.h but not exported"
-    assert set(names) == set(pici.EXPORTS) | set(coo.EXPORTS), "the Python binding and the header disagree on the entry points"
+    assert set(names) == set(pici.EXPORTS) | set(coo.EXPORTS) | set(prune.EXPORTS), "the Python binding and the header disagree on the entry points"
     assert lib.pici_version() == 100
     coo.lib()                                                # binds the pici_coo_* signatures
+    L = prune.lib()
+    INVALID, ALIGN, CAPACITY, WORKSPACE = -1, -3, -4, -5
+    n, m = 8192, 8
+    ws = prune.workspace_bytes(n, m)
+    assert ws >= pici.sizes(n)[3] + 4 * m and ws % 16 == 0
+    a, b, c, w = 0x10000, 0x20000, 0x30000, 0x40000
+    assert L.pici_prune_threshold(a, b, n, 1.0, c, m, 0, w, w + 0x1000, ws, None) == INVALID        # k >= 1
+    assert L.pici_prune_threshold(a, b, n, 1.0, c, m, m + 1, w, w + 0x1000, ws, None) == INVALID    # k <= m
+    assert L.pici_prune_threshold(a, b, n, 1.0, c, m, 1, w, w + 0x1000, ws - 16, None) == WORKSPACE
+    assert L.pici_prune_threshold(a + 4, b, n, 1.0, c, m, 1, w, w + 0x1000, ws, None) == ALIGN
+    assert L.pici_prune_compress(a, a, n, 1.0, w, b, c, c + 0x1000, n, w + 0x1000, ws, None) == INVALID   # g must not be e
+    assert L.pici_prune_compress(a, b, n, 1.0, w, c, c + 0x1000, c + 0x2000, n - 1, w + 0x1000, ws, None) == CAPACITY
 
 
 def test_coo_calls_validate_before_any_cuda_call():
