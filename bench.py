@@ -621,6 +621,37 @@ def run_policy_sweep(pk, iters: int, device, density: float = 0.05, ranks_per_no
     return rows
 
 
+def run_dist_ring(args, rank: int, world: int, device) -> None:
+    """`torchrun ... bench.py --gpus N --dist-ring`: the REAL ring (ring_dist.py, S8(f) f2) over N ranks, one process
+    per GPU, NCCL point-to-point: all-reduce of config 3's recipe (N = 2^26 per rank, 99 % sparsity, independent
+    supports), time = max over ranks (CUDA events, barrier on both sides).  One JSON line from rank 0."""
+    import torch.distributed as dist
+    from paper_2607_04676_b200 import replicas, ring_dist as rd
+    n_per_rank = 1 << 26
+    chunk = n_per_rank // world // (8 * TILE) * (8 * TILE)
+    x = wl.sparse_buffer(world * chunk, 0.01, seed=wl.stream_seed(0, rank), device=device)
+    out = torch.empty(world * chunk, dtype=torch.float32, device=device)
+    ring = rd.DistRing(chunk, device, strategy="fused", segments=8)
+    for _ in range(max(args.warmup, 3)):
+        ring.all_reduce(x, out, None, None)
+    dist.barrier(); torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ring.log.sent.clear()
+    a.record()
+    for _ in range(args.steps):
+        ring.all_reduce(x, out, None, None)
+    b.record()
+    dist.barrier(); torch.cuda.synchronize()
+    ms = replicas.max_over_ranks(a.elapsed_time(b), device) / args.steps
+    if rank == 0:
+        print(json.dumps({"metric": "sparse ring all-reduce, dense-equivalent GB/s", "value": world * chunk * 4 / ms / 1e6,
+                          "unit": "GB/s (dense-equivalent, per rank)", "n_gpus": world, "steps": args.steps, "ms_per_step": ms,
+                          "config": {"workload": f"config3 recipe over {world} real ranks, chunk {chunk}, fused strategy, 8 segments",
+                                     "transport": dist.get_backend()},
+                          "wire_bytes_per_rank_per_step": ring.log.bytes_sent() // args.steps,
+                          "dense_wire_bytes": 2 * (world - 1) * chunk * 4}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -647,6 +678,7 @@ def main():
     ap.add_argument("--no-rings", action="store_true")
     ap.add_argument("--coo-sweep", action="store_true", help="Pici vs COO kernel by kernel (one JSON line per row)")
     ap.add_argument("--no-coo", action="store_true")
+    ap.add_argument("--dist-ring", action="store_true", help="N > 1 under torchrun: the real ring over NCCL (ring_dist.py)")
     ap.add_argument("--prune", action="store_true", help="time the fused prune-and-compress step only (one JSON line)")
     ap.add_argument("--no-prune", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="sweep rows: eager launches timed one by one (for ncu captures)")
@@ -669,6 +701,13 @@ def main():
     from paper_2607_04676_b200 import pici as pk
     pk.lib()
 
+    if args.dist_ring:
+        if world < 2:
+            raise SystemExit("bench.py --dist-ring needs torchrun with --gpus N >= 2 (one process per GPU)")
+        run_dist_ring(args, rank, world, device)
+        dist.barrier()
+        dist.destroy_process_group()
+        return
     n = 1 << args.log2n
     density = 1.0 - args.sparsity
     peak, peak_src = measured_peak()
