@@ -723,7 +723,8 @@ def main():
         print(json.dumps(run_prune(pk, n, peak, args.sweep_iters, device)), flush=True)
         return
     if args.coo_sweep:
-        for r in run_coo_sweep(pk, n, peak, args.sweep_iters, device):
+        kw = {"sparsities": tuple(float(v) for v in args.sparsities.split(","))} if args.sparsities else {}
+        for r in run_coo_sweep(pk, n, peak, args.sweep_iters, device, **kw):
             print(json.dumps(r), flush=True)
         return
     if args.sweep_only:   # kernel-by-kernel timing (also the program the single-kernel ncu captures run)
