@@ -59,7 +59,10 @@ namespace pici {
 #endif
 constexpr int kCtasPerSm = PICI_MERGE_CTAS;
 constexpr int kWorkers = 16 / kCtasPerSm;                    // worker warps per CTA
-constexpr int kFlushers = 4 / kCtasPerSm;                    // flusher warps per CTA
+#ifndef PICI_MERGE_FLUSHERS
+#define PICI_MERGE_FLUSHERS 4
+#endif
+constexpr int kFlushers = PICI_MERGE_FLUSHERS / kCtasPerSm;  // flusher warps per CTA
 constexpr int kMergeThreads = 32 * (kWorkers + 3 + kFlushers);   // + the planner, the issuer and the publisher warp
 constexpr int kDesc = 8;                                     // items in flight per CTA
 constexpr uint32_t kTileWords = 2 * kSide;                   // u32 words of B per tile
