@@ -216,3 +216,53 @@ void oracle_dense_add_f32(const float *recv, const float *local, uint64_t n, flo
         out[i] = s;
     }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * bf16 reductions (SURVEY.md S8(b) "bf16 reductions are optional: add in fp32, round-to-nearest-even"; reading
+ * DESIGN.md S2 #24): both operands are widened to fp32 exactly (a bf16 is the high half of an fp32), added with
+ * ONE fp32 rounding, and the sum is rounded to bf16 to nearest, ties to even; a NaN sum becomes a quiet NaN that
+ * keeps the sum's sign and high payload bits.  Pinned by torch's bf16 addition in tests/test_oracle_pins.py.
+ * ---------------------------------------------------------------------------------------- */
+static float b16_to_f32(uint16_t h)
+{
+    uint32_t u = (uint32_t)h << 16;
+    float f;
+    memcpy(&f, &u, 4);
+    return f;
+}
+
+static uint16_t f32_to_b16_rne(float f)
+{
+    uint32_t u;
+    memcpy(&u, &f, 4);
+    if ((u & 0x7FFFFFFFu) > 0x7F800000u) return (uint16_t)((u >> 16) | 0x0040u); /* NaN stays NaN */
+    return (uint16_t)((u + 0x7FFFu + ((u >> 16) & 1u)) >> 16);
+}
+
+static uint16_t add_b16(uint16_t a, uint16_t b)
+{
+    volatile float s = b16_to_f32(a) + b16_to_f32(b);
+    return f32_to_b16_rne(s);
+}
+
+/* C4 for bf16: D[i] = bf16(D[i] + a) on set bits, everything else untouched. */
+uint64_t oracle_reduce_sd_b16(const uint64_t *B, const uint32_t *I, const uint16_t *A, uint64_t n, uint16_t *D)
+{
+    uint64_t T = num_tiles(n), k = 0;
+    (void)I;
+    for (uint64_t t = 0; t < T; ++t)
+        for (uint64_t c = 0; c < PICI_SIDE; ++c) {
+            uint64_t w = B[PICI_SIDE * t + c];
+            for (uint64_t r = 0; r < PICI_SIDE; ++r)
+                if ((w >> r) & 1u) {
+                    uint64_t i = PICI_TILE * t + PICI_SIDE * r + c;
+                    D[i] = add_b16(D[i], A[k++]);
+                }
+        }
+    return k;
+}
+
+void oracle_dense_add_b16(const uint16_t *recv, const uint16_t *local, uint64_t n, uint16_t *out)
+{
+    for (uint64_t i = 0; i < n; ++i) out[i] = add_b16(recv[i], local[i]);
+}

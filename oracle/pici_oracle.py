@@ -51,6 +51,8 @@ def lib():
             ("oracle_nnz_dense_b16", [p, u64], u64),
             ("oracle_maybe_densify_f32", [p, p, p, u64, u64, p], ctypes.c_int),
             ("oracle_dense_add_f32", [p, p, u64, p], None),
+            ("oracle_reduce_sd_b16", [p, p, p, u64, p], u64),
+            ("oracle_dense_add_b16", [p, p, u64, p], None),
         ]:
             f = getattr(_lib, name)
             f.argtypes, f.restype = args, res
@@ -124,11 +126,15 @@ def decompress_via_index(x: Pici) -> np.ndarray:
     return D
 
 
-def reduce_sd(x: Pici, dense_inout_f32: np.ndarray) -> None:
-    """dense[i] = dense[i] + a_i on set bits, in place (fp32)."""
-    assert x.dtype == "f32" and dense_inout_f32.dtype == np.float32 and dense_inout_f32.size == x.n
-    lib().oracle_reduce_sd_f32(_ptr(x.B), _ptr(x.I), _ptr(x.A) if x.A.size else None, x.n,
-                               _ptr(dense_inout_f32))
+def reduce_sd(x: Pici, dense_inout: np.ndarray) -> None:
+    """dense[i] = dense[i] + a_i on set bits, in place: float32, or bf16 bits as uint16 (add in fp32, round RNE)."""
+    assert dense_inout.size == x.n
+    if x.dtype == "f32":
+        assert dense_inout.dtype == np.float32
+        lib().oracle_reduce_sd_f32(_ptr(x.B), _ptr(x.I), _ptr(x.A) if x.A.size else None, x.n, _ptr(dense_inout))
+    else:
+        assert dense_inout.dtype == np.uint16
+        lib().oracle_reduce_sd_b16(_ptr(x.B), _ptr(x.I), _ptr(x.A) if x.A.size else None, x.n, _ptr(dense_inout))
 
 
 def reduce_ss(x: Pici, y: Pici) -> Pici:
@@ -161,8 +167,10 @@ def maybe_densify(x: Pici, nnz_switch: int, dense_out_bits: np.ndarray) -> bool:
                                                x.n, int(nnz_switch), _ptr(dense_out_bits)))
 
 
-def dense_add(recv_f32: np.ndarray, local_f32: np.ndarray) -> np.ndarray:
-    assert recv_f32.dtype == local_f32.dtype == np.float32 and recv_f32.size == local_f32.size
-    out = np.empty_like(recv_f32)
-    lib().oracle_dense_add_f32(_ptr(recv_f32), _ptr(local_f32), recv_f32.size, _ptr(out))
+def dense_add(recv: np.ndarray, local: np.ndarray) -> np.ndarray:
+    """recv + local elementwise: float32, or bf16 bits as uint16 (add in fp32, round RNE)."""
+    assert recv.dtype == local.dtype and recv.size == local.size and recv.dtype in (np.float32, np.uint16)
+    out = np.empty_like(recv)
+    fn = lib().oracle_dense_add_f32 if recv.dtype == np.float32 else lib().oracle_dense_add_b16
+    fn(_ptr(recv), _ptr(local), recv.size, _ptr(out))
     return out

@@ -340,3 +340,30 @@ def test_tiny_brute_force_python_loops():
     for t, c, r, _ in triples:
         assert (int(p.B[64 * t + c]) >> r) & 1
     assert sum(bin(int(w)).count("1") for w in p.B) == len(triples)
+
+
+# ---------------------------------------------------------------------------------------------
+# bf16 reductions: "add in fp32, round-to-nearest-even" - pinned by torch's bf16 addition, a library
+# routine that widens to fp32, adds and rounds RNE
+# ---------------------------------------------------------------------------------------------
+
+def test_bf16_dense_add_and_reduce_sd_are_torch_bf16_addition():
+    n = 3 * 4096 + 17
+    a = wl.sparse_buffer(n, 0.3, seed=21, dtype="bf16")
+    b = wl.sparse_buffer(n, 0.6, seed=22, dtype="bf16")
+    b[::5] = -a[::5]                                                  # cancellations
+    a[7], b[7] = 1.0, 2.0 ** -8                                       # a tie: 1 + 2^-8 rounds to even (1.0)
+    a[8], b[8] = 1.0 + 2.0 ** -7, 2.0 ** -8                           # a tie that rounds up to even
+    a[9], b[9] = 3.0e38, 3.0e38                                       # overflow to +inf
+    want = (a + b)                                                    # torch: fp32 add, RNE to bf16
+    got = po.dense_add(b16bits(a), b16bits(b))
+    assert np.array_equal(got, b16bits(want))
+    assert got[7] == 0x3F80 and got[8] == 0x3F82 and got[9] == 0x7F80
+    x = po.compress(b16bits(a), "bf16")
+    acc = b16bits(b).copy()
+    po.reduce_sd(x, acc)
+    mask = (a != 0).numpy()
+    ref = np.where(mask, b16bits(a + b), b16bits(b))                  # untouched where a has no value
+    assert np.array_equal(acc, ref)
+    nan = po.dense_add(np.array([0x7FC1, 0x7F80], np.uint16), np.array([0x3F80, 0xFF80], np.uint16))
+    assert (nan[0] & 0x7FFF) > 0x7F80 and (nan[1] & 0x7FFF) > 0x7F80  # NaN + 1 and inf - inf are NaN
