@@ -40,8 +40,10 @@
  *   - Thread safety: calls may be made from several host threads (one stream and one workspace per thread); the
  *     only shared state is a per-device "kernel attributes set" flag, kept in atomics.
  *   - Limits: 0 <= n < 2^32 (I is 32-bit).  n == 0 is valid: I[0] = 0 is written.
- *   - dtype: PICI_F32 or PICI_BF16 for compress / decompress / nnz / maybe_densify;
- *     reductions (reduce_sd, reduce_ss, dense_add) are PICI_F32 only (PICI_ERR_DTYPE otherwise).
+ *   - dtype: PICI_F32 or PICI_BF16 for compress / decompress / nnz / maybe_densify / reduce_sd / dense_add; a bf16
+ *     sum is taken in fp32 (both operands widened exactly, one fp32 add) and rounded to nearest even (SURVEY.md
+ *     S8(b)), and bf16 reduce_sd always streams the dense buffer (the read-modify-write regime is fp32).
+ *     reduce_ss and the ring engine are PICI_F32 only (PICI_ERR_DTYPE otherwise).
  *   - Return value: PICI_OK (0) or a negative PICI_ERR_* code; pici_strerror() names it.  No call
  *     throws, aborts or prints.
  *   - Gating: calls that take `d_gate` run only if d_gate == NULL or *d_gate == gate_value when the
@@ -104,7 +106,7 @@ int pici_decompress(const uint64_t *B, const uint32_t *I, const void *A, uint64_
 
 /* a5. reduce_sd, the scatter-add "decompression" used by reduce-scatter / all-reduce
  * (PAPER.md:193, 219): dense_inout[i] = dense_inout[i] + a_i for every set bit, one fp32 add each;
- * all other elements are left untouched (bit-exact, a -0.0 there survives).  fp32 only. */
+ * all other elements are left untouched (bit-exact, a -0.0 there survives).  fp32 or bf16 (see "dtype"). */
 int pici_reduce_sd(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
                    void *dense_inout, void *stream);
 
@@ -157,7 +159,7 @@ int pici_maybe_densify_gated(const uint64_t *B, const uint32_t *I, const void *A
                              uint64_t nnz_switch, void *dense_out, int32_t *d_fmt_out,
                              const int32_t *d_gate, int32_t gate_value, void *stream);
 
-/* out[i] = recv[i] + local[i] in fp32 (the dense ring step once a chunk has switched, the paper's
+/* out[i] = recv[i] + local[i], fp32 or bf16 (the dense ring step once a chunk has switched, the paper's
  * reduceCopy).  Runs only if the gate is open; then also sets *d_fmt_out (if not
  * NULL) to PICI_FMT_DENSE.  out may alias recv or local. */
 int pici_dense_add_gated(const void *recv, const void *local, uint64_t n, int dtype, void *out,

@@ -40,7 +40,6 @@ int do_expand(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, i
               void *out, int mode, DensifyCtl ctl, Gate g, void *stream) {
     int rc = check_pici(B, I, A, n, dtype);
     if (rc != PICI_OK) return rc;
-    if (mode == 1 && dtype != PICI_F32) return PICI_ERR_DTYPE;
     if (n != 0 && out == nullptr && ctl.d_flag == nullptr) return PICI_ERR_INVALID_ARG;
     if (n != 0 && mode == 1 && local == nullptr) return PICI_ERR_INVALID_ARG;
     if (!aligned(out, 16) || !aligned(local, 16)) return PICI_ERR_ALIGN;
@@ -181,12 +180,12 @@ int pici_maybe_densify_gated(const uint64_t *B, const uint32_t *I, const void *A
 int pici_dense_add_gated(const void *recv, const void *local, uint64_t n, int dtype, void *out, int32_t *d_fmt_out,
                          const int32_t *d_gate, int32_t gate_value, void *stream) {
     if (bad_dtype(dtype)) return PICI_ERR_DTYPE;
-    if (dtype != PICI_F32) return PICI_ERR_DTYPE;
     if (n >= kMaxN || (n != 0 && (recv == nullptr || local == nullptr || out == nullptr))) return PICI_ERR_INVALID_ARG;
     if (d_fmt_out != nullptr && d_fmt_out == d_gate) return PICI_ERR_INVALID_ARG;
     if (!aligned(recv, 16) || !aligned(local, 16) || !aligned(out, 16)) return PICI_ERR_ALIGN;
-    return cuda_rc(launch_dense_add(recv, local, n, out, d_fmt_out, gate_eq(d_gate, gate_value),
-                                    static_cast<cudaStream_t>(stream)));
+    return cuda_rc((dtype == PICI_F32 ? launch_dense_add : launch_dense_add_bf16)(recv, local, n, out, d_fmt_out,
+                                                                                 gate_eq(d_gate, gate_value),
+                                                                                 static_cast<cudaStream_t>(stream)));
 }
 
 int pici_dense_copy_gated(const void *src, void *dst, uint64_t n, int dtype, const int32_t *d_gate, int32_t gate_value,

@@ -13,8 +13,9 @@
 //     above 25 %, not a COO regime) takes its look-back at once and writes from registers;
 //   * decompress / merge find a block's index range in `off` (off[t] = first entry with idx >= 4096 t), built by a
 //     streaming pre-pass over idx (what Pici's I gives for free); decompress assembles the block in shared memory and
-//     writes every dense byte once; the merge scatters X then Y into a shared-memory block with a candidate
-//     bitmap, re-applies the predicate to the sums and emits survivors in ascending order behind a look-back;
+//     writes every dense byte once; the merge keeps two presence bitmaps per warp in shared memory, reads the values
+//     from the lists at popcount-prefix cursors, re-applies the predicate to the sums and emits survivors in
+//     ascending order behind a deferred look-back;
 //   * reduce_sd is the bare read-modify-write of the touched elements.
 #include <atomic>
 

@@ -95,8 +95,8 @@ expand_kernel(const Batch<ExpandJob> batch) {
     const DensifyCtl ctl = job.ctl;
 
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
-    if constexpr (MODE == kModeAdd) {  // in place: the sparse regime belongs to scatter_add_sparse_kernel
-        if (local == out && sparse_regime(I, T)) return;
+    if constexpr (MODE == kModeAdd && DT == PICI_F32) {  // in place: the sparse regime belongs to scatter_add_sparse_kernel
+        if (local == out && sparse_regime(I, T)) return;       // (bf16 sums always stream: include/pici.h)
     }
     if (ctl.d_flag != nullptr) {  // maybe_densify: integer compare on the measured nnz (C9 #9/#10)
         const bool switched = (uint64_t)I[T] >= ctl.nnz_switch;
@@ -144,6 +144,8 @@ expand_kernel(const Batch<ExpandJob> batch) {
 
         if constexpr (MODE == kModeAdd) {
             if (in_place && tile_nnz == 0) continue;
+        }
+        if constexpr (MODE == kModeAdd && DT == PICI_F32) {
             if (in_place && tile_nnz <= kSparseTileNnz) {
                 // ---- sparse form: index list, then batched gather / add / scatter ------------------
                 uint16_t *list = reinterpret_cast<uint16_t *>(stage_raw);
@@ -222,10 +224,18 @@ expand_kernel(const Batch<ExpandJob> batch) {
 #pragma unroll
             for (int c = 0; c < kSide / kChunk; ++c) {
                 uint2 loc[kChunk];
-                if constexpr (MODE == kModeAdd) {
+                if constexpr (MODE == kModeAdd && DT == PICI_F32) {
                     const uint2 *src = reinterpret_cast<const uint2 *>(Lin + base) + lane;
 #pragma unroll
                     for (int j = 0; j < kChunk; ++j) loc[j] = ld_coherent_u2(src + 32 * (kChunk * c + j));
+                } else if constexpr (MODE == kModeAdd) {      // bf16: a row is 128 bytes, one 32-bit word per lane
+                    const uint32_t *src = reinterpret_cast<const uint32_t *>(Lin + base) + lane;
+#pragma unroll
+                    for (int j = 0; j < kChunk; ++j) {
+                        uint32_t x;
+                        asm volatile("ld.global.L1::no_allocate.u32 %0, [%1];" : "=r"(x) : "l"(src + 32 * (kChunk * c + j)) : "memory");
+                        loc[j].x = x;
+                    }
                 }
                 if (c == 0) {
                     if (bulk != 0) {
@@ -258,6 +268,11 @@ expand_kernel(const Batch<ExpandJob> batch) {
                         if (b0) v.x = __float_as_uint(__fadd_rn(__uint_as_float(v.x), __uint_as_float(stage[k0++])));
                         if (b1) v.y = __float_as_uint(__fadd_rn(__uint_as_float(v.y), __uint_as_float(stage[k1++])));
                         stg_stream_u2(reinterpret_cast<uint2 *>(Dout + base) + lane + 32 * r, v);
+                    } else {                                  // bf16: columns 2l (low half) and 2l + 1 (high half)
+                        uint32_t lo = loc[j].x & 0xFFFFu, hi = loc[j].x >> 16;
+                        if (b0) lo = bf16_add_bits(lo, stage[k0++]);
+                        if (b1) hi = bf16_add_bits(hi, stage[k1++]);
+                        stg_stream_u32(reinterpret_cast<uint32_t *>(Dout + base) + lane + 32 * r, lo | (hi << 16));
                     }
                 }
             }
@@ -286,6 +301,15 @@ expand_kernel(const Batch<ExpandJob> batch) {
                     if (i0 + 1 < valid) {
                         const uint32_t l1 = Lin[base + i0 + 1];
                         Dout[base + i0 + 1] = b1 ? __float_as_uint(__fadd_rn(__uint_as_float(l1), __uint_as_float(a1))) : l1;
+                    }
+                } else {
+                    if (i0 < valid) {
+                        const uint16_t l0 = Lin[base + i0];
+                        Dout[base + i0] = b0 ? (uint16_t)bf16_add_bits(l0, a0) : l0;
+                    }
+                    if (i0 + 1 < valid) {
+                        const uint16_t l1 = Lin[base + i0 + 1];
+                        Dout[base + i0 + 1] = b1 ? (uint16_t)bf16_add_bits(l1, a1) : l1;
                     }
                 }
             }
@@ -452,7 +476,8 @@ static cudaError_t launch_expand_t(const ExpandJob *jobs, int count, cudaStream_
 cudaError_t launch_expand_batch(const ExpandJob *jobs, int count, int dtype, int mode, cudaStream_t s) {
     if (count <= 0) return cudaSuccess;
     if (count > kMaxBatch) return cudaErrorInvalidValue;
-    if (mode == kModeAdd) return launch_expand_t<PICI_F32, kModeAdd>(jobs, count, s);
+    if (mode == kModeAdd)
+        return dtype == PICI_F32 ? launch_expand_t<PICI_F32, kModeAdd>(jobs, count, s) : launch_expand_t<PICI_BF16, kModeAdd>(jobs, count, s);
     return dtype == PICI_F32 ? launch_expand_t<PICI_F32, kModeDecompress>(jobs, count, s)
                              : launch_expand_t<PICI_BF16, kModeDecompress>(jobs, count, s);
 }
@@ -460,7 +485,7 @@ cudaError_t launch_expand_batch(const ExpandJob *jobs, int count, int dtype, int
 cudaError_t launch_expand(const uint64_t *B, const uint32_t *I, const void *A, uint64_t n, int dtype,
                           const void *local, void *out, int mode, DensifyCtl ctl, Gate g, cudaStream_t s) {
     if (n == 0 && ctl.d_flag == nullptr) return cudaSuccess;
-    if (mode == kModeAdd && local == out) {  // in place: the sparse-regime kernel and the streaming kernel pick on the device
+    if (mode == kModeAdd && local == out && dtype == PICI_F32) {  // in place: the sparse-regime kernel and the streaming kernel pick on the device
         cudaError_t e = launch_scatter_add_sparse(B, I, A, n, out, g, s);
         if (e != cudaSuccess) return e;
     }

@@ -105,6 +105,8 @@ struct DenseAddJob {
     Gate gate;
 };
 cudaError_t launch_dense_add_batch(const DenseAddJob *jobs, int count, cudaStream_t s);
+cudaError_t launch_dense_add_bf16(const void *recv, const void *local, uint64_t n, void *out, int32_t *d_fmt_out, Gate g,
+                                  cudaStream_t s);
 cudaError_t launch_dense_add(const void *recv, const void *local, uint64_t n, void *out, int32_t *d_fmt_out,
                              Gate g, cudaStream_t s);
 

@@ -132,6 +132,39 @@ cudaError_t launch_dense_add(const void *recv, const void *local, uint64_t n, vo
     return launch_dense_add_batch(&job, 1, s);
 }
 
+// bf16: out[i] = bf16(recv[i] + local[i]) - widened to fp32, one fp32 add, rounded to nearest even (pici_common.cuh).
+__global__ void __launch_bounds__(256) dense_add_bf16_kernel(const DenseAddJob job) {
+    if (gate_closed(job.gate.ptr, job.gate.mask, job.gate.value)) return;
+    const uint16_t *recv = reinterpret_cast<const uint16_t *>(job.recv), *local = reinterpret_cast<const uint16_t *>(job.local);
+    uint16_t *out = reinterpret_cast<uint16_t *>(job.out);
+    const uint64_t n = job.n;
+    if (job.d_fmt_out != nullptr && blockIdx.x == 0 && threadIdx.x == 0) *job.d_fmt_out = PICI_FMT_DENSE;
+    const uint64_t nvec = n / 8;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint4 *a = reinterpret_cast<const uint4 *>(recv), *b = reinterpret_cast<const uint4 *>(local);
+    uint4 *o = reinterpret_cast<uint4 *>(out);
+    auto add2 = [](uint32_t x, uint32_t y) {
+        return bf16_add_bits(x & 0xFFFFu, y & 0xFFFFu) | (bf16_add_bits(x >> 16, y >> 16) << 16);
+    };
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+        const uint4 x = ldg_stream_u4(a + i), y = ldg_stream_u4(b + i);
+        stg_stream_u4(o + i, make_uint4(add2(x.x, y.x), add2(x.y, y.y), add2(x.z, y.z), add2(x.w, y.w)));
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        for (uint64_t j = nvec * 8; j < n; ++j) out[j] = (uint16_t)bf16_add_bits(recv[j], local[j]);
+}
+
+cudaError_t launch_dense_add_bf16(const void *recv, const void *local, uint64_t n, void *out, int32_t *d_fmt_out, Gate g,
+                                  cudaStream_t s) {
+    const DenseAddJob job = {recv, local, n, out, d_fmt_out, g};
+    uint64_t blocks = (n / 8 + 255) / 256;
+    const uint64_t cap = (uint64_t)num_sms() * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks == 0) blocks = 1;
+    dense_add_bf16_kernel<<<(unsigned)blocks, 256, 0, s>>>(job);
+    return cudaGetLastError();
+}
+
 // dst[i] = src[i] (bit copy), gated: a dense message landing in its all-gather slot.
 __global__ void __launch_bounds__(256) dense_copy_kernel(const Batch<DenseCopyJob> batch) {
     const DenseCopyJob &job = batch.job[blockIdx.y];

@@ -22,6 +22,15 @@ __device__ __forceinline__ bool nz32(uint32_t u) { return (u & 0x7FFFFFFFu) != 0
 __device__ __forceinline__ bool nz16lo(uint32_t u) { return (u & 0x00007FFFu) != 0u; }
 __device__ __forceinline__ bool nz16hi(uint32_t u) { return (u & 0x7FFF0000u) != 0u; }
 
+// ---- bf16 arithmetic of the reductions (include/pici.h: add in fp32, round to nearest even) -----------------------
+// A bf16 is the high half of an fp32, so widening is exact; the sum takes ONE fp32 rounding (__fadd_rn) and one
+// rounding to bf16 (ties to even); a NaN sum stays a (quiet) NaN with the sum's sign and high payload bits.
+__device__ __forceinline__ uint32_t bf16_add_bits(uint32_t a16, uint32_t b16) {   // operands and result in the low 16 bits
+    const uint32_t u = __float_as_uint(__fadd_rn(__uint_as_float(a16 << 16), __uint_as_float(b16 << 16)));
+    if ((u & 0x7FFFFFFFu) > 0x7F800000u) return (u >> 16) | 0x0040u;
+    return (u + 0x7FFFu + ((u >> 16) & 1u)) >> 16;
+}
+
 // ---- streaming global accesses ---------------------------------------------------------------
 __device__ __forceinline__ uint2 ldg_stream_u2(const uint2 *p) {
     uint2 v;

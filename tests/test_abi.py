@@ -126,7 +126,7 @@ def test_sizes_and_calls_reject_bad_arguments_without_touching_the_device():
     assert S(a, a, a, a, a, a, n, pici.BF16, a, a, a, n, a, ws.value, None) == DTYPE       # reductions are fp32 only
     assert S(a, a, a, a, a, a, n, pici.F32, a, a, a, n - 1, a, ws.value, None) == CAPACITY
     assert S(a, a, a, a, None, a, n, pici.F32, a, a, a, n, a, ws.value, None) == INVALID
-    assert lib.pici_reduce_sd(a, a, a, n, pici.BF16, a, None) == DTYPE
+    assert lib.pici_reduce_sd(a, a, a, n, 7, a, None) == DTYPE                               # unknown dtype (bf16 sums exist)
     assert lib.pici_decompress(a, a, a, n, pici.F32, None, None) == INVALID
     assert lib.pici_decompress(a, a, a, n, pici.F32, a + 4, None) == ALIGN
     for code in (0, INVALID, DTYPE, ALIGN, CAPACITY, WORKSPACE, -6, -99):

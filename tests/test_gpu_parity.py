@@ -308,3 +308,39 @@ def test_probe_random_rmw_adds_one_at_the_indices(pk):
     want = d.clone()
     want[idx.cpu().long()] += 1.0
     assert torch.equal(got.cpu().view(torch.int32), want.view(torch.int32))
+
+
+@pytest.mark.parametrize("n,dens", [(4096, 0.5), (4097, 0.01), (70001, 0.3), ((1 << 20) + 5, 0.02), (1 << 20, 1.0), (1 << 18, 0.0)])
+def test_bf16_reductions_match_oracle(pk, n, dens):
+    """bf16 reduce_sd (in place and with a separate output) and dense add: widened to fp32, one add, rounded to nearest
+    even - bit-exact with the oracle (which is pinned to torch's bf16 addition); untouched elements keep their bits."""
+    xh = wl.sparse_buffer(n, dens, seed=n + 3, dtype="bf16")
+    yh = wl.sparse_buffer(n, 0.7, seed=n + 4, dtype="bf16")
+    yh[::9] = -xh[::9]
+    yb = _bits(yh).copy()
+    yb[1::13] = 0x8000                                              # -0.0 in the dense operand survives where x has no value
+    yh = torch.from_numpy(yb.view(np.int16)).view(torch.bfloat16)
+    xo = po.compress(_bits(xh), "bf16")
+    want = yb.copy()
+    po.reduce_sd(xo, want)
+    acc = yh.clone().cuda()
+    pk.reduce_sd(_upload(pk, xo), acc)
+    assert np.array_equal(_bits(acc), want)
+    out = torch.full((n,), 7.0, dtype=torch.bfloat16, device="cuda")
+    pk.reduce_sd_out(_upload(pk, xo), yh.cuda(), out)
+    assert np.array_equal(_bits(out), want)
+    got = torch.empty(n, dtype=torch.bfloat16, device="cuda")
+    pk.dense_add(xh.cuda(), yh.cuda(), got)
+    assert np.array_equal(_bits(got), po.dense_add(_bits(xh), yb))
+
+
+def test_bf16_reduce_sd_full_size(pk):
+    """N = 2^28 bf16: the scatter-add equals torch's bf16 addition on the whole buffer."""
+    n = 1 << 28
+    x = wl.sparse_buffer(n, 0.05, seed=0, dtype="bf16", device="cuda")
+    y = wl.sparse_buffer(n, 0.5, seed=1, dtype="bf16", device="cuda")
+    px = pk.alloc_pici(n, pk.BF16)
+    pk.compress(x, px, pk.alloc_workspace(n))
+    acc = y.clone()
+    pk.reduce_sd(px, acc)
+    assert torch.equal(acc.view(torch.int16), (x + y).view(torch.int16))
