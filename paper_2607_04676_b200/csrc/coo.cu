@@ -409,9 +409,9 @@ static cudaError_t allow_smem(K kernel, size_t smem, std::atomic<bool> (&done)[6
     }
     return cudaSuccess;
 }
-static unsigned persistent_grid(uint64_t T) {
+static unsigned persistent_grid(uint64_t T, uint64_t waves = 1) {   // waves > 1: the block scheduler balances the SMs
     uint64_t blocks = (T + kCooWarps - 1) / kCooWarps;
-    const uint64_t cap = (uint64_t)num_sms() * 3;
+    const uint64_t cap = (uint64_t)num_sms() * 3 * waves;
     return (unsigned)(blocks > cap ? cap : (blocks ? blocks : 1));
 }
 
@@ -449,7 +449,7 @@ static cudaError_t launch_coo_decompress(const uint32_t *idx, const void *val, c
     e = launch_coo_offsets(idx, d_nnz, w.offx, nullptr, nullptr, nullptr, n, s);
     if (e != cudaSuccess) return e;
     const CooExpandArgs a = {idx, reinterpret_cast<const uint32_t *>(val), w.offx, reinterpret_cast<uint32_t *>(dense), n};
-    coo_decompress_kernel<<<persistent_grid((n + kTile - 1) / kTile), kCooWarps * 32, smem, s>>>(a);
+    coo_decompress_kernel<<<persistent_grid((n + kTile - 1) / kTile, 12), kCooWarps * 32, smem, s>>>(a);   // write-bound: see expand.cu
     return cudaGetLastError();
 }
 
