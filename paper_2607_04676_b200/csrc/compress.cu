@@ -24,6 +24,10 @@
 namespace pici {
 
 constexpr int kCompressWarps = 4;
+#ifndef PICI_COMPRESS_DEFER
+#define PICI_COMPRESS_DEFER 2
+#endif
+constexpr int kDefer = PICI_COMPRESS_DEFER;   // iterations a tile's look-back and flush lag behind its publish
 constexpr uint32_t kRowSkipNnz = 256;   // tiles with at most this many values skip empty rows in Phase 3
 
 template <int DT>
@@ -33,13 +37,93 @@ struct CompressCfg<PICI_F32> {
     using Elem = uint32_t;
     static constexpr int kRegs = 128;       // 64 rows x 2 columns
     static constexpr int kMinBlocks = 3;    // 12 warps / SM, <= 168 registers
+    static constexpr uint32_t kScanBlockLog = 8;
 };
 template <>
 struct CompressCfg<PICI_BF16> {
     using Elem = uint16_t;
     static constexpr int kRegs = 64;        // 64 rows x (2 packed columns)
     static constexpr int kMinBlocks = 5;
+    static constexpr uint32_t kScanBlockLog = 9;
 };
+
+// ---- Phase 2 as a service ---------------------------------------------------------------------------------------------
+// The device-wide exclusive scan of the tile counts is not taken by the warps that compress (a decoupled look-back
+// cost them 3.5 - 4.7 dependent L2 round trips per tile: the whole gap between 0.79 and 1.03 of the HBM peak) but by
+// the four warps of CTA 0: warp w takes the 1024-tile blocks b = w, w + 4, ...; it waits until the block's counts are
+// all published (tickets hand tiles out in order, so that is when the front of the launch has passed it), scans them
+// (32 coalesced 256-byte rows of status words, a warp scan per row), receives the block's base from the warp that
+// scanned block b - 1 through shared memory, writes I for the block - I itself is the result - and marks the block
+// done (a word tagged with the launch epoch).  A compressing warp flushes a tile two iterations after publishing
+// its count; by then the block is normally done and the flush costs one load of the done word and one of I[t].
+struct ScanShared {
+    volatile uint32_t seq;    // blocks whose base has been handed on
+    volatile uint32_t base;   // exclusive prefix of block `seq`
+};
+// log2 of the scan block: 256 tiles (fp32) / 512 (bf16) for a full-size launch - measured at N = 2^28, 99 %: blocks of
+// 256 / 512 / 1024 tiles give fp32 0.169 / 0.169 / 0.177 ms and bf16 0.180 / 0.137 / 0.156 (small blocks: the service's
+// four warps, one L2 round trip per poll, fall behind bf16's tile rate; large blocks: a tile waits longer for the rest
+// of its block, and at 50 % sparsity, where a tile is flushed one iteration after its publish, 512 / 1024 stall:
+// fp32 0.270 / 0.519 / 0.628) - smaller when the launch has few warps, so that the tiles one warp takes one after the
+// other (about `warps` apart) fall into different blocks (see flush_one)
+__device__ __forceinline__ uint32_t scan_block_log(uint32_t worker_warps, uint32_t max_log) {
+    const uint32_t half = max(worker_warps / 2u, 32u);
+    return min(31u - (uint32_t)__clz(half), max_log);
+}
+__device__ __forceinline__ void scan_service(ScanShared &sh, uint64_t *blk_done, const uint64_t *status, uint32_t tag,
+                                             uint32_t T, uint32_t sb_log, uint32_t *__restrict__ I, int warp, int lane) {
+    const uint32_t sb = 1u << sb_log, rows = sb >> 5;
+    const uint32_t nblk = (T + sb - 1u) >> sb_log;
+    for (uint32_t b = (uint32_t)warp; b < nblk; b += kCompressWarps) {
+        const uint32_t t0 = b << sb_log;
+        uint32_t cnt[32];
+        uint64_t w[32];
+        // all rows are requested together (one L2 round trip for the block) and the whole block is read again until
+        // every word carries the tag
+        for (;;) {
+            bool ok = true;
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {      // row i: tiles t0 + 32 i + lane
+                const uint32_t t = t0 + 32u * i + (uint32_t)lane;
+                w[i] = ((uint32_t)i < rows && t < T) ? ld_status(status + t) : ((uint64_t)tag << 32);   // others count 0
+            }
+#pragma unroll
+            for (int i = 0; i < 32; ++i) ok = ok && tagged(w[i], tag);
+            if (__all_sync(kFull, ok)) break;
+            __nanosleep(500);
+        }
+#pragma unroll
+        for (int i = 0; i < 32; ++i) cnt[i] = (uint32_t)w[i];
+        uint32_t run = 0;                   // block-local exclusive prefixes, in place
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            if ((uint32_t)i < rows) {       // warp-uniform
+                const uint32_t incl = warp_incl_scan(cnt[i], lane);
+                const uint32_t tot = __shfl_sync(kFull, incl, 31);
+                cnt[i] = run + incl - cnt[i];
+                run += tot;
+            }
+        }
+        uint32_t base = 0;
+        if (lane == 0) {
+            while (sh.seq != b) __nanosleep(32);
+            base = sh.base;
+            sh.base = base + run;           // hand the next block its base before the stores below
+            __threadfence_block();
+            sh.seq = b + 1u;
+        }
+        base = __shfl_sync(kFull, base, 0);
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            const uint32_t t = t0 + 32u * i + (uint32_t)lane;
+            if ((uint32_t)i < rows && t < T) I[t] = base + cnt[i];
+        }
+        if (b + 1u == nblk && lane == 0) I[T] = base + run;
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) st_status(blk_done + b, tag, base + run);   // done; the value is the prefix at the block's end
+    }
+}
 
 // PRUNE (fp32 only): the tile that is compressed is not read but MADE while it is loaded - sampled top-k pruning with
 // leaky error feedback fused into the same pass (include/pici_prune.h): acc = g + leak * e (two
@@ -61,7 +145,8 @@ compress_kernel(const Batch<CompressJob> batch) {
     uint32_t *__restrict__ I = job.I;
     void *__restrict__ A = job.A;
     void *const ws = job.ws;
-    uint64_t *const status = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes) + kWsAccWords;
+    uint64_t *const blk_acc = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(ws) + kWsHeaderBytes);
+    uint64_t *const status = blk_acc + kWsAccWords;   // one tagged count per tile
     // [ticket, warps that have left] live behind the workspace header; the launch's last warp resets them and
     // advances the epoch, so no launch starts with a memset (status words carry the epoch, pici_common.cuh)
     uint32_t *const ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + kWsCompressTicket);
@@ -69,8 +154,23 @@ compress_kernel(const Batch<CompressJob> batch) {
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    Elem *stage = reinterpret_cast<Elem *>(smem_raw) + warp * kTile;
+    // tiles come from one of several ticket counters (pici_common.cuh "tile tickets from SEVERAL counters")
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile);
+    const uint32_t worker_ctas = gridDim.x - 1u;            // CTA 0 of every job is the scan service
+    if (blockIdx.x == 0) {
+        __shared__ ScanShared scan_sh;
+        if (threadIdx.x == 0) {
+            scan_sh.seq = 0;
+            scan_sh.base = 0;
+        }
+        __syncthreads();
+        scan_service(scan_sh, blk_acc, status, tag, T, scan_block_log(worker_ctas * (uint32_t)kCompressWarps, Cfg::kScanBlockLog), I, warp, lane);
+        return;
+    }
+    const uint32_t cC = ticket_counters(worker_ctas * (uint32_t)kCompressWarps);
+    const uint32_t cj = ((blockIdx.x - 1u) * (uint32_t)kCompressWarps + (uint32_t)warp) % cC;
+    uint32_t *const tk = ticket_counter(ws, T, cj);
+    Elem *stage = reinterpret_cast<Elem *>(smem_raw) + warp * kTile;
     const uint32_t Tfull = (uint32_t)(n / kTile);
     Elem *Aout = reinterpret_cast<Elem *>(A);
 
@@ -158,32 +258,95 @@ compress_kernel(const Batch<CompressJob> batch) {
     };
 
     uint32_t v[Cfg::kRegs];
-    uint32_t t = next_ticket(ticket, lane);
+    uint32_t t = 0;
+    if (lane == 0) t = ticket_tile(tk, cC, cj);
+    t = __shfl_sync(kFull, t, 0);
     if (t < Tfull) load_full(t, v);
     else if (t < T) load_ragged(t, v);
 
-    // Per-warp software pipeline.  A tile's count is published as soon as its data has arrived and
-    // Phase 1 is done; its look-back (and the flush of its compacted values) is deferred until AFTER
-    // the next tile's count has been published, so the look-back latency hides behind the next tile
-    // and no count is ever held back by a wait.
-    bool pending = false;       // stage holds the compacted values of tile pt, not yet flushed
-    uint32_t pt = 0, pnnz = 0;
-    auto flush_pending = [&]() {
-        if (pending) {
-            const uint32_t excl = lookback_prefix(status, tag, pt, pnnz, T, I, lane);
-            Elem *dst = Aout + excl;
-            for (uint32_t i = lane; i < pnnz; i += 32) dst[i] = stage[i];
-            __syncwarp();
-            pending = false;
+    // Per-warp software pipeline.  A tile's count is published as soon as its data has arrived and Phase 1 is done; its
+    // look-back (and the flush of its compacted values) is deferred until kDefer later tiles of this warp have published
+    // theirs.  The look-back waits for the counts of the 32 tiles below, and those tiles are HELD by other warps - a
+    // warp claims its next tile a whole iteration before it can publish it - so a look-back taken one iteration late
+    // still found unpublished tiles and spun: with the publish and the look-back compiled out the kernel ran at 1.03
+    // (fp32) / 0.98 (bf16) of the HBM peak instead of 0.79 / 0.57.  Deferring by kDefer = 2 iterations gives the tiles
+    // below one more iteration to appear.  The stage is cut into kDefer + 1 slots for that; a tile with more values
+    // than a slot holds (denser than ~67 % sparsity) takes the whole stage and everything pending is flushed first.
+    constexpr uint32_t kSlot = kTile / (kDefer + 1);
+    uint32_t q_t[kDefer], q_n[kDefer], q_o[kDefer];   // pending tiles, oldest first: tile, count, stage offset
+    bool q_on[kDefer];
+#pragma unroll
+    for (int i = 0; i < kDefer; ++i) q_on[i] = false;
+    bool wide_pending = false;     // a pending tile lies across the slots
+    uint32_t seq = 0;
+    const uint32_t sb_log = scan_block_log(worker_ctas * (uint32_t)kCompressWarps, Cfg::kScanBlockLog);
+    uint32_t held = 0xFFFFFFFFu;   // the tile this warp has claimed but not yet published (>= T: none)
+    auto wait_done = [&](uint32_t b) -> uint32_t {   // prefix at the end of scan block b, once the service has it
+        const uint64_t *done = blk_acc + b;
+        unsigned ns = 16;
+        uint64_t v;
+        while (!tagged(v = ld_status(done), tag)) {
+            __nanosleep(ns);
+            if (ns < 128) ns += ns;
         }
+        return (uint32_t)v;
+    };
+    auto flush_one = [&](uint32_t pt, uint32_t pnnz, uint32_t off) {
+        // The scan service finishes a block only when EVERY tile of it has published its count - also the tile this
+        // warp holds unpublished.  So the warp waits for the service only if that tile lies in a later block (blocks
+        // then resolve in increasing order: no cycle); otherwise - small launches, the tail of a launch - it takes the
+        // prefix itself: the end of the block below plus the counts of the tiles of its own block below pt (all of
+        // them lower than anything this warp holds).
+        const uint32_t bq = pt >> sb_log;
+        uint32_t excl;
+        if (held >= T || bq < (held >> sb_log)) {
+            wait_done(bq);
+            asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(excl) : "l"(I + pt) : "memory");
+        } else {
+            excl = bq ? wait_done(bq - 1u) : 0u;
+            uint32_t part = 0;
+            for (uint32_t u0 = bq << sb_log; u0 < pt; u0 += 32u) {
+                const uint32_t u = u0 + (uint32_t)lane;
+                uint64_t v = (uint64_t)tag << 32;
+                if (u < pt) {
+                    unsigned ns = 16;
+                    while (!tagged(v = ld_status(status + u), tag)) {
+                        __nanosleep(ns);
+                        if (ns < 128) ns += ns;
+                    }
+                }
+                part += (uint32_t)v;
+            }
+            excl += warp_sum(part);
+        }
+        Elem *dst = Aout + excl;
+        const Elem *src = stage + off;
+        for (uint32_t i = lane; i < pnnz; i += 32) dst[i] = src[i];
+        __syncwarp();
+    };
+    auto flush_all = [&]() {       // oldest first
+#pragma unroll
+        for (int i = 0; i < kDefer; ++i) {
+            if (q_on[i]) flush_one(q_t[i], q_n[i], q_o[i]);
+            q_on[i] = false;
+        }
+        wide_pending = false;
+    };
+    auto push = [&](uint32_t pt, uint32_t pnnz, uint32_t off) {   // the oldest entry has been flushed: shift, append
+#pragma unroll
+        for (int i = 0; i + 1 < kDefer; ++i) {
+            q_t[i] = q_t[i + 1]; q_n[i] = q_n[i + 1]; q_o[i] = q_o[i + 1]; q_on[i] = q_on[i + 1];
+        }
+        q_t[kDefer - 1] = pt; q_n[kDefer - 1] = pnnz; q_o[kDefer - 1] = off; q_on[kDefer - 1] = true;
     };
 
     uint32_t t_next = 0;  // next ticket (lane 0): requested right behind a tile's loads, it arrives while they do
-    if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
+    if (t < T && lane == 0) t_next = ticket_tile(tk, cC, cj);
     while (t < T) {
         // ---- the next tile starts moving HBM -> L2 now, as ONE bulk prefetch of its 16 KB / 8 KB: the 64 row
         // loads issued at the end of this iteration then hit L2 ----
         const uint32_t tn = __shfl_sync(kFull, t_next, 0);
+        held = tn;
         if (tn < Tfull && lane == 0) {
             const unsigned char *src = reinterpret_cast<const unsigned char *>(dense) + (size_t)tn * kTile * sizeof(Elem);
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(kTile * sizeof(Elem))) : "memory");
@@ -228,7 +391,7 @@ compress_kernel(const Batch<CompressJob> batch) {
         const uint32_t tile_nnz = __shfl_sync(kFull, incl, 31);
 
         // ---- Phase 2: publish this tile's count (the look-back itself is deferred, see above) ----
-        publish_count(status, tag, t, tile_nnz, lane);
+        if (lane == 0) st_status(status + t, tag, tile_nnz);
 
         // B: lane l holds words 2l, 2l+1 -> one 16-byte store per lane, 512 contiguous bytes per warp
         {
@@ -238,8 +401,12 @@ compress_kernel(const Batch<CompressJob> batch) {
             reinterpret_cast<ulonglong2 *>(B + (size_t)t * kSide)[lane] = w;
         }
 
-        // ---- Phase 3b of the PREVIOUS tile: its prefix has had a whole iteration to arrive --------
-        flush_pending();
+        // ---- Phase 3b of the tile kDefer iterations back: its prefix has had that long to arrive; a tile that does
+        // not fit a slot, or follows one, needs the whole stage ----
+        const bool wide = tile_nnz > kSlot;
+        if (wide || wide_pending) flush_all();
+        else if (q_on[0]) flush_one(q_t[0], q_n[0], q_o[0]);
+        Elem *const stg = stage + (wide ? 0u : (seq % (kDefer + 1)) * kSlot);
 
         // ---- Phase 3a: compact into the warp's stage (tile-local offsets; order: column, row) ---
         if (tile_nnz <= kRowSkipNnz) {
@@ -251,11 +418,11 @@ compress_kernel(const Batch<CompressJob> batch) {
             for (int r = 0; r < kSide; ++r) {
                 if (((r < 32 ? anylo : anyhi) >> (r & 31)) & 1u) {
                     if constexpr (DT == PICI_F32) {
-                        if (nz32(v[2 * r])) stage[pos0++] = v[2 * r];
-                        if (nz32(v[2 * r + 1])) stage[pos1++] = v[2 * r + 1];
+                        if (nz32(v[2 * r])) stg[pos0++] = v[2 * r];
+                        if (nz32(v[2 * r + 1])) stg[pos1++] = v[2 * r + 1];
                     } else {
-                        if (nz16lo(v[r])) stage[pos0++] = (uint16_t)v[r];
-                        if (nz16hi(v[r])) stage[pos1++] = (uint16_t)(v[r] >> 16);
+                        if (nz16lo(v[r])) stg[pos0++] = (uint16_t)v[r];
+                        if (nz16hi(v[r])) stg[pos1++] = (uint16_t)(v[r] >> 16);
                     }
                 }
             }
@@ -264,46 +431,46 @@ compress_kernel(const Batch<CompressJob> batch) {
 #pragma unroll
             for (int r = 0; r < kSide; ++r) {
                 if constexpr (DT == PICI_F32) {
-                    if (nz32(v[2 * r])) stage[pos++] = v[2 * r];
+                    if (nz32(v[2 * r])) stg[pos++] = v[2 * r];
                 } else {
-                    if (nz16lo(v[r])) stage[pos++] = (uint16_t)v[r];
+                    if (nz16lo(v[r])) stg[pos++] = (uint16_t)v[r];
                 }
             }
 #pragma unroll
             for (int r = 0; r < kSide; ++r) {
                 if constexpr (DT == PICI_F32) {
-                    if (nz32(v[2 * r + 1])) stage[pos++] = v[2 * r + 1];
+                    if (nz32(v[2 * r + 1])) stg[pos++] = v[2 * r + 1];
                 } else {
-                    if (nz16hi(v[r])) stage[pos++] = (uint16_t)(v[r] >> 16);
+                    if (nz16hi(v[r])) stg[pos++] = (uint16_t)(v[r] >> 16);
                 }
             }
         }
         __syncwarp();
-        pending = true;
-        pt = t;
-        pnnz = tile_nnz;
+        push(t, tile_nnz, (uint32_t)(stg - stage));
+        wide_pending = wide;
+        ++seq;
 
         if (tn < Tfull) {
             load_full(tn, v);
         } else if (tn < T) {  // the ragged tile is padded through the stage: flush first
-            flush_pending();
+            flush_all();
             load_ragged(tn, v);
         }
         t = tn;
-        if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
+        if (t < T && lane == 0) t_next = ticket_tile(tk, cC, cj);
     }
-    flush_pending();
+    held = 0xFFFFFFFFu;
+    flush_all();
     // ---- the last warp of the launch to leave resets the ticket and advances the epoch ------------------------
     uint32_t last = 0;
     if (lane == 0) {
         __threadfence();
-        last = atomicAdd(ticket + 1, 1u) + 1u == gridDim.x * (uint32_t)kCompressWarps;
+        last = atomicAdd(ticket + 1, 1u) + 1u == worker_ctas * (uint32_t)kCompressWarps;
     }
     if (__shfl_sync(kFull, last, 0)) {
-        if (lane == 0) {
-            ticket[0] = 0;
-            ticket[1] = 0;
-        }
+        ticket_reset(ws, T, lane);
+        if (lane == 0) ticket[1] = 0;
+        for (uint32_t q = lane; q < ((T + (1u << sb_log) - 1u) >> sb_log); q += 32) blk_acc[q] = 0;   // the service's done words
         finish_epoch(ws, tag, status, T, lane);
     }
 }
@@ -325,7 +492,7 @@ int num_sms() {
 // Scratch for the scans (layout: pici_common.cuh): header, reduce_ss's accumulators, one word per tile.
 uint64_t scan_workspace_bytes(uint64_t n) {
     const uint64_t T = (n + kTile - 1) / kTile;
-    return (uint64_t)kWsHeaderBytes + ((uint64_t)kWsAccWords + ((T + 65) & ~1ull)) * 8;   // multiple of 16
+    return ticket_area_offset(T) + kTicketAreaBytes;   // header, accumulators, per-tile words, ticket counters (multiple of 16)
 }
 
 template <int DT>
@@ -345,8 +512,8 @@ static cudaError_t launch_compress_t(const CompressJob *jobs, int count, cudaStr
         batch.job[j] = jobs[j];
         T = max(T, (jobs[j].n + kTile - 1) / kTile);
     }
-    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
-    const uint64_t cap = max((uint64_t)num_sms() * Cfg::kMinBlocks / count, (uint64_t)1);   // persistent: one resident wave
+    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps + 1;   // + the scan service (CTA 0 of every job)
+    const uint64_t cap = max((uint64_t)num_sms() * Cfg::kMinBlocks / count, (uint64_t)2);   // persistent: one resident wave
     if (blocks > cap) blocks = cap;
     compress_kernel<DT, false><<<dim3((unsigned)blocks, (unsigned)count), kCompressWarps * 32, smem, s>>>(batch);
     return cudaGetLastError();
@@ -364,7 +531,7 @@ cudaError_t launch_prune_compress(const CompressJob &job, cudaStream_t s) {
     Batch<CompressJob> batch;
     batch.job[0] = job;
     const uint64_t T = (job.n + kTile - 1) / kTile;
-    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps;
+    uint64_t blocks = (T + kCompressWarps - 1) / kCompressWarps + 1;   // + the scan service
     const uint64_t cap = (uint64_t)num_sms() * 2;
     if (blocks > cap) blocks = cap;
     compress_kernel<PICI_F32, true><<<dim3((unsigned)blocks, 1u), kCompressWarps * 32, smem, s>>>(batch);

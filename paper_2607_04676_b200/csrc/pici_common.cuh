@@ -152,8 +152,16 @@ __device__ __forceinline__ void publish_count(uint64_t *status, uint32_t tag, ui
 
 // Step 2 (warp-collective): exclusive prefix of tile t = sum of the counts of tiles 0..t-1; publishes
 // the tile's inclusive prefix and writes I[t] (and I[T] from the last tile).
+// `first` / `have_first`: the status words of the first window (lane l <-> tile t-1-l), loaded by the caller well
+// ahead (lookback_peek) so that their L2 round trip is off the warp's critical path; a window that is not complete
+// yet is simply loaded again.
+__device__ __forceinline__ uint64_t lookback_peek(const uint64_t *status, uint32_t tag, uint32_t t, int lane) {
+    const int64_t idx = (int64_t)t - 1 - lane;
+    return idx >= 0 ? ld_status(status + idx) : ((uint64_t)(tag | kTagPrefix) << 32);
+}
 __device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t tag, uint32_t t, uint32_t count, uint32_t T,
-                                                    uint32_t *__restrict__ I, int lane) {
+                                                    uint32_t *__restrict__ I, int lane, uint64_t first = 0,
+                                                    bool have_first = false) {
     uint32_t excl = 0;
     int64_t pos = t;  // tiles [0, pos) are not yet accounted for
     while (pos > 0) {  // warp-uniform
@@ -162,7 +170,8 @@ __device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t t
         unsigned pm, em;
         unsigned ns = 8;
         for (;;) {
-            s = idx >= 0 ? ld_status(status + idx) : ((uint64_t)(tag | kTagPrefix) << 32);
+            if (have_first) s = first;
+            else s = idx >= 0 ? ld_status(status + idx) : ((uint64_t)(tag | kTagPrefix) << 32);
             const uint32_t hi = (uint32_t)(s >> 32);
             const bool valid = (hi & ~kTagPrefix) == tag;
             pm = __ballot_sync(kFull, valid && (hi & kTagPrefix) != 0u);
@@ -172,10 +181,14 @@ __device__ __forceinline__ uint32_t lookback_prefix(uint64_t *status, uint32_t t
             if ((em & rel) == 0u) {
                 const uint32_t v = ((1u << lane) & rel) ? (uint32_t)s : 0u;
                 excl += warp_sum(v);
+                have_first = false;
                 break;
             }
-            __nanosleep(ns);
-            if (ns < 64) ns += ns;
+            if (!have_first) {
+                __nanosleep(ns);
+                if (ns < 64) ns += ns;
+            }
+            have_first = false;
         }
         if (pm) break;
         pos -= 32;
@@ -264,6 +277,33 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
 }
 // Orders earlier generic-proxy accesses to shared memory before later async-proxy (TMA) ones.
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// ---- tile tickets from SEVERAL counters ------------------------------------------------------------------------------
+// One ticket per tile from ONE counter is what bounded every tile-per-warp kernel of this library: ~1800 resident warps
+// each keep one atomic on the same address in flight, the L2 serves them at ~3 ns apiece under load, so a ticket takes
+// ~5 us to return and 65 536 of them take 0.2 ms - exactly compress's run time at every sparsity from 95 % up.  (A bare
+// kernel that only reads 1 GiB tile by tile: 5.2 TB/s with one counter, 7.2 TB/s with four or more.)  So there are
+// kTicketCounters counters, 128 bytes apart, behind the per-tile words of the workspace (zero between launches: the
+// launch's last warp clears them again); warp w draws from counter w mod kTicketCounters,
+// and ticket k of counter j is tile C * k + j (C = kTicketCounters, or the number of warps of the launch if that is smaller:
+// every counter needs a warp).  Each counter's tiles increase, the counters advance at
+// about the same pace, and the smallest unclaimed tile always belongs to a group whose warps only wait for claimed
+// tiles - forward progress is as with one counter.
+constexpr uint32_t kTicketCounters = 8;
+constexpr uint32_t kTicketAreaBytes = kTicketCounters * 128u;
+__host__ __device__ __forceinline__ uint64_t ticket_area_offset(uint64_t T) {   // bytes from the start of the workspace
+    return (uint64_t)kWsHeaderBytes + ((uint64_t)kWsAccWords + ((T + 65) & ~1ull)) * 8;
+}
+__device__ __forceinline__ uint32_t *ticket_counter(void *ws, uint32_t T, uint32_t j) {
+    return reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + ticket_area_offset(T)) + 32u * j;
+}
+__device__ __forceinline__ uint32_t ticket_counters(uint32_t warps_in_launch) { return min(kTicketCounters, warps_in_launch); }
+__device__ __forceinline__ uint32_t ticket_tile(uint32_t *counter, uint32_t C, uint32_t j) {   // one lane
+    return atomicAdd(counter, 1u) * C + j;
+}
+__device__ __forceinline__ void ticket_reset(void *ws, uint32_t T, int lane) {     // the launch's last warp
+    if ((uint32_t)lane < kTicketCounters) *ticket_counter(ws, T, (uint32_t)lane) = 0u;
+}
 
 // Dynamic tile ticket (one atomic per tile, issued by lane 0 and broadcast).
 __device__ __forceinline__ uint32_t next_ticket(uint32_t *ticket, int lane) {
