@@ -90,7 +90,7 @@ __device__ __forceinline__ void scan_service(ScanShared &sh, uint64_t *blk_done,
 #pragma unroll
             for (int i = 0; i < 32; ++i) ok = ok && tagged(w[i], tag);
             if (__all_sync(kFull, ok)) break;
-            __nanosleep(500);
+            __nanosleep(100);    // 100 / 500 / 2000 ns: fp32 0.266 / 0.272 / 0.312 ms at 50 % sparsity, no difference above
         }
 #pragma unroll
         for (int i = 0; i < 32; ++i) cnt[i] = (uint32_t)w[i];
