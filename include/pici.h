@@ -92,9 +92,9 @@ int pici_sizes(uint64_t n, int dtype, uint64_t *bitvec_words, uint64_t *index_en
 int pici_workspace_init(void *ws, uint64_t ws_bytes, void *stream);
 
 /* a1-a3. Compress (Algorithm 1): dense[n] -> (B, I, A) in ONE pass over `dense`:
- * mask words + tile counts (Phase 1), device-wide exclusive scan of tile counts by decoupled
- * look-back (Phase 2; the paper scans block-locally per segment, PAPER.md:124 - here I is one global
- * prefix, reading C9 #3), compaction staged through shared memory (Phase 3).
+ * mask words + tile counts (Phase 1), a device-wide exclusive scan of the tile counts taken by a scan service inside
+ * the same launch over the counts the compressing warps publish (Phase 2; the paper scans block-locally per segment,
+ * here I is one global prefix, reading C9 #3), compaction staged through shared memory (Phase 3).
  * Reads dense; writes all 64*T words of B, all T+1 entries of I and A[0 .. nnz).  ws is scratch. */
 int pici_compress(const void *dense, uint64_t n, int dtype, uint64_t *B, uint32_t *I, void *A,
                   uint64_t A_capacity, void *ws, uint64_t ws_bytes, void *stream);

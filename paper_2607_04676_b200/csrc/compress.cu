@@ -8,9 +8,10 @@
 //     256-byte (fp32, 64-bit per lane) or 128-byte (bf16, 32-bit per lane) request, all 64 row loads
 //     of the tile are in flight at once, and the tile is read from HBM exactly ONCE: its values stay
 //     in registers between Phase 1 and Phase 3;
-//   * Phase 2 is a device-wide single-pass decoupled look-back over per-tile status words (the paper
-//     scans block-locally per NCCLX segment); tiles are handed out by a dynamic ticket
-//     and a tile's look-back is deferred behind the next tile's loads;
+//   * Phase 2, the device-wide exclusive scan of the tile counts (the paper scans block-locally per NCCLX segment,
+//     PAPER.md:124), is a SERVICE: the compressing warps only publish their counts; CTA 0 scans them block by block
+//     and writes I ("Phase 2 as a service" below); tiles are handed out by dynamic tickets from several counters,
+//     and a tile's flush is deferred behind the next two tiles;
 //   * Phase 3 compacts into a per-warp shared-memory stage (lane l's values are one contiguous run),
 //     which is then written to A with coalesced stores.
 #include <cuda_bf16.h>
@@ -27,7 +28,7 @@ constexpr int kCompressWarps = 4;
 #ifndef PICI_COMPRESS_DEFER
 #define PICI_COMPRESS_DEFER 2
 #endif
-constexpr int kDefer = PICI_COMPRESS_DEFER;   // iterations a tile's look-back and flush lag behind its publish
+constexpr int kDefer = PICI_COMPRESS_DEFER;   // iterations a tile's flush lags behind its publish
 constexpr uint32_t kRowSkipNnz = 256;   // tiles with at most this many values skip empty rows in Phase 3
 
 template <int DT>
@@ -264,14 +265,11 @@ compress_kernel(const Batch<CompressJob> batch) {
     if (t < Tfull) load_full(t, v);
     else if (t < T) load_ragged(t, v);
 
-    // Per-warp software pipeline.  A tile's count is published as soon as its data has arrived and Phase 1 is done; its
-    // look-back (and the flush of its compacted values) is deferred until kDefer later tiles of this warp have published
-    // theirs.  The look-back waits for the counts of the 32 tiles below, and those tiles are HELD by other warps - a
-    // warp claims its next tile a whole iteration before it can publish it - so a look-back taken one iteration late
-    // still found unpublished tiles and spun: with the publish and the look-back compiled out the kernel ran at 1.03
-    // (fp32) / 0.98 (bf16) of the HBM peak instead of 0.79 / 0.57.  Deferring by kDefer = 2 iterations gives the tiles
-    // below one more iteration to appear.  The stage is cut into kDefer + 1 slots for that; a tile with more values
-    // than a slot holds (denser than ~67 % sparsity) takes the whole stage and everything pending is flushed first.
+    // Per-warp software pipeline.  A tile's count is published as soon as its data has arrived and Phase 1 is done; the
+    // flush of its compacted values (which needs its prefix from the scan service) is deferred until kDefer later tiles
+    // of this warp have published theirs, by which time the service has normally passed the tile's block.  The stage is
+    // cut into kDefer + 1 slots for that; a tile with more values than a slot holds (denser than ~67 % sparsity) takes
+    // the whole stage and everything pending is flushed first.
     constexpr uint32_t kSlot = kTile / (kDefer + 1);
     uint32_t q_t[kDefer], q_n[kDefer], q_o[kDefer];   // pending tiles, oldest first: tile, count, stage offset
     bool q_on[kDefer];
@@ -390,7 +388,7 @@ compress_kernel(const Batch<CompressJob> batch) {
         const uint32_t incl = warp_incl_scan(cnt0 + cnt1, lane);
         const uint32_t tile_nnz = __shfl_sync(kFull, incl, 31);
 
-        // ---- Phase 2: publish this tile's count (the look-back itself is deferred, see above) ----
+        // ---- Phase 2: publish this tile's count for the scan service ----
         if (lane == 0) st_status(status + t, tag, tile_nnz);
 
         // B: lane l holds words 2l, 2l+1 -> one 16-byte store per lane, 512 contiguous bytes per warp
