@@ -48,83 +48,7 @@ struct CompressCfg<PICI_BF16> {
     static constexpr uint32_t kScanBlockLog = 9;
 };
 
-// ---- Phase 2 as a service ---------------------------------------------------------------------------------------------
-// The device-wide exclusive scan of the tile counts is not taken by the warps that compress (a decoupled look-back
-// cost them 3.5 - 4.7 dependent L2 round trips per tile: the whole gap between 0.79 and 1.03 of the HBM peak) but by
-// the four warps of CTA 0: warp w takes the 1024-tile blocks b = w, w + 4, ...; it waits until the block's counts are
-// all published (tickets hand tiles out in order, so that is when the front of the launch has passed it), scans them
-// (32 coalesced 256-byte rows of status words, a warp scan per row), receives the block's base from the warp that
-// scanned block b - 1 through shared memory, writes I for the block - I itself is the result - and marks the block
-// done (a word tagged with the launch epoch).  A compressing warp flushes a tile two iterations after publishing
-// its count; by then the block is normally done and the flush costs one load of the done word and one of I[t].
-struct ScanShared {
-    volatile uint32_t seq;    // blocks whose base has been handed on
-    volatile uint32_t base;   // exclusive prefix of block `seq`
-};
-// log2 of the scan block: 256 tiles (fp32) / 512 (bf16) for a full-size launch - measured at N = 2^28, 99 %: blocks of
-// 256 / 512 / 1024 tiles give fp32 0.169 / 0.169 / 0.177 ms and bf16 0.180 / 0.137 / 0.156 (small blocks: the service's
-// four warps, one L2 round trip per poll, fall behind bf16's tile rate; large blocks: a tile waits longer for the rest
-// of its block, and at 50 % sparsity, where a tile is flushed one iteration after its publish, 512 / 1024 stall:
-// fp32 0.270 / 0.519 / 0.628) - smaller when the launch has few warps, so that the tiles one warp takes one after the
-// other (about `warps` apart) fall into different blocks (see flush_one)
-__device__ __forceinline__ uint32_t scan_block_log(uint32_t worker_warps, uint32_t max_log) {
-    const uint32_t half = max(worker_warps / 2u, 32u);
-    return min(31u - (uint32_t)__clz(half), max_log);
-}
-__device__ __forceinline__ void scan_service(ScanShared &sh, uint64_t *blk_done, const uint64_t *status, uint32_t tag,
-                                             uint32_t T, uint32_t sb_log, uint32_t *__restrict__ I, int warp, int lane) {
-    const uint32_t sb = 1u << sb_log, rows = sb >> 5;
-    const uint32_t nblk = (T + sb - 1u) >> sb_log;
-    for (uint32_t b = (uint32_t)warp; b < nblk; b += kCompressWarps) {
-        const uint32_t t0 = b << sb_log;
-        uint32_t cnt[32];
-        uint64_t w[32];
-        // all rows are requested together (one L2 round trip for the block) and the whole block is read again until
-        // every word carries the tag
-        for (;;) {
-            bool ok = true;
-#pragma unroll
-            for (int i = 0; i < 32; ++i) {      // row i: tiles t0 + 32 i + lane
-                const uint32_t t = t0 + 32u * i + (uint32_t)lane;
-                w[i] = ((uint32_t)i < rows && t < T) ? ld_status(status + t) : ((uint64_t)tag << 32);   // others count 0
-            }
-#pragma unroll
-            for (int i = 0; i < 32; ++i) ok = ok && tagged(w[i], tag);
-            if (__all_sync(kFull, ok)) break;
-            __nanosleep(100);    // 100 / 500 / 2000 ns: fp32 0.266 / 0.272 / 0.312 ms at 50 % sparsity, no difference above
-        }
-#pragma unroll
-        for (int i = 0; i < 32; ++i) cnt[i] = (uint32_t)w[i];
-        uint32_t run = 0;                   // block-local exclusive prefixes, in place
-#pragma unroll
-        for (int i = 0; i < 32; ++i) {
-            if ((uint32_t)i < rows) {       // warp-uniform
-                const uint32_t incl = warp_incl_scan(cnt[i], lane);
-                const uint32_t tot = __shfl_sync(kFull, incl, 31);
-                cnt[i] = run + incl - cnt[i];
-                run += tot;
-            }
-        }
-        uint32_t base = 0;
-        if (lane == 0) {
-            while (sh.seq != b) __nanosleep(32);
-            base = sh.base;
-            sh.base = base + run;           // hand the next block its base before the stores below
-            __threadfence_block();
-            sh.seq = b + 1u;
-        }
-        base = __shfl_sync(kFull, base, 0);
-#pragma unroll
-        for (int i = 0; i < 32; ++i) {
-            const uint32_t t = t0 + 32u * i + (uint32_t)lane;
-            if ((uint32_t)i < rows && t < T) I[t] = base + cnt[i];
-        }
-        if (b + 1u == nblk && lane == 0) I[T] = base + run;
-        __threadfence();
-        __syncwarp();
-        if (lane == 0) st_status(blk_done + b, tag, base + run);   // done; the value is the prefix at the block's end
-    }
-}
+// (Phase 2 as a service: scan_service / service_prefix, pici_common.cuh)
 
 // PRUNE (fp32 only): the tile that is compressed is not read but MADE while it is loaded - sampled top-k pruning with
 // leaky error feedback fused into the same pass (include/pici_prune.h): acc = g + leak * e (two
@@ -165,7 +89,8 @@ compress_kernel(const Batch<CompressJob> batch) {
             scan_sh.base = 0;
         }
         __syncthreads();
-        scan_service(scan_sh, blk_acc, status, tag, T, scan_block_log(worker_ctas * (uint32_t)kCompressWarps, Cfg::kScanBlockLog), I, warp, lane);
+        scan_service(scan_sh, blk_acc, status, tag, T, scan_block_log(worker_ctas * (uint32_t)kCompressWarps, Cfg::kScanBlockLog), I, nullptr, warp,
+                     kCompressWarps, lane);
         return;
     }
     const uint32_t cC = ticket_counters(worker_ctas * (uint32_t)kCompressWarps);
@@ -279,44 +204,8 @@ compress_kernel(const Batch<CompressJob> batch) {
     uint32_t seq = 0;
     const uint32_t sb_log = scan_block_log(worker_ctas * (uint32_t)kCompressWarps, Cfg::kScanBlockLog);
     uint32_t held = 0xFFFFFFFFu;   // the tile this warp has claimed but not yet published (>= T: none)
-    auto wait_done = [&](uint32_t b) -> uint32_t {   // prefix at the end of scan block b, once the service has it
-        const uint64_t *done = blk_acc + b;
-        unsigned ns = 16;
-        uint64_t v;
-        while (!tagged(v = ld_status(done), tag)) {
-            __nanosleep(ns);
-            if (ns < 128) ns += ns;
-        }
-        return (uint32_t)v;
-    };
     auto flush_one = [&](uint32_t pt, uint32_t pnnz, uint32_t off) {
-        // The scan service finishes a block only when EVERY tile of it has published its count - also the tile this
-        // warp holds unpublished.  So the warp waits for the service only if that tile lies in a later block (blocks
-        // then resolve in increasing order: no cycle); otherwise - small launches, the tail of a launch - it takes the
-        // prefix itself: the end of the block below plus the counts of the tiles of its own block below pt (all of
-        // them lower than anything this warp holds).
-        const uint32_t bq = pt >> sb_log;
-        uint32_t excl;
-        if (held >= T || bq < (held >> sb_log)) {
-            wait_done(bq);
-            asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(excl) : "l"(I + pt) : "memory");
-        } else {
-            excl = bq ? wait_done(bq - 1u) : 0u;
-            uint32_t part = 0;
-            for (uint32_t u0 = bq << sb_log; u0 < pt; u0 += 32u) {
-                const uint32_t u = u0 + (uint32_t)lane;
-                uint64_t v = (uint64_t)tag << 32;
-                if (u < pt) {
-                    unsigned ns = 16;
-                    while (!tagged(v = ld_status(status + u), tag)) {
-                        __nanosleep(ns);
-                        if (ns < 128) ns += ns;
-                    }
-                }
-                part += (uint32_t)v;
-            }
-            excl += warp_sum(part);
-        }
+        const uint32_t excl = service_prefix(blk_acc, status, I, tag, sb_log, pt, held, T, lane);
         Elem *dst = Aout + excl;
         const Elem *src = stage + off;
         for (uint32_t i = lane; i < pnnz; i += 32) dst[i] = src[i];

@@ -27,7 +27,8 @@
 namespace pici {
 
 constexpr int kCooWarps = 4;
-constexpr uint32_t kCooStage = 1024;                 // entries a stage buffer holds before a block goes direct
+constexpr uint32_t kCooStage = 640;                  // entries a stage buffer holds before a block goes direct
+constexpr int kCooBufs = 3;                          // stage buffers per warp: the block in hand + two whose flush is deferred
 constexpr uint32_t kCooStageWords = kCooStage + 128; // + one row of slack (the check is per row)
 
 struct CooWs {            // views into the caller's workspace (layout: coo_workspace_bytes)
@@ -86,13 +87,30 @@ struct CooCompressArgs {
 __global__ void __launch_bounds__(kCooWarps * 32, 3) coo_compress_kernel(const CooCompressArgs a) {
     extern __shared__ __align__(16) uint32_t coo_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // per warp: two buffers of (idx[kCooStageWords], val[kCooStageWords])
-    uint32_t *const stage = coo_smem + (size_t)warp * 4 * kCooStageWords;
+    // per warp: kCooBufs buffers of (idx[kCooStageWords], val[kCooStageWords])
+    uint32_t *const stage = coo_smem + (size_t)warp * kCooBufs * 2 * kCooStageWords;
     uint32_t *const ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(a.ws.hdr) + kWsCompressTicket);
     const uint32_t tag = launch_tag(a.ws.hdr);
     const uint64_t n = a.n;
     const uint32_t T = (uint32_t)((n + kTile - 1) / kTile), Tfull = (uint32_t)(n / kTile);
     const uint32_t lt = (1u << lane) - 1u;
+    // Phase 2 is a service, as in pici_compress (pici_common.cuh): CTA 0 scans the published counts block by block and
+    // writes the exclusive prefixes into ws.excl (and the total into *d_nnz); the other CTAs compress
+    const uint32_t worker_ctas = gridDim.x - 1u;
+    const uint32_t sb_log = scan_block_log(worker_ctas * (uint32_t)kCooWarps, 8u);
+    if (blockIdx.x == 0) {
+        __shared__ ScanShared scan_sh;
+        if (threadIdx.x == 0) {
+            scan_sh.seq = 0;
+            scan_sh.base = 0;
+        }
+        __syncthreads();
+        scan_service(scan_sh, a.ws.blk_acc, a.ws.status, tag, T, sb_log, a.ws.excl, a.d_nnz, warp, kCooWarps, lane);
+        return;
+    }
+    const uint32_t cC = ticket_counters(worker_ctas * (uint32_t)kCooWarps);
+    const uint32_t cj = ((blockIdx.x - 1u) * (uint32_t)kCooWarps + (uint32_t)warp) % cC;
+    uint32_t *const tk = ticket_counter(a.ws.hdr, T, cj);
 
     uint4 v[32];
     auto load_block = [&](uint32_t tt) {
@@ -145,31 +163,37 @@ __global__ void __launch_bounds__(kCooWarps * 32, 3) coo_compress_kernel(const C
         return base;
     };
 
-    bool pending = false;
-    uint32_t pt = 0, pcnt = 0, pbuf = 0, cur = 0;
-    auto finish_block = [&](uint32_t tt, uint32_t cnt) -> uint32_t {   // look-back; the last block writes nnz
-        const uint32_t excl = lookback_prefix(a.ws.status, tag, tt, cnt, T, a.ws.excl, lane);
-        if (tt + 1u == T && lane == 0) *a.d_nnz = excl + cnt;
-        return excl;
+    // two deferred blocks (oldest first) + the block in hand: three stage buffers
+    uint32_t q_t[2], q_n[2], q_b[2];
+    bool q_on[2] = {false, false};
+    uint32_t cur = 0;
+    uint32_t held = 0xFFFFFFFFu;   // the block this warp has claimed but not yet published (>= T: none)
+    auto flush_one = [&](uint32_t pt, uint32_t pcnt, uint32_t pbuf) {
+        const uint32_t excl = service_prefix(a.ws.blk_acc, a.ws.status, a.ws.excl, tag, sb_log, pt, held, T, lane);
+        const uint32_t *si = stage + (size_t)pbuf * 2 * kCooStageWords, *sv = si + kCooStageWords;
+        for (uint32_t i = lane; i < pcnt; i += 32) {
+            a.idx[excl + i] = si[i];
+            a.val[excl + i] = sv[i];
+        }
+        __syncwarp();
     };
-    auto flush_pending = [&]() {
-        if (pending) {
-            const uint32_t excl = finish_block(pt, pcnt);
-            const uint32_t *si = stage + (size_t)pbuf * 2 * kCooStageWords, *sv = si + kCooStageWords;
-            for (uint32_t i = lane; i < pcnt; i += 32) {
-                a.idx[excl + i] = si[i];
-                a.val[excl + i] = sv[i];
-            }
-            pending = false;
+    auto flush_all = [&]() {
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            if (q_on[i]) flush_one(q_t[i], q_n[i], q_b[i]);
+            q_on[i] = false;
         }
     };
 
-    uint32_t t = next_ticket(ticket, lane);
+    uint32_t t = 0;
+    if (lane == 0) t = ticket_tile(tk, cC, cj);
+    t = __shfl_sync(kFull, t, 0);
     if (t < T) load_block(t);
     uint32_t t_next = 0;
-    if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
+    if (t < T && lane == 0) t_next = ticket_tile(tk, cC, cj);
     while (t < T) {
         const uint32_t tn = __shfl_sync(kFull, t_next, 0);
+        held = tn;
         if (tn < Tfull && lane == 0) {   // the next block starts moving HBM -> L2 now (one bulk prefetch)
             const unsigned char *src = reinterpret_cast<const unsigned char *>(a.dense) + (size_t)tn * kTile * 4;
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(kTile * 4)) : "memory");
@@ -177,22 +201,35 @@ __global__ void __launch_bounds__(kCooWarps * 32, 3) coo_compress_kernel(const C
         uint32_t *si = stage + (size_t)cur * 2 * kCooStageWords;
         const uint32_t cnt = compact(t, si, si + kCooStageWords, true);
         __syncwarp();
-        publish_count(a.ws.status, tag, t, cnt, lane);
-        flush_pending();                        // the previous block: its prefix has had an iteration to arrive
+        if (lane == 0) st_status(a.ws.status + t, tag, cnt);      // for the scan service
+        if (q_on[0]) flush_one(q_t[0], q_n[0], q_b[0]);           // the block two iterations back
+        q_t[0] = q_t[1]; q_n[0] = q_n[1]; q_b[0] = q_b[1]; q_on[0] = q_on[1];
         if (stored_all) {
-            pending = true;
-            pt = t; pcnt = cnt; pbuf = cur;
-            cur ^= 1u;
-        } else {                                // dense block: look-back now, write from the registers
-            const uint32_t excl = finish_block(t, cnt);
+            q_t[1] = t; q_n[1] = cnt; q_b[1] = cur; q_on[1] = true;
+            cur = cur == (uint32_t)kCooBufs - 1u ? 0u : cur + 1u;
+        } else {                                // dense block: its prefix now, write from the registers
+            q_on[1] = false;
+            const uint32_t excl = service_prefix(a.ws.blk_acc, a.ws.status, a.ws.excl, tag, sb_log, t, held, T, lane);
             compact(t, a.idx + excl, a.val + excl, false);
         }
         if (tn < T) load_block(tn);
         t = tn;
-        if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
+        if (t < T && lane == 0) t_next = ticket_tile(tk, cC, cj);
     }
-    flush_pending();
-    coo_leave(a.ws.hdr, ticket, tag, a.ws.status, T, gridDim.x * (uint32_t)kCooWarps, lane);
+    held = 0xFFFFFFFFu;
+    flush_all();
+    // ---- the launch's last warp clears the service's done words and the tickets and advances the epoch ----
+    uint32_t last = 0;
+    if (lane == 0) {
+        __threadfence();
+        last = atomicAdd(ticket + 1, 1u) + 1u == worker_ctas * (uint32_t)kCooWarps;
+    }
+    if (__shfl_sync(kFull, last, 0)) {
+        for (uint32_t q = lane; q < ((T + (1u << sb_log) - 1u) >> sb_log); q += 32) a.ws.blk_acc[q] = 0;
+        ticket_reset(a.ws.hdr, T, lane);
+        if (lane == 0) ticket[1] = 0;
+        finish_epoch(a.ws.hdr, tag, a.ws.status, T, lane);
+    }
 }
 
 // ============================================ block offsets (pre-pass) ============================================
@@ -419,12 +456,16 @@ static cudaError_t launch_coo_compress(const void *dense, uint64_t n, uint32_t *
                                        cudaStream_t s) {
     if (n == 0) return launch_set_u32(d_nnz, 0u, Gate{nullptr, 0, 0}, s);
     static std::atomic<bool> done[64];
-    const size_t smem = (size_t)kCooWarps * 4 * kCooStageWords * sizeof(uint32_t);
+    const size_t smem = (size_t)kCooWarps * kCooBufs * 2 * kCooStageWords * sizeof(uint32_t);
     cudaError_t e = allow_smem(coo_compress_kernel, smem, done);
     if (e != cudaSuccess) return e;
     const CooCompressArgs a = {reinterpret_cast<const uint32_t *>(dense), n, idx, reinterpret_cast<uint32_t *>(val), d_nnz,
                                coo_ws(ws, n)};
-    coo_compress_kernel<<<persistent_grid((n + kTile - 1) / kTile), kCooWarps * 32, smem, s>>>(a);
+    // + CTA 0, the scan service; all CTAs resident (one wave)
+    const uint64_t T = (n + kTile - 1) / kTile;
+    uint64_t blocks = (T + kCooWarps - 1) / kCooWarps + 1;
+    if (blocks > (uint64_t)num_sms() * 3) blocks = (uint64_t)num_sms() * 3;
+    coo_compress_kernel<<<(unsigned)blocks, kCooWarps * 32, smem, s>>>(a);
     return cudaGetLastError();
 }
 
