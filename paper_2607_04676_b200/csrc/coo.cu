@@ -59,23 +59,6 @@ static CooWs coo_ws(void *ws, uint64_t n) {
     return w;
 }
 
-// The launch's last warp resets the ticket pair and advances the epoch (as pici_compress does).
-__device__ __forceinline__ void coo_leave(void *ws, uint32_t *ticket, uint32_t tag, uint64_t *status, uint32_t T,
-                                          uint32_t warps, int lane) {
-    uint32_t last = 0;
-    if (lane == 0) {
-        __threadfence();
-        last = atomicAdd(ticket + 1, 1u) + 1u == warps;
-    }
-    if (__shfl_sync(kFull, last, 0)) {
-        if (lane == 0) {
-            ticket[0] = 0;
-            ticket[1] = 0;
-        }
-        finish_epoch(ws, tag, status, T, lane);
-    }
-}
-
 // ================================================ compress ================================================
 struct CooCompressArgs {
     const uint32_t *dense;
@@ -334,6 +317,22 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
     const uint32_t tag = launch_tag(a.ws.hdr);
     const uint32_t T = (uint32_t)((a.n + kTile - 1) / kTile);
     const uint32_t *__restrict__ ix = a.ix, *__restrict__ iy = a.iy, *__restrict__ vx = a.vx, *__restrict__ vy = a.vy;
+    // the device-wide scan of the survivor counts is a service (CTA 0; pici_common.cuh), as in the compress kernels
+    const uint32_t worker_ctas = gridDim.x - 1u;
+    const uint32_t sb_log = scan_block_log(worker_ctas * (uint32_t)kMergeWarps, 9u);
+    if (blockIdx.x == 0) {
+        __shared__ ScanShared scan_sh;
+        if (threadIdx.x == 0) {
+            scan_sh.seq = 0;
+            scan_sh.base = 0;
+        }
+        __syncthreads();
+        scan_service(scan_sh, a.ws.blk_acc, a.ws.status, tag, T, sb_log, a.ws.excl, a.d_no, warp, kMergeWarps, lane);
+        return;
+    }
+    const uint32_t cC = ticket_counters(worker_ctas * (uint32_t)kMergeWarps);
+    const uint32_t cj = ((blockIdx.x - 1u) * (uint32_t)kMergeWarps + (uint32_t)warp) % cC;
+    uint32_t *const tk = ticket_counter(a.ws.hdr, T, cj);
 
     // lane 0 .. 3 hold offx[t], offx[t + 1], offy[t], offy[t + 1] of the block in hand / the next block
     auto load_off = [&](uint32_t tt) -> uint32_t {
@@ -372,27 +371,27 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
         }
         return cnt;
     };
-    bool pending = false;
-    Blk P;                                                    // the block whose emission is deferred
-    auto flush_pending = [&]() {
-        if (pending) {
-            const uint32_t excl = lookback_prefix(a.ws.status, tag, P.t, P.total, T, a.ws.excl, lane);
-            if (P.t + 1u == T && lane == 0) *a.d_no = excl + P.total;
-            if (P.total) walk(P, true, excl + P.before);
-            pending = false;
-        }
+    Blk P0, P1;                                              // blocks whose emission is deferred, oldest first
+    bool on0 = false, on1 = false;
+    uint32_t held = 0xFFFFFFFFu;                              // claimed, not yet published (>= T: none)
+    auto emit = [&](const Blk &P) {
+        const uint32_t excl = service_prefix(a.ws.blk_acc, a.ws.status, a.ws.excl, tag, sb_log, P.t, held, T, lane);
+        if (P.total) walk(P, true, excl + P.before);
     };
 
-    uint32_t t = next_ticket(ticket, lane);
+    uint32_t t = 0;
+    if (lane == 0) t = ticket_tile(tk, cC, cj);
+    t = __shfl_sync(kFull, t, 0);
     uint32_t off = load_off(t);
     uint32_t t_next = 0;
-    if (t < T && lane == 0) t_next = atomicAdd(ticket, 1u);
+    if (t < T && lane == 0) t_next = ticket_tile(tk, cC, cj);
     while (t < T) {
         const uint32_t x0 = __shfl_sync(kFull, off, 0), x1 = __shfl_sync(kFull, off, 1), y0 = __shfl_sync(kFull, off, 2),
                        y1 = __shfl_sync(kFull, off, 3);
         const uint32_t tn = __shfl_sync(kFull, t_next, 0);
+        held = tn;
         off = load_off(tn);                                   // arrives while this block is merged
-        if (tn < T && lane == 0) t_next = atomicAdd(ticket, 1u);
+        if (tn < T && lane == 0) t_next = ticket_tile(tk, cC, cj);
         Blk C;
 #pragma unroll
         for (int q = 0; q < 4; ++q) C.wx[q] = C.wy[q] = 0u;
@@ -425,14 +424,27 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
         const uint32_t incl = warp_incl_scan(C.cnt, lane);
         C.before = incl - C.cnt;
         C.total = __shfl_sync(kFull, incl, 31);
-        publish_count(a.ws.status, tag, t, C.total, lane);
-        flush_pending();                                      // the previous block: its prefix has had a block's time
-        P = C;
-        pending = true;
+        if (lane == 0) st_status(a.ws.status + t, tag, C.total);   // for the scan service
+        if (on0) emit(P0);                                    // the block two iterations back
+        P0 = P1; on0 = on1;
+        P1 = C; on1 = true;
         t = tn;
     }
-    flush_pending();
-    coo_leave(a.ws.hdr, ticket, tag, a.ws.status, T, gridDim.x * (uint32_t)kMergeWarps, lane);
+    held = 0xFFFFFFFFu;
+    if (on0) emit(P0);
+    if (on1) emit(P1);
+    // ---- the launch's last warp clears the service's done words and the tickets and advances the epoch ----
+    uint32_t last = 0;
+    if (lane == 0) {
+        __threadfence();
+        last = atomicAdd(ticket + 1, 1u) + 1u == worker_ctas * (uint32_t)kMergeWarps;
+    }
+    if (__shfl_sync(kFull, last, 0)) {
+        for (uint32_t q = lane; q < ((T + (1u << sb_log) - 1u) >> sb_log); q += 32) a.ws.blk_acc[q] = 0;
+        ticket_reset(a.ws.hdr, T, lane);
+        if (lane == 0) ticket[1] = 0;
+        finish_epoch(a.ws.hdr, tag, a.ws.status, T, lane);
+    }
 }
 
 // ================================================= launchers =================================================
@@ -512,7 +524,7 @@ static cudaError_t launch_coo_merge(const uint32_t *ix, const void *vx, const ui
     const CooMergeArgs a = {ix, reinterpret_cast<const uint32_t *>(vx), iy, reinterpret_cast<const uint32_t *>(vy), io,
                             reinterpret_cast<uint32_t *>(vo), d_no, n, w};
     const uint64_t T = (n + kTile - 1) / kTile;
-    uint64_t blocks = (T + kMergeWarps - 1) / kMergeWarps;
+    uint64_t blocks = (T + kMergeWarps - 1) / kMergeWarps + 1;   // + CTA 0, the scan service
     const uint64_t cap = (uint64_t)num_sms() * 4;
     if (blocks > cap) blocks = cap;
     coo_merge_kernel<<<(unsigned)blocks, kMergeWarps * 32, 0, s>>>(a);
