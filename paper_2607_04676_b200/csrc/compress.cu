@@ -39,13 +39,17 @@ struct CompressCfg<PICI_F32> {
     static constexpr int kRegs = 128;       // 64 rows x 2 columns
     static constexpr int kMinBlocks = 3;    // 12 warps / SM, <= 168 registers
     static constexpr uint32_t kScanBlockLog = 8;
+    static constexpr uint32_t kStageElems = kTile;          // 16 KB per warp
 };
 template <>
 struct CompressCfg<PICI_BF16> {
     using Elem = uint16_t;
     static constexpr int kRegs = 64;        // 64 rows x (2 packed columns)
-    static constexpr int kMinBlocks = 5;
+    // 3 CTAs / SM (with 5 the scan service fell behind: 0.141 ms at 99 %; 4: 0.128; 3: 0.122; 2: 0.168) and the same 16 KB
+    // of stage per warp as fp32: three slots of 2730 values, so a tile at 50 % sparsity still fits a slot
+    static constexpr int kMinBlocks = 3;
     static constexpr uint32_t kScanBlockLog = 9;
+    static constexpr uint32_t kStageElems = 2 * kTile;
 };
 
 // (Phase 2 as a service: scan_service / service_prefix, pici_common.cuh)
@@ -96,7 +100,7 @@ compress_kernel(const Batch<CompressJob> batch) {
     const uint32_t cC = ticket_counters(worker_ctas * (uint32_t)kCompressWarps);
     const uint32_t cj = ((blockIdx.x - 1u) * (uint32_t)kCompressWarps + (uint32_t)warp) % cC;
     uint32_t *const tk = ticket_counter(ws, T, cj);
-    Elem *stage = reinterpret_cast<Elem *>(smem_raw) + warp * kTile;
+    Elem *stage = reinterpret_cast<Elem *>(smem_raw) + warp * Cfg::kStageElems;
     const uint32_t Tfull = (uint32_t)(n / kTile);
     Elem *Aout = reinterpret_cast<Elem *>(A);
 
@@ -195,7 +199,7 @@ compress_kernel(const Batch<CompressJob> batch) {
     // of this warp have published theirs, by which time the service has normally passed the tile's block.  The stage is
     // cut into kDefer + 1 slots for that; a tile with more values than a slot holds (denser than ~67 % sparsity) takes
     // the whole stage and everything pending is flushed first.
-    constexpr uint32_t kSlot = kTile / (kDefer + 1);
+    constexpr uint32_t kSlot = Cfg::kStageElems / (kDefer + 1);
     uint32_t q_t[kDefer], q_n[kDefer], q_o[kDefer];   // pending tiles, oldest first: tile, count, stage offset
     bool q_on[kDefer];
 #pragma unroll
@@ -385,7 +389,7 @@ uint64_t scan_workspace_bytes(uint64_t n) {
 template <int DT>
 static cudaError_t launch_compress_t(const CompressJob *jobs, int count, cudaStream_t s) {
     using Cfg = CompressCfg<DT>;
-    const size_t smem = (size_t)kCompressWarps * kTile * sizeof(typename Cfg::Elem);
+    const size_t smem = (size_t)kCompressWarps * Cfg::kStageElems * sizeof(typename Cfg::Elem);
     static std::atomic<bool> configured_on[64];   // one-time setup per device; doing it twice is harmless
     std::atomic<bool> &configured = configured_on[current_device_slot()];
     if (!configured.load(std::memory_order_acquire)) {
