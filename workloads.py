@@ -176,3 +176,24 @@ def edge_sizes() -> tuple[int, ...]:
 
 
 assert math.isclose(config4().expected_density(1), 0.10, rel_tol=1e-12)
+
+
+def scattered_buffer(n: int, k: int, seed: int, dense_tiles: tuple[int, ...] = (), tile: int = 4096,
+                     device="cuda") -> torch.Tensor:
+    """fp32 buffer for the maximum-size cases (n up to 2^32 - 1, where a Bernoulli mask would cost 4 more
+    buffers of n): zeros, k values N(0, 1) scattered at uniformly drawn positions (collisions overwrite), the first
+    and last element and the elements around every 2^30 boundary set, and the listed tiles filled completely."""
+    g = _gen(seed + 11_000_027, device)
+    out = torch.zeros(n, dtype=torch.float32, device=device)
+    step = 1 << 24
+    for lo in range(0, k, step):
+        c = min(step, k - lo)
+        idx = torch.randint(0, n, (c,), generator=g, device=device, dtype=torch.int64)
+        out[idx] = torch.randn(c, generator=g, device=device, dtype=torch.float32)
+    edges = [0, n - 1] + [b + d for b in range(1 << 30, n, 1 << 30) for d in (-1, 0, 1) if 0 <= b + d < n]
+    out[torch.tensor(edges, device=device)] = 1.5
+    for t in dense_tiles:
+        lo, hi = t * tile, min(n, (t + 1) * tile)
+        if lo < n:
+            out[lo:hi] = torch.randn(hi - lo, generator=g, device=device, dtype=torch.float32) + 4.0   # no zeros
+    return out
