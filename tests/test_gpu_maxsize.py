@@ -124,3 +124,27 @@ def test_coo_at_max_n(mods):
     ck.reduce_sd(cx, acc)
     x += 1.0
     assert torch.equal(acc.view(torch.int32), x.view(torch.int32))
+
+
+def test_pici_bf16_at_max_n(mods):
+    pk, _ = mods
+    x = wl.scattered_buffer(N, 30_000_000, seed=4, dense_tiles=DENSE_TILES).to(torch.bfloat16)
+    ws = pk.alloc_workspace(N)
+    px = pk.alloc_pici(N, pk.BF16)
+    pk.compress(x, px, ws)
+    nx = int(torch.count_nonzero(x))
+    assert px.nnz_host() == nx
+    I = px.I[:T + 1].cpu().numpy().view(np.uint32).astype(np.int64)
+    assert I[0] == 0 and I[T] == nx and np.all(np.diff(I) >= 0) and np.all(np.diff(I) <= TILE)
+    for t in _sample_tiles(6):
+        bits = x[t * TILE:min(N, (t + 1) * TILE)].cpu().view(torch.int16).numpy().view(np.uint16)
+        want = po.compress(bits, "bf16")
+        assert np.array_equal(px.B[64 * t:64 * (t + 1)].cpu().numpy().view(np.uint64), want.B), f"tile {t}: bitvector"
+        A = px.A[int(I[t]):int(I[t + 1])].cpu().view(torch.int16).numpy().view(np.uint16)
+        assert np.array_equal(A, want.A), f"tile {t}: values"
+    out = torch.full_like(x, float("nan"))
+    pk.decompress(px, out)
+    assert torch.equal(out.view(torch.int16), x.view(torch.int16))
+    y = torch.ones_like(x)
+    pk.reduce_sd(px, y)
+    assert torch.equal(y.view(torch.int16), (x + 1.0).view(torch.int16))
