@@ -99,8 +99,9 @@ compress_kernel(const Batch<CompressJob> batch) {
             scan_sh.base = 0;
         }
         __syncthreads();
-        scan_service(scan_sh, blk_acc, status, tag, T, scan_block_log(worker_ctas * (uint32_t)kCompressWarps, Cfg::kScanBlockLog), I, nullptr, warp,
-                     kCompressWarps, lane);
+        const uint32_t sbl = scan_block_log(worker_ctas * (uint32_t)kCompressWarps, Cfg::kScanBlockLog);
+        scan_service(scan_sh, blk_acc, status, tag, T, sbl, I, nullptr, warp, kCompressWarps, lane);
+        launch_exit(ws, ticket + 1, blk_acc, status, tag, T, sbl, gridDim.x * (uint32_t)kCompressWarps, lane);
         return;
     }
     const uint32_t cC = ticket_counters(worker_ctas * (uint32_t)kCompressWarps);
@@ -358,18 +359,7 @@ compress_kernel(const Batch<CompressJob> batch) {
     }
     held = 0xFFFFFFFFu;
     flush_all();
-    // ---- the last warp of the launch to leave resets the ticket and advances the epoch ------------------------
-    uint32_t last = 0;
-    if (lane == 0) {
-        __threadfence();
-        last = atomicAdd(ticket + 1, 1u) + 1u == worker_ctas * (uint32_t)kCompressWarps;
-    }
-    if (__shfl_sync(kFull, last, 0)) {
-        ticket_reset(ws, T, lane);
-        if (lane == 0) ticket[1] = 0;
-        for (uint32_t q = lane; q < ((T + (1u << sb_log) - 1u) >> sb_log); q += 32) blk_acc[q] = 0;   // the service's done words
-        finish_epoch(ws, tag, status, T, lane);
-    }
+    launch_exit(ws, ticket + 1, blk_acc, status, tag, T, sb_log, gridDim.x * (uint32_t)kCompressWarps, lane);
 }
 
 int num_sms() {
@@ -389,7 +379,7 @@ int num_sms() {
 // Scratch for the scans (layout: pici_common.cuh): header, reduce_ss's accumulators, one word per tile.
 uint64_t scan_workspace_bytes(uint64_t n) {
     const uint64_t T = (n + kTile - 1) / kTile;
-    return ticket_area_offset(T) + kTicketAreaBytes;   // header, accumulators, per-tile words, ticket counters (multiple of 16)
+    return tile_words_end(T);   // header (with the ticket counters), accumulators, per-tile words (multiple of 16)
 }
 
 template <int DT>

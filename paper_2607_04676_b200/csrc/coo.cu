@@ -89,6 +89,7 @@ __global__ void __launch_bounds__(kCooWarps * 32, 3) coo_compress_kernel(const C
         }
         __syncthreads();
         scan_service(scan_sh, a.ws.blk_acc, a.ws.status, tag, T, sb_log, a.ws.excl, a.d_nnz, warp, kCooWarps, lane);
+        launch_exit(a.ws.hdr, ticket + 1, a.ws.blk_acc, a.ws.status, tag, T, sb_log, gridDim.x * (uint32_t)kCooWarps, lane);
         return;
     }
     const uint32_t cC = ticket_counters(worker_ctas * (uint32_t)kCooWarps);
@@ -201,18 +202,7 @@ __global__ void __launch_bounds__(kCooWarps * 32, 3) coo_compress_kernel(const C
     }
     held = 0xFFFFFFFFu;
     flush_all();
-    // ---- the launch's last warp clears the service's done words and the tickets and advances the epoch ----
-    uint32_t last = 0;
-    if (lane == 0) {
-        __threadfence();
-        last = atomicAdd(ticket + 1, 1u) + 1u == worker_ctas * (uint32_t)kCooWarps;
-    }
-    if (__shfl_sync(kFull, last, 0)) {
-        for (uint32_t q = lane; q < ((T + (1u << sb_log) - 1u) >> sb_log); q += 32) a.ws.blk_acc[q] = 0;
-        ticket_reset(a.ws.hdr, T, lane);
-        if (lane == 0) ticket[1] = 0;
-        finish_epoch(a.ws.hdr, tag, a.ws.status, T, lane);
-    }
+    launch_exit(a.ws.hdr, ticket + 1, a.ws.blk_acc, a.ws.status, tag, T, sb_log, gridDim.x * (uint32_t)kCooWarps, lane);
 }
 
 // ============================================ block offsets (pre-pass) ============================================
@@ -328,6 +318,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
         }
         __syncthreads();
         scan_service(scan_sh, a.ws.blk_acc, a.ws.status, tag, T, sb_log, a.ws.excl, a.d_no, warp, kMergeWarps, lane);
+        launch_exit(a.ws.hdr, ticket + 1, a.ws.blk_acc, a.ws.status, tag, T, sb_log, gridDim.x * (uint32_t)kMergeWarps, lane);
         return;
     }
     const uint32_t cC = ticket_counters(worker_ctas * (uint32_t)kMergeWarps);
@@ -433,18 +424,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
     held = 0xFFFFFFFFu;
     if (on0) emit(P0);
     if (on1) emit(P1);
-    // ---- the launch's last warp clears the service's done words and the tickets and advances the epoch ----
-    uint32_t last = 0;
-    if (lane == 0) {
-        __threadfence();
-        last = atomicAdd(ticket + 1, 1u) + 1u == worker_ctas * (uint32_t)kMergeWarps;
-    }
-    if (__shfl_sync(kFull, last, 0)) {
-        for (uint32_t q = lane; q < ((T + (1u << sb_log) - 1u) >> sb_log); q += 32) a.ws.blk_acc[q] = 0;
-        ticket_reset(a.ws.hdr, T, lane);
-        if (lane == 0) ticket[1] = 0;
-        finish_epoch(a.ws.hdr, tag, a.ws.status, T, lane);
-    }
+    launch_exit(a.ws.hdr, ticket + 1, a.ws.blk_acc, a.ws.status, tag, T, sb_log, gridDim.x * (uint32_t)kMergeWarps, lane);
 }
 
 // ================================================= launchers =================================================

@@ -102,8 +102,12 @@ __device__ __forceinline__ bool gate_closed(const int32_t *gate, int32_t mask, i
 // is never cleared between launches: high 32 bits = 1 (bit 31) | kind (bit 30: 0 aggregate, 1 prefix) | epoch tag
 // (30 bits), low 32 bits = value.  A word of an earlier launch (or a zero word) never carries the current tag.
 constexpr uint32_t kTagValid = 0x80000000u, kTagPrefix = 0x40000000u, kTagMask = 0x3FFFFFFFu;
-constexpr int kWsHeaderBytes = 128;       // [0, 64): WsHeader; [64, 128): compress's ticket and exit counter
+// [0, 64): WsHeader; [64, 128): compress's exit counter; [128, 1152): the ticket counters (kTicketAreaBytes, below) - all
+// at FIXED offsets: a workspace is shared by calls with different n, and what must be zero between launches may not
+// lie where another call's per-tile words do
+constexpr int kWsHeaderBytes = 1152;
 constexpr int kWsCompressTicket = 64;
+constexpr int kWsTicketArea = 128;
 // Behind the header, at FIXED offsets (so that calls with different n can share a workspace): reduce_ss's
 // accumulators - one word per 1024 tiles and one per 32 tiles, sized for the largest n (2^20 tiles), zero between
 // launches - then one word per tile: compress's status words / reduce_ss's tagged tile counts.
@@ -418,7 +422,7 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // each keep one atomic on the same address in flight, the L2 serves them at ~3 ns apiece under load, so a ticket takes
 // ~5 us to return and 65 536 of them take 0.2 ms - exactly compress's run time at every sparsity from 95 % up.  (A bare
 // kernel that only reads 1 GiB tile by tile: 5.2 TB/s with one counter, 7.2 TB/s with four or more.)  So there are
-// kTicketCounters counters, 128 bytes apart, behind the per-tile words of the workspace (zero between launches: the
+// kTicketCounters counters, 128 bytes apart, in the tail of the workspace header (zero between launches: the
 // launch's last warp clears them again); warp w draws from counter w mod kTicketCounters,
 // and ticket k of counter j is tile C * k + j (C = kTicketCounters, or the number of warps of the launch if that is smaller:
 // every counter needs a warp).  Each counter's tiles increase, the counters advance at
@@ -426,11 +430,13 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // tiles - forward progress is as with one counter.
 constexpr uint32_t kTicketCounters = 8;
 constexpr uint32_t kTicketAreaBytes = kTicketCounters * 128u;
-__host__ __device__ __forceinline__ uint64_t ticket_area_offset(uint64_t T) {   // bytes from the start of the workspace
+static_assert(kWsTicketArea + (int)kTicketAreaBytes == kWsHeaderBytes, "ticket counters fill the header's tail");
+__host__ __device__ __forceinline__ uint64_t tile_words_end(uint64_t T) {   // bytes from the start of the workspace
     return (uint64_t)kWsHeaderBytes + ((uint64_t)kWsAccWords + ((T + 65) & ~1ull)) * 8;
 }
 __device__ __forceinline__ uint32_t *ticket_counter(void *ws, uint32_t T, uint32_t j) {
-    return reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + ticket_area_offset(T)) + 32u * j;
+    (void)T;
+    return reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + kWsTicketArea) + 32u * j;
 }
 __device__ __forceinline__ uint32_t ticket_counters(uint32_t warps_in_launch) { return min(kTicketCounters, warps_in_launch); }
 __device__ __forceinline__ uint32_t ticket_tile(uint32_t *counter, uint32_t C, uint32_t j) {   // one lane
@@ -438,6 +444,27 @@ __device__ __forceinline__ uint32_t ticket_tile(uint32_t *counter, uint32_t C, u
 }
 __device__ __forceinline__ void ticket_reset(void *ws, uint32_t T, int lane) {     // the launch's last warp
     if ((uint32_t)lane < kTicketCounters) *ticket_counter(ws, T, (uint32_t)lane) = 0u;
+}
+
+// Every warp of a tile-ticket launch - the compressing warps AND the warps of the scan service - leaves through here.
+// The last one clears what must be zero between launches (ticket counters, the exit counter, the service's done words:
+// that area is reduce_ss's accumulators) and advances the epoch.  The service's warps count too: a compressing warp
+// can take its last prefix from a tile word and leave before the service has stored that block's done word, and a
+// done word stored after the clear would stay behind.
+__device__ __forceinline__ void launch_exit(void *ws, uint32_t *exit_counter, uint64_t *blk_done, uint64_t *status, uint32_t tag,
+                                            uint32_t T, uint32_t sb_log, uint32_t warps_in_launch, int lane) {
+    uint32_t last = 0;
+    if (lane == 0) {
+        __threadfence();
+        last = atomicAdd(exit_counter, 1u) + 1u == warps_in_launch;
+    }
+    if (__shfl_sync(kFull, last, 0)) {
+        __threadfence();
+        ticket_reset(ws, T, lane);
+        if (lane == 0) *exit_counter = 0;
+        for (uint32_t q = lane; q < ((T + (1u << sb_log) - 1u) >> sb_log); q += 32) blk_done[q] = 0;
+        finish_epoch(ws, tag, status, T, lane);
+    }
 }
 
 // Dynamic tile ticket (one atomic per tile, issued by lane 0 and broadcast).

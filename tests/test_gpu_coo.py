@@ -136,3 +136,54 @@ def test_full_size_properties_and_samples(ck, sparsity):
     acc = y.clone()
     ck.reduce_sd(cx, acc)
     assert torch.equal(acc.view(torch.int32), s.view(torch.int32))    # x + y == y + x bit for bit (no NaN here)
+
+
+def test_mixed_calls_of_many_sizes_share_one_workspace(ck):
+    """One workspace, 90 calls of random size and density back to back, no synchronisation: Pici compress (fp32 and
+    bf16), Pici reduce_ss, COO compress, COO reduce_ss.  What one call leaves behind (tagged words, the service's done
+    words, ticket and exit counters, the epoch) must never be mistaken by the next, whatever its n."""
+    from oracle import pici_oracle as po
+    from paper_2607_04676_b200 import pici as pk
+    rng = np.random.default_rng(77)
+    nmax = (1 << 22) + 4097
+    ws = ck.alloc_workspace(nmax)
+    checks = []
+    for j in range(90):
+        op = j % 5
+        n = int(rng.integers(1, nmax)) if j % 4 else int(rng.integers(1, 24 * 4096))
+        dx, dy = (float(rng.choice([0.0, 0.001, 0.01, 0.08, 0.3, 0.6, 1.0])) for _ in range(2))
+        x = wl.sparse_buffer(n, dx, seed=500 + 2 * j)
+        if op in (0, 1):                                        # Pici compress
+            dtype = "f32" if op == 0 else "bf16"
+            if op == 1:
+                x = wl.sparse_buffer(n, dx, seed=500 + 2 * j, dtype="bf16")
+            out = pk.alloc_pici(n, pk.F32 if op == 0 else pk.BF16)
+            pk.compress(x.cuda(), out, ws)
+            bits = _bits(x) if op == 0 else x.view(torch.int16).numpy().view(np.uint16)
+            checks.append(("pici", out, po.compress(bits, dtype)))
+        elif op == 2:                                           # Pici reduce_ss
+            y = wl.sparse_buffer(n, dy, seed=501 + 2 * j)
+            ox, oy = po.compress(_bits(x), "f32"), po.compress(_bits(y), "f32")
+            dxp, dyp, out = pk.alloc_pici(n, pk.F32), pk.alloc_pici(n, pk.F32), pk.alloc_pici(n, pk.F32)
+            pk.compress(x.cuda(), dxp, ws)
+            pk.compress(y.cuda(), dyp, ws)
+            pk.reduce_ss(dxp, dyp, out, ws)
+            checks.append(("pici", out, po.reduce_ss(ox, oy)))
+        elif op == 3:                                           # COO compress
+            out = ck.alloc_coo(n)
+            ck.compress(x.cuda(), out, ws)
+            checks.append(("coo", out, co.compress(_bits(x))))
+        else:                                                   # COO reduce_ss
+            y = wl.sparse_buffer(n, dy, seed=501 + 2 * j)
+            cx, cy, out = ck.alloc_coo(n), ck.alloc_coo(n), ck.alloc_coo(n)
+            ck.compress(x.cuda(), cx, ws)
+            ck.compress(y.cuda(), cy, ws)
+            ck.reduce_ss(cx, cy, out, ws)
+            checks.append(("coo", out, co.reduce_ss(co.compress(_bits(x)), co.compress(_bits(y)))))
+    for kind, got, want in checks:
+        if kind == "coo":
+            _assert_equal(got, want)
+        else:
+            B, I, A = got.to_host()
+            Tn = po.num_tiles(want.n)
+            assert np.array_equal(I[:Tn + 1], want.I) and np.array_equal(B[:64 * Tn], want.B) and np.array_equal(A, want.A)

@@ -344,3 +344,27 @@ def test_bf16_reduce_sd_full_size(pk):
     acc = y.clone()
     pk.reduce_sd(px, acc)
     assert torch.equal(acc.view(torch.int16), (x + y).view(torch.int16))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_compress_random_sizes_share_one_workspace(pk, dtype):
+    """The scan service under many launch shapes: 120 random (n, density) pairs - sizes from one tile to 2^23 + tail,
+    densities from empty to full, including mixed tiles - compressed back to back through ONE workspace (the launch
+    epoch is all that separates them) and compared with the oracle bit for bit."""
+    rng = np.random.default_rng(2024 if dtype == "f32" else 2025)
+    nmax = (1 << 23) + 4097
+    ws = pk.alloc_workspace(nmax)
+    dt = pk.F32 if dtype == "f32" else pk.BF16
+    cases = []
+    for j in range(120):
+        n = int(rng.integers(1, nmax)) if j % 3 else int(rng.integers(1, 40 * 4096))
+        dens = float(rng.choice([0.0, 0.0005, 0.01, 0.05, 0.12, 0.3, 0.5, 0.7, 1.0]))
+        host = wl.sparse_buffer(n, dens, seed=9000 + j, dtype=dtype)
+        if j % 5 == 0 and n > 3 * 4096:      # a dense stretch inside a sparse buffer: wide tiles among narrow ones
+            lo = int(rng.integers(0, n - 2 * 4096))
+            host[lo:lo + 2 * 4096 + 17] = 1.0
+        out = pk.alloc_pici(n, dt)
+        pk.compress(host.cuda(), out, ws)     # no synchronisation between the launches
+        cases.append((host, out))
+    for host, out in cases:
+        _assert_pici_equal(pk, out, po.compress(_bits(host), dtype))
