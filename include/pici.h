@@ -26,8 +26,10 @@
  *     no global state; it is re-entrant.  `ws` is scratch that must not be shared by calls that may
  *     run concurrently (one workspace per stream).  A workspace must be cleared ONCE after it is
  *     allocated (pici_workspace_init, or any memset to 0); after that any sequence of calls on one
- *     stream may reuse it without clearing: its first 64 bytes hold a launch epoch that the kernels
- *     advance themselves, and every scan word is tagged with it, so no call starts with a memset.
+ *     stream - of any n the workspace is large enough for, compress, reduce_ss, the COO and prune calls
+ *     mixed - may reuse it without clearing: its first 64 bytes hold a launch epoch that the kernels
+ *     advance themselves, every scan word is tagged with it, and everything that must be zero between
+ *     launches lies at offsets that do not depend on n, so no call starts with a memset.
  *   - Alignment: dense, B, A, ws pointers 16-byte aligned; I 4-byte aligned.  Violations return
  *     PICI_ERR_ALIGN.
  *   - Sizes: B holds 64*T words and I holds T+1 entries even when n % 4096 != 0; A (and Ao) must

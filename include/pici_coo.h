@@ -17,7 +17,8 @@
  * in which one index is needed per nonzero value").  dense, idx, val, ws 16-byte aligned, d_nnz 4-byte.
  * 0 <= n < 2^32.  fp32 only (the paper's space calculations assume 32-bit values).  `ws` is scratch of
  * pici_coo_sizes().workspace_bytes bytes, cleared ONCE after allocation (pici_workspace_init) and then reusable by
- * any sequence of calls on one stream (same launch-epoch scheme as pici.h); one workspace per stream.
+ * any sequence of calls on one stream, of any n it is large enough for, mixed with the calls of pici.h (same
+ * launch-epoch scheme); one workspace per stream.
  * A COO object handed to decompress / reduce_sd / reduce_ss must have ascending, distinct indices < n (what
  * pici_coo_compress and pici_coo_reduce_ss produce); anything else is undefined behaviour on the device.
  */
@@ -34,7 +35,8 @@ extern "C" {
 int pici_coo_sizes(uint64_t n, uint64_t *capacity, uint64_t *workspace_bytes);
 
 /* dense[n] -> (idx, val, *d_nnz) in ONE pass over `dense`: nonzero test, device-wide single-pass exclusive scan of
- * per-4096-element counts (decoupled look-back), compaction staged through shared memory. */
+ * per-4096-element counts (a scan service inside the launch, as in pici_compress), compaction staged through shared
+ * memory. */
 int pici_coo_compress(const void *dense, uint64_t n, uint32_t *idx, void *val, uint64_t capacity,
                       uint32_t *d_nnz, void *ws, uint64_t ws_bytes, void *stream);
 

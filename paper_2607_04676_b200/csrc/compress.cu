@@ -379,6 +379,9 @@ int num_sms() {
 // Scratch for the scans (layout: pici_common.cuh): header, reduce_ss's accumulators, one word per tile.
 uint64_t scan_workspace_bytes(uint64_t n) {
     const uint64_t T = (n + kTile - 1) / kTile;
+#if PICI_TICKET_OLD
+    return tile_words_end(T) + 1024;
+#endif
     return tile_words_end(T);   // header (with the ticket counters), accumulators, per-tile words (multiple of 16)
 }
 

@@ -44,7 +44,9 @@ uint64_t coo_workspace_bytes(uint64_t n) {
     const uint64_t T = (n + kTile - 1) / kTile;
     return scan_workspace_bytes(n) + 3 * round16((T + 1) * 4);
 }
-static CooWs coo_ws(void *ws, uint64_t n) {
+// The three scratch arrays lie at the END of the caller's buffer, not behind this call's tile words: a workspace is
+// shared by calls with different n, and scratch data must not land where a larger call keeps tagged words.
+static CooWs coo_ws(void *ws, uint64_t ws_bytes, uint64_t n) {
     const uint64_t T = (n + kTile - 1) / kTile;
     unsigned char *b = reinterpret_cast<unsigned char *>(ws);
     CooWs w;
@@ -52,7 +54,7 @@ static CooWs coo_ws(void *ws, uint64_t n) {
     w.blk_acc = reinterpret_cast<uint64_t *>(b + kWsHeaderBytes);
     w.grp_acc = w.blk_acc + kWsBlkWords;
     w.status = w.blk_acc + kWsAccWords;
-    unsigned char *tail = b + scan_workspace_bytes(n);
+    unsigned char *tail = b + ((ws_bytes & ~15ull) - 3 * round16((T + 1) * 4));
     w.excl = reinterpret_cast<uint32_t *>(tail);
     w.offx = reinterpret_cast<uint32_t *>(tail + round16((T + 1) * 4));
     w.offy = reinterpret_cast<uint32_t *>(tail + 2 * round16((T + 1) * 4));
@@ -445,14 +447,14 @@ static unsigned persistent_grid(uint64_t T, uint64_t waves = 1) {   // waves > 1
 }
 
 static cudaError_t launch_coo_compress(const void *dense, uint64_t n, uint32_t *idx, void *val, uint32_t *d_nnz, void *ws,
-                                       cudaStream_t s) {
+                                       uint64_t ws_bytes, cudaStream_t s) {
     if (n == 0) return launch_set_u32(d_nnz, 0u, Gate{nullptr, 0, 0}, s);
     static std::atomic<bool> done[64];
     const size_t smem = (size_t)kCooWarps * kCooBufs * 2 * kCooStageWords * sizeof(uint32_t);
     cudaError_t e = allow_smem(coo_compress_kernel, smem, done);
     if (e != cudaSuccess) return e;
     const CooCompressArgs a = {reinterpret_cast<const uint32_t *>(dense), n, idx, reinterpret_cast<uint32_t *>(val), d_nnz,
-                               coo_ws(ws, n)};
+                               coo_ws(ws, ws_bytes, n)};
     // + CTA 0, the scan service; all CTAs resident (one wave)
     const uint64_t T = (n + kTile - 1) / kTile;
     uint64_t blocks = (T + kCooWarps - 1) / kCooWarps + 1;
@@ -472,13 +474,13 @@ static cudaError_t launch_coo_offsets(const uint32_t *ix, const uint32_t *d_nx, 
 }
 
 static cudaError_t launch_coo_decompress(const uint32_t *idx, const void *val, const uint32_t *d_nnz, uint64_t n, void *dense,
-                                         void *ws, cudaStream_t s) {
+                                         void *ws, uint64_t ws_bytes, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
     static std::atomic<bool> done[64];
     const size_t smem = (size_t)kCooWarps * kTile * sizeof(uint32_t);
     cudaError_t e = allow_smem(coo_decompress_kernel, smem, done);
     if (e != cudaSuccess) return e;
-    const CooWs w = coo_ws(ws, n);
+    const CooWs w = coo_ws(ws, ws_bytes, n);
     e = launch_coo_offsets(idx, d_nnz, w.offx, nullptr, nullptr, nullptr, n, s);
     if (e != cudaSuccess) return e;
     const CooExpandArgs a = {idx, reinterpret_cast<const uint32_t *>(val), w.offx, reinterpret_cast<uint32_t *>(dense), n};
@@ -496,9 +498,9 @@ static cudaError_t launch_coo_reduce_sd(const uint32_t *idx, const void *val, co
 
 static cudaError_t launch_coo_merge(const uint32_t *ix, const void *vx, const uint32_t *d_nx, const uint32_t *iy, const void *vy,
                                     const uint32_t *d_ny, uint64_t n, uint32_t *io, void *vo, uint32_t *d_no, void *ws,
-                                    cudaStream_t s) {
+                                    uint64_t ws_bytes, cudaStream_t s) {
     if (n == 0) return launch_set_u32(d_no, 0u, Gate{nullptr, 0, 0}, s);
-    const CooWs w = coo_ws(ws, n);
+    const CooWs w = coo_ws(ws, ws_bytes, n);
     cudaError_t e = launch_coo_offsets(ix, d_nx, w.offx, iy, d_ny, w.offy, n, s);
     if (e != cudaSuccess) return e;
     const CooMergeArgs a = {ix, reinterpret_cast<const uint32_t *>(vx), iy, reinterpret_cast<const uint32_t *>(vy), io,
@@ -549,7 +551,7 @@ int pici_coo_compress(const void *dense, uint64_t n, uint32_t *idx, void *val, u
     if (!al(dense, 16)) return PICI_ERR_ALIGN;
     if (capacity < n) return PICI_ERR_CAPACITY;
     if ((rc = check_ws(ws, ws_bytes, n)) != PICI_OK) return rc;
-    return rc_of(launch_coo_compress(dense, n, idx, val, d_nnz, ws, static_cast<cudaStream_t>(stream)));
+    return rc_of(launch_coo_compress(dense, n, idx, val, d_nnz, ws, ws_bytes, static_cast<cudaStream_t>(stream)));
 }
 
 int pici_coo_decompress(const uint32_t *idx, const void *val, const uint32_t *d_nnz, uint64_t n, void *dense_out,
@@ -559,7 +561,7 @@ int pici_coo_decompress(const uint32_t *idx, const void *val, const uint32_t *d_
     if (n != 0 && dense_out == nullptr) return PICI_ERR_INVALID_ARG;
     if (!al(dense_out, 16)) return PICI_ERR_ALIGN;
     if ((rc = check_ws(ws, ws_bytes, n)) != PICI_OK) return rc;
-    return rc_of(launch_coo_decompress(idx, val, d_nnz, n, dense_out, ws, static_cast<cudaStream_t>(stream)));
+    return rc_of(launch_coo_decompress(idx, val, d_nnz, n, dense_out, ws, ws_bytes, static_cast<cudaStream_t>(stream)));
 }
 
 int pici_coo_reduce_sd(const uint32_t *idx, const void *val, const uint32_t *d_nnz, uint64_t n, void *dense_inout,
@@ -581,7 +583,7 @@ int pici_coo_reduce_ss(const uint32_t *ix, const void *vx, const uint32_t *d_nx,
     if (capacity < n) return PICI_ERR_CAPACITY;
     if ((rc = check_ws(ws, ws_bytes, n)) != PICI_OK) return rc;
     if (n != 0 && (io == ix || io == iy || vo == vx || vo == vy || d_no == d_nx || d_no == d_ny)) return PICI_ERR_INVALID_ARG;
-    return rc_of(launch_coo_merge(ix, vx, d_nx, iy, vy, d_ny, n, io, vo, d_no, ws, static_cast<cudaStream_t>(stream)));
+    return rc_of(launch_coo_merge(ix, vx, d_nx, iy, vy, d_ny, n, io, vo, d_no, ws, ws_bytes, static_cast<cudaStream_t>(stream)));
 }
 
 }  // extern "C"

@@ -105,7 +105,10 @@ constexpr uint32_t kTagValid = 0x80000000u, kTagPrefix = 0x40000000u, kTagMask =
 // [0, 64): WsHeader; [64, 128): compress's exit counter; [128, 1152): the ticket counters (kTicketAreaBytes, below) - all
 // at FIXED offsets: a workspace is shared by calls with different n, and what must be zero between launches may not
 // lie where another call's per-tile words do
-constexpr int kWsHeaderBytes = 1152;
+#ifndef PICI_TICKET_STRIDE
+#define PICI_TICKET_STRIDE 128
+#endif
+constexpr int kWsHeaderBytes = 128 + 8 * PICI_TICKET_STRIDE;
 constexpr int kWsCompressTicket = 64;
 constexpr int kWsTicketArea = 128;
 // Behind the header, at FIXED offsets (so that calls with different n can share a workspace): reduce_ss's
@@ -429,14 +432,18 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // about the same pace, and the smallest unclaimed tile always belongs to a group whose warps only wait for claimed
 // tiles - forward progress is as with one counter.
 constexpr uint32_t kTicketCounters = 8;
-constexpr uint32_t kTicketAreaBytes = kTicketCounters * 128u;
+constexpr uint32_t kTicketAreaBytes = kTicketCounters * (uint32_t)PICI_TICKET_STRIDE;
 static_assert(kWsTicketArea + (int)kTicketAreaBytes == kWsHeaderBytes, "ticket counters fill the header's tail");
 __host__ __device__ __forceinline__ uint64_t tile_words_end(uint64_t T) {   // bytes from the start of the workspace
     return (uint64_t)kWsHeaderBytes + ((uint64_t)kWsAccWords + ((T + 65) & ~1ull)) * 8;
 }
 __device__ __forceinline__ uint32_t *ticket_counter(void *ws, uint32_t T, uint32_t j) {
+#if PICI_TICKET_OLD
+    return reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + tile_words_end(T)) + 32u * j;
+#else
     (void)T;
-    return reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + kWsTicketArea) + 32u * j;
+    return reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(ws) + kWsTicketArea) + (uint32_t)(PICI_TICKET_STRIDE / 4) * j;
+#endif
 }
 __device__ __forceinline__ uint32_t ticket_counters(uint32_t warps_in_launch) { return min(kTicketCounters, warps_in_launch); }
 __device__ __forceinline__ uint32_t ticket_tile(uint32_t *counter, uint32_t C, uint32_t j) {   // one lane
@@ -451,7 +458,10 @@ __device__ __forceinline__ void ticket_reset(void *ws, uint32_t T, int lane) {  
 // that area is reduce_ss's accumulators) and advances the epoch.  The service's warps count too: a compressing warp
 // can take its last prefix from a tile word and leave before the service has stored that block's done word, and a
 // done word stored after the clear would stay behind.
-__device__ __forceinline__ void launch_exit(void *ws, uint32_t *exit_counter, uint64_t *blk_done, uint64_t *status, uint32_t tag,
+#ifndef PICI_EXIT_INLINE
+#define PICI_EXIT_INLINE __noinline__
+#endif
+static __device__ PICI_EXIT_INLINE void launch_exit(void *ws, uint32_t *exit_counter, uint64_t *blk_done, uint64_t *status, uint32_t tag,
                                             uint32_t T, uint32_t sb_log, uint32_t warps_in_launch, int lane) {
     uint32_t last = 0;
     if (lane == 0) {
