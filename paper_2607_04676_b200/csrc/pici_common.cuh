@@ -120,6 +120,7 @@ struct WsHeader {             // first bytes of the workspace; persistent across
     uint32_t epoch;           // tag of the last finished launch (compress and reduce_ss share it)
     uint32_t ticket;          // reduce_ss: next block
     uint32_t finished;        // reduce_ss: flusher warps that have left
+    uint32_t high_words;      // the most per-tile words any launch on this workspace has used (for the wrap, below)
 };
 // Tag of the launch that starts now (read by every thread at kernel entry; 1 .. kTagMask).
 __device__ __forceinline__ uint32_t launch_tag(const void *ws) {
@@ -127,15 +128,20 @@ __device__ __forceinline__ uint32_t launch_tag(const void *ws) {
     return kTagValid | ((e + 1u) & kTagMask);
 }
 // The launch's last warp: every tagged word of an earlier launch is stale from now on.  When the 30-bit tag is
-// about to wrap, the `words` tagged words are cleared first (once per 2^30 launches), by the calling warp.
+// about to wrap, the tagged words are cleared first (once per 2^30 launches), by the calling warp - all the words ANY
+// launch on this workspace has used (the header keeps the high-water mark: calls with different n share a
+// workspace, and a word a larger call tagged 2^30 launches ago must not meet its tag again).
 __device__ __forceinline__ void finish_epoch(void *ws, uint32_t tag, uint64_t *tagged, uint64_t words, int lane) {
+    WsHeader *h = reinterpret_cast<WsHeader *>(ws);
     uint32_t e = tag & kTagMask;
+    const uint32_t high = max(*reinterpret_cast<volatile uint32_t *>(&h->high_words), (uint32_t)words);
     if (e == kTagMask) {
-        for (uint64_t q = lane; q < words; q += 32) tagged[q] = 0;
+        for (uint64_t q = lane; q < high; q += 32) tagged[q] = 0;
         e = 0;
     }
     __syncwarp();
     if (lane == 0) {
+        *reinterpret_cast<volatile uint32_t *>(&h->high_words) = high;
         __threadfence();
         *reinterpret_cast<volatile uint32_t *>(ws) = e;
     }

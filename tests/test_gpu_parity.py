@@ -368,3 +368,36 @@ def test_compress_random_sizes_share_one_workspace(pk, dtype):
         cases.append((host, out))
     for host, out in cases:
         _assert_pici_equal(pk, out, po.compress(_bits(host), dtype))
+
+
+def test_launch_epoch_wraps(pk):
+    """The 30-bit launch epoch that tags every scan word wraps after 2^30 launches.  White box: the epoch word (the
+    first 4 bytes of the workspace) is set to three launches before the wrap; a large call, small calls across the
+    wrap and the large call again must all match the oracle - the wrap clears every word the workspace has ever
+    tagged, not only the current call's."""
+    n_big, n_small = (1 << 21) + 77, 5 * 4096 + 3
+    ws = pk.alloc_workspace(n_big)
+    ws[:4].view(torch.int32).fill_(0x3FFFFFFF - 3)
+    big = wl.sparse_buffer(n_big, 0.05, seed=41)
+    small = wl.sparse_buffer(n_small, 0.3, seed=42)
+    want_big, want_small = po.compress(_bits(big), "f32"), po.compress(_bits(small), "f32")
+    want_sum = po.reduce_ss(want_small, want_small)
+    dbig, dsmall = big.cuda(), small.cuda()
+    outs = []
+    for step in range(12):                      # the epoch passes 0x3FFFFFFF at the fourth launch
+        if step in (0, 7, 11):
+            o = pk.alloc_pici(n_big, pk.F32)
+            pk.compress(dbig, o, ws)
+            outs.append((o, want_big))
+        elif step % 2:
+            o = pk.alloc_pici(n_small, pk.F32)
+            pk.compress(dsmall, o, ws)
+            outs.append((o, want_small))
+        else:
+            o = pk.alloc_pici(n_small, pk.F32)
+            pk.reduce_ss(outs[-1][0], outs[-1][0], o, ws) if outs[-1][1] is want_small else pk.compress(dsmall, o, ws)
+            outs.append((o, want_sum if outs[-1][1] is want_small else want_small))
+    torch.cuda.synchronize()
+    assert int(ws[:4].view(torch.int32).item()) < 16, "the epoch has wrapped"
+    for o, want in outs:
+        _assert_pici_equal(pk, o, want)
