@@ -26,6 +26,26 @@ def _bits(t):
 @pytest.mark.parametrize("n,leak,keep", [(4096, 1.0, 0.01), (4097, 0.5, 0.05), (70_001, 0.9, 0.01), (1 << 20, 0.75, 0.01),
                                          ((1 << 22) + 333, 1.0, 0.001), (1 << 18, 0.0, 0.5)])
 def test_prune_compress_matches_oracle(mods, n, leak, keep):
+    _run_case(mods, n, leak, keep, None)
+
+
+def test_prune_calls_of_many_sizes_share_one_workspace(mods):
+    """The same cases through ONE workspace (sized for the largest), a plain compress of yet another size in between."""
+    pk, pn = mods
+    cases = [((1 << 22) + 333, 1.0, 0.001), (4097, 0.5, 0.05), (1 << 20, 0.75, 0.01), (70_001, 0.9, 0.01), (4096, 1.0, 0.01)]
+    ws = pn.alloc_workspace(cases[0][0], cases[0][0] // 1000)
+    for j, (n, leak, keep) in enumerate(cases):
+        _run_case(mods, n, leak, keep, ws)
+        nn = 3 * 4096 * (j + 1) + 5
+        x = wl.sparse_buffer(nn, 0.1, seed=60 + j)
+        o = pk.alloc_pici(nn, pk.F32)
+        pk.compress(x.cuda(), o, ws)
+        want = po.compress(_bits(x), "f32")
+        B, I, A = o.to_host()
+        assert np.array_equal(I[:want.I.size], want.I) and np.array_equal(B[:want.B.size], want.B) and np.array_equal(A, want.A)
+
+
+def _run_case(mods, n, leak, keep, ws):
     pk, pn = mods
     m = max(4, n // 1000)
     k = max(1, int(np.ceil(keep * m)))
@@ -33,7 +53,8 @@ def test_prune_compress_matches_oracle(mods, n, leak, keep):
     sample = sample_h.cuda()
     e_h = np.zeros(n, np.float32)
     e_d = torch.zeros(n, device="cuda")
-    ws = pn.alloc_workspace(n, m)
+    if ws is None:
+        ws = pn.alloc_workspace(n, m)
     d_tau = torch.zeros(1, device="cuda")
     out = pk.alloc_pici(n, pk.F32)
     for it in range(3):                                              # three iterations: the residual carries over
