@@ -401,3 +401,31 @@ def test_launch_epoch_wraps(pk):
     assert int(ws[:4].view(torch.int32).item()) < 16, "the epoch has wrapped"
     for o, want in outs:
         _assert_pici_equal(pk, o, want)
+
+
+def test_concurrent_streams_with_their_own_workspaces(pk):
+    """Three streams, each with its own workspace, launch compress / reduce_ss at the same time: every launch is sized
+    for a full resident wave, so the launches share the SMs and each runs partly resident - the kernels' waits (scan
+    service, tickets, flushers) must only ever be on work that is already running."""
+    n = (1 << 23) + 4097
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    xs = [wl.sparse_buffer(n, d, seed=70 + i) for i, d in enumerate((0.01, 0.1, 0.5))]
+    wants = [po.compress(_bits(x), "f32") for x in xs]
+    want_ss = [po.reduce_ss(w, w) for w in wants]
+    dev = [x.cuda() for x in xs]
+    ws = [pk.alloc_workspace(n) for _ in streams]
+    outs = [[] for _ in streams]
+    torch.cuda.synchronize()
+    for rep in range(6):
+        for i, st in enumerate(streams):
+            with torch.cuda.stream(st):
+                o = pk.alloc_pici(n, pk.F32)
+                pk.compress(dev[i], o, ws[i], stream=st)
+                s = pk.alloc_pici(n, pk.F32)
+                pk.reduce_ss(o, o, s, ws[i], stream=st)
+                outs[i].append((o, s))
+    torch.cuda.synchronize()
+    for i in range(3):
+        for o, s in outs[i][::2]:
+            _assert_pici_equal(pk, o, wants[i])
+            _assert_pici_equal(pk, s, want_ss[i])
