@@ -13,7 +13,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libpici_b200.so")
-SOURCES = ("api.cu", "compress.cu", "coo.cu", "expand.cu", "merge.cu", "misc.cu", "prune.cu", "ring.cu")
+SOURCES = ("api.cu", "compress.cu", "coo.cu", "expand.cu", "merge.cu", "misc.cu", "prune.cu", "ring.cu", "static_ws.cu")
 HEADERS = ("launch.h", "pici_common.cuh")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]

@@ -8,7 +8,7 @@ import re
 
 import pytest
 
-from paper_2607_04676_b200 import coo, pici, prune
+from paper_2607_04676_b200 import coo, pici, prune, static_ws
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -30,7 +30,7 @@ def test_every_declared_symbol_is_exported_and_bound():
     lib = pici.lib()
     for n in names:
         assert hasattr(lib, n), f"{n} is declared in include/pici.h but not exported"
-    assert set(names) == set(pici.EXPORTS) | set(coo.EXPORTS) | set(prune.EXPORTS), "the Python binding and the header disagree on the entry points"
+    assert set(names) == set(pici.EXPORTS) | set(coo.EXPORTS) | set(prune.EXPORTS) | set(static_ws.EXPORTS), "the Python binding and the header disagree on the entry points"
     assert lib.pici_version() == 100
     coo.lib()                                                # binds the pici_coo_* signatures
     L = prune.lib()
