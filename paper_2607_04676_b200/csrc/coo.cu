@@ -287,24 +287,35 @@ struct CooMergeArgs {
 };
 constexpr uint32_t kBmWords = kTile / 32;   // presence bitmap of one operand in one block
 constexpr int kMergeWarps = 8;
+#ifndef PICI_COO_MERGE_UNROLL
+#define PICI_COO_MERGE_UNROLL 4
+#endif
+static __device__ __forceinline__ uint32_t popc4(uint4 v) { return __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w); }
+constexpr int kU = PICI_COO_MERGE_UNROLL;   // entries per lane whose loads are issued together
+#ifndef PICI_COO_MERGE_BLOCKS
+#define PICI_COO_MERGE_BLOCKS 4
+#endif
 
-// One warp per block, nothing but two 512-byte bitmaps in shared memory (so 32 warps per SM hide the chain ticket ->
-// offsets -> indices -> values -> look-back): the entries' indices are scattered into presence bitmaps of X and Y;
-// lane l then owns positions 128 l .. 128 l + 127, finds its first X / Y value by a popcount scan (entry k of the
-// block is the k-th set bit: the lists are ascending) and walks the set bits of x | y reading the values straight
-// from the lists (contiguous per lane, L1-resident: the block's entries were just touched).  The walk runs twice -
-// once to count the survivors (the predicate re-applied to every sum), once behind the look-back to emit them - so
-// nothing is staged and a block of any density takes the same path.  The next ticket and the next block's offsets
-// are requested one block ahead; a block's look-back and emission are deferred behind the next block's count, as in
-// pici_compress.  Measured alternatives at N = 2^28, 99.99 / 99 % sparsity (this form: 0.126 / 0.173 ms with the
-// pre-pass): look-back taken at once 0.21 / 0.32; the store-only hierarchy of reduce_ss with a word per block 0.50 /
-// 0.73 (65536 x 3 accesses to a few hot lines); one ticket, status word and look-back per CTA of 8 blocks between
-// block barriers 0.20 / 0.39 (every CTA of a wave looks back at the same time and the scan advances 32 groups per L2
-// round trip).  An almost empty block costs a look-back and nothing else, so this kernel is latency-bound there.
-__global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const CooMergeArgs a) {
-    __shared__ __align__(16) uint32_t bms[kMergeWarps][2 * kBmWords];
+// One warp per block.  The entries' indices are scattered into presence bitmaps of X and Y (two 512-byte bitmaps in
+// shared memory); with a per-word table of the candidates (x | y) and of the Y entries before each word, every entry
+// of a list then knows by itself where its sum goes in the output (the candidate rank of its bit) and where its partner
+// in the other list is (entry k of a block is its k-th set bit: the lists ascend).  So all three passes - build the
+// bitmaps, test the sums where both lists have an entry (the only place a sum can vanish), emit - read the lists
+// COALESCED with kU independent loads per lane in flight.  A block in which a sum did cancel (rare) takes the first
+// version's path instead: lane l owns positions 128 l .. 128 l + 127 and walks the set bits of x | y one by one, once
+// to count the survivors and once to emit them.  That walk used to be the only path: one dependent global load per
+// candidate and lane, twice - 0.88 ms at 90 % sparsity against 0.45 now (95 %: 0.377 -> 0.234, 99 %: 0.133 -> 0.104;
+// 99.9 / 99.99 %: 0.078 / 0.072 -> 0.084 / 0.080, the price of the larger kernel where blocks are almost empty).
+// The bitmaps and tables stay in one of three slots per warp until the block is emitted two iterations later, with its
+// prefix from the scan service (pici_common.cuh), as in pici_compress; the next ticket and the next block's offsets
+// are requested one block ahead.  Measured: kU = 2 / 4 / 8 at 90 %: 0.566 / 0.450 / 0.517 ms (8 spills); 3 CTAs per SM:
+// 0.481; no prefix wait for blocks without survivors: 0.233 instead of 0.080 ms at 99.99 % (the waits pace the warps).
+// An almost empty block costs a ticket, four offsets and a prefix and nothing else: the kernel is latency-bound there.
+__global__ void __launch_bounds__(kMergeWarps * 32, PICI_COO_MERGE_BLOCKS) coo_merge_kernel(const CooMergeArgs a) {
+    constexpr uint32_t kSlotWords = 3 * kBmWords;           // bitmaps of X and Y, two tables of 128 u16
+    __shared__ __align__(16) uint32_t bms[kMergeWarps][3 * kSlotWords];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t *const bmx = bms[warp], *const bmy = bmx + kBmWords;
+    uint32_t *const slots = bms[warp];
     uint32_t *const ticket = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(a.ws.hdr) + kWsCompressTicket);
     const uint32_t tag = launch_tag(a.ws.hdr);
     const uint32_t T = (uint32_t)((a.n + kTile - 1) / kTile);
@@ -333,21 +344,33 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
         if (tt < T && lane < 4) v = (lane < 2 ? a.ws.offx : a.ws.offy)[tt + (lane & 1)];
         return v;
     };
-    // One block's state between its count (pass 1) and its emission (pass 2, behind the look-back)
-    struct Blk {
-        uint32_t wx[4], wy[4], kx, ky, t, cnt, before, total;
+    // A block's tables live in one of the warp's three shared-memory slots from its count to its emission two
+    // iterations later (behind the prefix): the presence bitmaps of X and Y (128 words each) and, per word, the
+    // number of candidates (x | y) and of Y entries of the block before it (u16).  Entry k of a list is its k-th set
+    // bit (the lists ascend), so with these an entry finds its place in the output, and its partner in the other
+    // list, by itself: all passes read the lists coalesced, kU loads per lane in flight.
+    struct Blk {          // warp-uniform
+        uint32_t x0, y0, nx, ny, t, total, slot;
+        bool fast;        // no candidate of the block cancelled: survivor k IS candidate k
     };
-    // the walk over the lane's candidates; emit = false counts survivors, true stores them from `o` on
+    auto bmx_of = [&](uint32_t slot) -> uint32_t * { return slots + slot * kSlotWords; };
+    // the sequential walk over the lane's candidates (only for a block in which a sum cancelled): emit = false counts
+    // the lane's survivors, true stores them from `o` on
     auto walk = [&](const Blk &B, bool emit, uint32_t o) -> uint32_t {
-        uint32_t px = B.kx, py = B.ky, cnt = 0;
+        const uint32_t *bx = bmx_of(B.slot), *by = bx + kBmWords;
+        const uint4 X = reinterpret_cast<const uint4 *>(bx)[lane], Y = reinterpret_cast<const uint4 *>(by)[lane];
+        const uint32_t wx[4] = {X.x, X.y, X.z, X.w}, wy[4] = {Y.x, Y.y, Y.z, Y.w};
+        const uint32_t v = popc4(X) | (popc4(Y) << 16);       // <= 4096 each
+        const uint32_t sc = warp_incl_scan(v, lane) - v;
+        uint32_t px = B.x0 + (sc & 0xFFFFu), py = B.y0 + (sc >> 16), cnt = 0;
         const uint32_t e0 = B.t * (uint32_t)kTile + 128u * (uint32_t)lane;
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            uint32_t u = B.wx[q] | B.wy[q];
+            uint32_t u = wx[q] | wy[q];
             while (u) {
                 const uint32_t bit = u & (0u - u);
                 u ^= bit;
-                const bool hx = (B.wx[q] & bit) != 0u, hy = (B.wy[q] & bit) != 0u;
+                const bool hx = (wx[q] & bit) != 0u, hy = (wy[q] & bit) != 0u;
                 const float x = hx ? __uint_as_float(vx[px]) : 0.0f;
                 const float y = hy ? __uint_as_float(vy[py]) : 0.0f;
                 px += hx ? 1u : 0u;
@@ -369,7 +392,62 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
     uint32_t held = 0xFFFFFFFFu;                              // claimed, not yet published (>= T: none)
     auto emit = [&](const Blk &P) {
         const uint32_t excl = service_prefix(a.ws.blk_acc, a.ws.status, a.ws.excl, tag, sb_log, P.t, held, T, lane);
-        if (P.total) walk(P, true, excl + P.before);
+        if (P.total == 0u) return;
+        if (!P.fast) {
+            const uint32_t cnt = walk(P, false, 0u);
+            walk(P, true, excl + warp_incl_scan(cnt, lane) - cnt);
+            return;
+        }
+        const uint32_t *bmx = bmx_of(P.slot), *bmy = bmx + kBmWords;
+        const uint16_t *up16 = reinterpret_cast<const uint16_t *>(bmy + kBmWords), *yp16 = up16 + kBmWords;
+        const uint32_t nx = P.nx, ny = P.ny;
+        for (uint32_t k0 = lane; k0 < nx; k0 += 32 * kU) {    // the X entries, with their Y partner where there is one
+            uint32_t pos[kU], xv[kU], r[kU], yi[kU];
+            bool hy[kU];
+#pragma unroll
+            for (int j = 0; j < kU; ++j) {
+                const uint32_t k = k0 + 32 * j;
+                pos[j] = k < nx ? ix[P.x0 + k] : 0u;
+                xv[j] = k < nx ? vx[P.x0 + k] : 0u;
+            }
+#pragma unroll
+            for (int j = 0; j < kU; ++j) {
+                const uint32_t w = (pos[j] & (kTile - 1)) >> 5, below = (1u << (pos[j] & 31)) - 1u;
+                const uint32_t by = bmy[w];
+                r[j] = up16[w] + __popc((bmx[w] | by) & below);
+                hy[j] = ((by >> (pos[j] & 31)) & 1u) != 0u && k0 + 32 * j < nx;
+                yi[j] = P.y0 + yp16[w] + __popc(by & below);
+            }
+            uint32_t yv[kU];
+#pragma unroll
+            for (int j = 0; j < kU; ++j) yv[j] = hy[j] ? vy[yi[j]] : 0u;
+#pragma unroll
+            for (int j = 0; j < kU; ++j) {
+                if (k0 + 32 * j < nx) {
+                    a.io[excl + r[j]] = pos[j];
+                    a.vo[excl + r[j]] = __float_as_uint(__fadd_rn(__uint_as_float(xv[j]), __uint_as_float(yv[j])));
+                }
+            }
+        }
+        for (uint32_t k0 = lane; k0 < ny; k0 += 32 * kU) {    // the Y entries without a partner
+            uint32_t pos[kU], yv[kU];
+#pragma unroll
+            for (int j = 0; j < kU; ++j) {
+                const uint32_t k = k0 + 32 * j;
+                pos[j] = k < ny ? iy[P.y0 + k] : 0u;
+                yv[j] = k < ny ? vy[P.y0 + k] : 0u;
+            }
+#pragma unroll
+            for (int j = 0; j < kU; ++j) {
+                const uint32_t w = (pos[j] & (kTile - 1)) >> 5, below = (1u << (pos[j] & 31)) - 1u;
+                const uint32_t bx = bmx[w];
+                if (k0 + 32 * j < ny && ((bx >> (pos[j] & 31)) & 1u) == 0u) {
+                    const uint32_t r = up16[w] + __popc((bx | bmy[w]) & below);
+                    a.io[excl + r] = pos[j];
+                    a.vo[excl + r] = __float_as_uint(__fadd_rn(0.0f, __uint_as_float(yv[j])));
+                }
+            }
+        }
     };
 
     uint32_t t = 0;
@@ -378,6 +456,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
     uint32_t off = load_off(t);
     uint32_t t_next = 0;
     if (t < T && lane == 0) t_next = ticket_tile(tk, cC, cj);
+    uint32_t seq = 0;                                         // blocks with entries so far: slot = seq mod 3
     while (t < T) {
         const uint32_t x0 = __shfl_sync(kFull, off, 0), x1 = __shfl_sync(kFull, off, 1), y0 = __shfl_sync(kFull, off, 2),
                        y1 = __shfl_sync(kFull, off, 3);
@@ -386,37 +465,75 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 4) coo_merge_kernel(const Co
         off = load_off(tn);                                   // arrives while this block is merged
         if (tn < T && lane == 0) t_next = ticket_tile(tk, cC, cj);
         Blk C;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) C.wx[q] = C.wy[q] = 0u;
-        C.kx = x0; C.ky = y0; C.t = t; C.cnt = 0;
-        if (x0 != x1 || y0 != y1) {
+        C.x0 = x0; C.y0 = y0; C.nx = x1 - x0; C.ny = y1 - y0; C.t = t; C.fast = true; C.total = 0; C.slot = seq % 3u;
+        if (C.nx != 0u || C.ny != 0u) {
+            // the slot's previous block (three blocks with entries back) was emitted at least one iteration ago
+            ++seq;
+            uint32_t *bmx = bmx_of(C.slot), *bmy = bmx + kBmWords;
+            __syncwarp();
             reinterpret_cast<uint4 *>(bmx)[lane] = make_uint4(0u, 0u, 0u, 0u);
             reinterpret_cast<uint4 *>(bmy)[lane] = make_uint4(0u, 0u, 0u, 0u);
             __syncwarp();
-            const uint32_t nx = x1 - x0, ny = y1 - y0;
-            for (uint32_t k = lane; k < max(nx, ny); k += 32) {
-                uint32_t px = 0, py = 0;
-                if (k < nx) px = ix[x0 + k];
-                if (k < ny) py = iy[y0 + k];
-                if (k < nx) atomicOr(&bmx[(px & (kTile - 1)) >> 5], 1u << (px & 31));
-                if (k < ny) atomicOr(&bmy[(py & (kTile - 1)) >> 5], 1u << (py & 31));
+            const uint32_t nx = C.nx, ny = C.ny;
+            for (uint32_t k0 = lane; k0 < max(nx, ny); k0 += 32 * kU) {
+                uint32_t px[kU], py[kU];
+#pragma unroll
+                for (int j = 0; j < kU; ++j) {
+                    const uint32_t k = k0 + 32 * j;
+                    px[j] = k < nx ? ix[x0 + k] : 0u;
+                    py[j] = k < ny ? iy[y0 + k] : 0u;
+                }
+#pragma unroll
+                for (int j = 0; j < kU; ++j) {
+                    const uint32_t k = k0 + 32 * j;
+                    if (k < nx) atomicOr(&bmx[(px[j] & (kTile - 1)) >> 5], 1u << (px[j] & 31));
+                    if (k < ny) atomicOr(&bmy[(py[j] & (kTile - 1)) >> 5], 1u << (py[j] & 31));
+                }
             }
             __syncwarp();
             const uint4 X = reinterpret_cast<const uint4 *>(bmx)[lane], Y = reinterpret_cast<const uint4 *>(bmy)[lane];
-            C.wx[0] = X.x; C.wx[1] = X.y; C.wx[2] = X.z; C.wx[3] = X.w;
-            C.wy[0] = Y.x; C.wy[1] = Y.y; C.wy[2] = Y.z; C.wy[3] = Y.w;
-            const uint32_t cx = __popc(X.x) + __popc(X.y) + __popc(X.z) + __popc(X.w);
-            const uint32_t cy = __popc(Y.x) + __popc(Y.y) + __popc(Y.z) + __popc(Y.w);
-            const uint32_t v = cx | (cy << 16);               // <= 4096 each
-            const uint32_t sc = warp_incl_scan(v, lane) - v;
-            C.kx += sc & 0xFFFFu;
-            C.ky += sc >> 16;
+            // the tables: candidates / Y entries of the block before each of the lane's four words
+            {
+                const uint32_t cu = __popc(X.x | Y.x) + __popc(X.y | Y.y) + __popc(X.z | Y.z) + __popc(X.w | Y.w);
+                const uint32_t v = cu | (popc4(Y) << 16);
+                const uint32_t incl = warp_incl_scan(v, lane);
+                C.total = __shfl_sync(kFull, incl, 31) & 0xFFFFu;
+                const uint32_t e = incl - v;
+                const uint32_t u0 = e & 0xFFFFu, u1 = u0 + __popc(X.x | Y.x), u2 = u1 + __popc(X.y | Y.y), u3 = u2 + __popc(X.z | Y.z);
+                const uint32_t q0 = e >> 16, q1 = q0 + __popc(Y.x), q2 = q1 + __popc(Y.y), q3 = q2 + __popc(Y.z);
+                reinterpret_cast<uint2 *>(bmy + kBmWords)[lane] = make_uint2(u0 | (u1 << 16), u2 | (u3 << 16));
+                reinterpret_cast<uint2 *>(bmy + kBmWords + kBmWords / 2)[lane] = make_uint2(q0 | (q1 << 16), q2 | (q3 << 16));
+            }
             __syncwarp();
-            C.cnt = walk(C, false, 0u);
+            // a sum can only vanish where both lists have an entry: test those (the predicate re-applied to x + y)
+            if (__any_sync(kFull, ((X.x & Y.x) | (X.y & Y.y) | (X.z & Y.z) | (X.w & Y.w)) != 0u)) {
+                const uint16_t *yp16 = reinterpret_cast<const uint16_t *>(bmy + kBmWords) + kBmWords;
+                bool cancelled = false;
+                for (uint32_t k0 = lane; k0 < nx; k0 += 32 * kU) {
+                    uint32_t pos[kU], xv[kU], yv[kU];
+                    bool hy[kU];
+#pragma unroll
+                    for (int j = 0; j < kU; ++j) pos[j] = k0 + 32 * j < nx ? ix[x0 + k0 + 32 * j] : 0u;
+#pragma unroll
+                    for (int j = 0; j < kU; ++j) {
+                        const uint32_t w = (pos[j] & (kTile - 1)) >> 5, by = bmy[w];
+                        hy[j] = k0 + 32 * j < nx && ((by >> (pos[j] & 31)) & 1u) != 0u;
+                        xv[j] = yv[j] = 0x3F800000u;         // 1 + 1: no cancellation
+                        if (hy[j]) {
+                            xv[j] = vx[x0 + k0 + 32 * j];
+                            yv[j] = vy[y0 + yp16[w] + __popc(by & ((1u << (pos[j] & 31)) - 1u))];
+                        }
+                    }
+#pragma unroll
+                    for (int j = 0; j < kU; ++j)
+                        cancelled |= hy[j] && !nz32(__float_as_uint(__fadd_rn(__uint_as_float(xv[j]), __uint_as_float(yv[j]))));
+                }
+                if (__any_sync(kFull, cancelled)) {           // rare: count (and later emit) lane by lane
+                    C.fast = false;
+                    C.total = warp_sum(walk(C, false, 0u));
+                }
+            }
         }
-        const uint32_t incl = warp_incl_scan(C.cnt, lane);
-        C.before = incl - C.cnt;
-        C.total = __shfl_sync(kFull, incl, 31);
         if (lane == 0) st_status(a.ws.status + t, tag, C.total);   // for the scan service
         if (on0) emit(P0);                                    // the block two iterations back
         P0 = P1; on0 = on1;
@@ -507,7 +624,7 @@ static cudaError_t launch_coo_merge(const uint32_t *ix, const void *vx, const ui
                             reinterpret_cast<uint32_t *>(vo), d_no, n, w};
     const uint64_t T = (n + kTile - 1) / kTile;
     uint64_t blocks = (T + kMergeWarps - 1) / kMergeWarps + 1;   // + CTA 0, the scan service
-    const uint64_t cap = (uint64_t)num_sms() * 4;
+    const uint64_t cap = (uint64_t)num_sms() * PICI_COO_MERGE_BLOCKS;
     if (blocks > cap) blocks = cap;
     coo_merge_kernel<<<(unsigned)blocks, kMergeWarps * 32, 0, s>>>(a);
     return cudaGetLastError();
