@@ -124,6 +124,13 @@ def test_coo_at_max_n(mods):
     ck.reduce_sd(cx, acc)
     x += 1.0
     assert torch.equal(acc.view(torch.int32), x.view(torch.int32))
+    del acc, x
+    # the merge at this size: X + X (every entry has a partner, nothing cancels) = the same indices, doubled values
+    co_ = ck.alloc_coo(N)
+    ck.reduce_ss(cx, cx, co_, ws)
+    assert co_.nnz_host() == nx
+    assert torch.equal(co_.idx[:nx], cx.idx[:nx])
+    assert torch.equal(co_.val[:nx], cx.val[:nx] * 2.0)
 
 
 def test_pici_bf16_at_max_n(mods):
